@@ -1,0 +1,163 @@
+/*
+ * nsfrb.h -- C ABI of the B200-native NSFRB image-plane single-pulse search.
+ *
+ * The library computes the search stage of the DSA-110 NSFRB pipeline ("cerberus",
+ * arxiv 2510.18136 sec. 2.2): per-pixel incoherent dedispersion of a
+ * stack of sub-band images over trial DMs, boxcar matched filter over trial widths,
+ * S/N normalisation by the per-(pixel, DM) standard deviation, maximum S/N and its time
+ * of arrival, and a thresholded candidate list.  Where the paper is silent the readings
+ * R1..R23 in DESIGN.md apply.  Every step runs in CUDA kernels for sm_100a; there is no
+ * CPU fallback.
+ *
+ * Notation: npix = nx*ny, pixel p = y*nx + x; cube I[c][t][p] float32, pixel-contiguous,
+ * index (c*nt + t)*npix + p.  For DM trial k and channel c the integer delay is
+ *     d[k][c] = floor(((4.15e-3*dm[k]) * (f[c]^-2 - f_ref^-2)) / tsamp + 0.5), f_ref = max f
+ * (PAPER.md:L83 dispersion constant, L98 integer shift table), T_k = nt - max_c d[k][c].
+ *     D_k[t] = sum_c I[c][t+d[k][c]][p]            0 <= t < T_k
+ *     S(k,j,t) = sum_{u=t}^{t+w_j-1} (D_k[u]-mu_k) / (sigma_k*sqrt(w_j)),  0 <= t <= T_k-w_j
+ * with mu_k, sigma_k the mean and population standard deviation of D_k over all valid t
+ * (S = 0 where sigma_k = 0).  Outputs per pixel: snr = max S, argmax = lexicographically
+ * smallest (k, j, t) attaining it; candidates = pixels with snr > threshold (strict).
+ *
+ * Threading: a plan serves one call at a time.  Calls enqueue work on the given stream and
+ * return; outputs are valid once the caller has synchronised that stream.  No call
+ * synchronises the device except nsfrb_plan_create/destroy and the *_host variants.
+ * Errors: 0 on success, negative code otherwise; nsfrb_last_error() gives the text.
+ */
+#ifndef NSFRB_H
+#define NSFRB_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NSFRB_OK 0
+#define NSFRB_EINVAL (-1) /* bad argument (null, non-positive size, bad list, misaligned) */
+#define NSFRB_ENOMEM (-2) /* device or host allocation failed / does not fit shared memory */
+#define NSFRB_ECUDA (-3)  /* CUDA runtime error; message holds cudaGetErrorString          */
+#define NSFRB_ESTATE (-4) /* call not allowed in the plan's state (see nsfrb_search)        */
+
+typedef struct nsfrb_plan nsfrb_plan; /* opaque; owns tables, workspace, ring */
+
+/* One candidate: a pixel whose peak S/N exceeds the threshold ("A nominal
+ * 6 sigma S/N threshold is imposed to identify candidates"; L146 one per time series). */
+typedef struct {
+    int32_t pixel;     /* y*nx + x                                        */
+    int32_t dm_idx;    /* index into dm_list (lowest index among duplicates) */
+    int32_t width_idx; /* index into width_list                            */
+    int32_t t;         /* window start, reference-frequency frame          */
+    float snr;
+} nsfrb_cand;
+
+/* Sizes and launch facts of a plan, for harnesses (all host values). */
+typedef struct {
+    int32_t npix, nchan, nt, ndm, nwidth;
+    int32_t ndm_unique;        /* distinct delay vectors actually searched           */
+    int32_t dmax;              /* largest delay in the table, samples                */
+    int32_t wmax;              /* largest width                                      */
+    int32_t n_groups;          /* DM groups per pixel (one CTA each)                 */
+    int32_t n_width_batches;   /* width batches per pixel (<= 32 widths each)        */
+    int32_t series_per_cta;    /* DM trials one CTA holds on chip                    */
+    int32_t block_len;         /* dedispersed samples per time block                 */
+    int32_t ring_len;          /* prefix-sum history kept per series in shared memory */
+    int32_t search_threads;    /* threads per CTA of the search kernel               */
+    int64_t search_smem_bytes; /* dynamic shared memory per CTA                      */
+    int64_t workspace_bytes;   /* device bytes owned by the plan                     */
+    int64_t cells_per_pixel;   /* offline: sum_k sum_j max(0, T_k - w_j + 1), all ndm */
+    int64_t shift_adds_per_pixel; /* offline: nchan * sum_k T_k, all ndm            */
+} nsfrb_plan_info;
+
+/*
+ * Create a plan (DM trials, widths and the shift table are fixed ahead of
+ * the search and kept on the GPU).
+ *   nx, ny, nchan > 0; nt > 0 is the cube length for nsfrb_search and the ring length L
+ *   for nsfrb_stream_push.  freqs_GHz: host [nchan], finite, > 0, any order.  tsamp_s > 0.
+ *   dm_list: host [ndm], finite, >= 0.  width_list: host [nwidth], each >= 1, distinct.
+ *   Every trial must keep at least one sample: nt > max_c d[k][c] for all k.
+ * All host arrays are copied.  The plan allocates nchan*nt*npix*4 B of device workspace
+ * (the time-contiguous copy of the cube, which doubles as the streaming ring) plus small
+ * tables, on the current CUDA device.
+ */
+int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt,
+                      const double *freqs_GHz, double tsamp_s,
+                      const double *dm_list, int ndm,
+                      const int32_t *width_list, int nwidth, float threshold);
+
+/*
+ * Offline search of one cube (definition at the top of this file).
+ *   cube      device, [nchan][nt][npix] float32, 16-byte aligned, read only
+ *   stream    cudaStream_t (NULL = legacy default stream)
+ *   snr_map   device, [npix] float32.  -INFINITY where no cell is defined
+ *   argmax    device, [3][npix] int32: dm_idx | width_idx | t ; (-1,-1,-1) where no cell
+ *   cands     device, [cand_capacity]; may be NULL iff cand_capacity == 0; order arbitrary
+ *   ncands    device, 1: total number of candidates found (may exceed cand_capacity, in
+ *             which case only cand_capacity of them are stored -- not an error)
+ * Returns NSFRB_ESTATE if the plan has received stream pushes (call nsfrb_stream_reset).
+ * Non-finite input values give unspecified results.
+ */
+int nsfrb_search(nsfrb_plan *plan, const float *cube, void *stream,
+                 float *snr_map, int32_t *argmax,
+                 nsfrb_cand *cands, uint32_t cand_capacity, uint32_t *ncands);
+
+/*
+ * Real-time mode (25-sample chunks arrive every 3.35 s and must be
+ * searched as they arrive).  Appends chunk [nchan][chunk_nt][npix] (device, 16-byte
+ * aligned) to the plan's ring of the last nt samples and searches it:
+ *   n_prev -> n = n_prev + chunk_nt samples received; ring = samples [lo, n), lo = max(0, n-nt)
+ *   mu_k, sigma_k span every valid sample of the ring; only windows whose LAST raw sample
+ *   arrived in this push are evaluated: n_prev <= t + w_j - 1 + dmax_k < n, t >= lo;
+ *   reported t is the absolute sample index since the first push (mod 2^31).
+ * 1 <= chunk_nt <= nt.  Outputs as nsfrb_search.
+ */
+int nsfrb_stream_push(nsfrb_plan *plan, const float *chunk, int chunk_nt, void *stream,
+                      float *snr_map, int32_t *argmax,
+                      nsfrb_cand *cands, uint32_t cand_capacity, uint32_t *ncands);
+
+/* Forget all pushed samples; the plan can be used for nsfrb_search again. */
+int nsfrb_stream_reset(nsfrb_plan *plan);
+
+/*
+ * Same calls with HOST buffers (pinned memory recommended): the library copies the input
+ * host->device, runs the search, copies snr_map/argmax/cands/ncands device->host on
+ * `stream` and synchronises it before returning.  Staging buffers belong to the plan.
+ */
+int nsfrb_search_host(nsfrb_plan *plan, const float *cube_host, void *stream,
+                      float *snr_map_host, int32_t *argmax_host,
+                      nsfrb_cand *cands_host, uint32_t cand_capacity, uint32_t *ncands_host);
+int nsfrb_stream_push_host(nsfrb_plan *plan, const float *chunk_host, int chunk_nt, void *stream,
+                           float *snr_map_host, int32_t *argmax_host,
+                           nsfrb_cand *cands_host, uint32_t cand_capacity, uint32_t *ncands_host);
+
+/* Release everything the plan owns.  NULL is a no-op returning 0. */
+int nsfrb_plan_destroy(nsfrb_plan *plan);
+
+/* Copy the integer delay table to host memory out[ndm][nchan] (bit-exact parity check). */
+int nsfrb_plan_get_delays(const nsfrb_plan *plan, int32_t *out);
+
+/* Fill *info. */
+int nsfrb_plan_get_info(const nsfrb_plan *plan, nsfrb_plan_info *info);
+
+/* Number of kernel launches the last nsfrb_search / nsfrb_stream_push enqueued. */
+int nsfrb_plan_last_launches(const nsfrb_plan *plan);
+
+/*
+ * Per-kernel device timing for harnesses.  With profiling on, every call records CUDA events
+ * on its stream around each kernel it enqueues.  nsfrb_plan_get_kernel_ms waits for the last
+ * call's events and writes the milliseconds of out[0] = layout kernel (transpose or ring push),
+ * out[1] = search kernel, out[2] = finalize kernel, out[3] = candidate compaction.
+ */
+int nsfrb_plan_set_profiling(nsfrb_plan *plan, int on);
+int nsfrb_plan_get_kernel_ms(nsfrb_plan *plan, float out[4]);
+
+/* Thread-local text of the last error; never NULL. */
+const char *nsfrb_last_error(void);
+
+/* "major.minor (build tag)". */
+const char *nsfrb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NSFRB_H */

@@ -5,7 +5,7 @@
  * search computes (arxiv 2510.18136, "cerberus" search stage).  Only tests/,
  * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
  * load this file.  It shares no code, header, table or constant with the CUDA path
- * in paper_2510_18136_b200/csrc/.
+ * (the csrc/ directory of the product package).
  *
  * What the paper fixes (PAPER.md = /root/reference/PAPER.md):
  *   - L73-L75 (sec. 2.2): images are de-dispersed over trial DMs with pre-computed

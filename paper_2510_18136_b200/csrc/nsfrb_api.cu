@@ -1,0 +1,480 @@
+// C ABI (include/nsfrb.h) and the host-side plan: validation, delay table (a0), trial
+// de-duplication and grouping, workspace, launch sequencing.  All arithmetic of the search
+// itself is in nsfrb_kernels.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <string>
+#include <vector>
+
+#include "nsfrb_internal.h"
+
+using namespace nsfrb;
+
+namespace {
+
+thread_local std::string g_err = "";
+
+int fail(int code, const std::string &msg)
+{
+    g_err = msg;
+    return code;
+}
+int fail_cuda(cudaError_t e, const char *what)
+{
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    cudaGetLastError(); // clear non-sticky error state
+    return NSFRB_ECUDA;
+}
+#define CU(call, what)                                         \
+    do {                                                       \
+        cudaError_t e__ = (call);                              \
+        if (e__ != cudaSuccess) return fail_cuda(e__, what);   \
+    } while (0)
+
+inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+constexpr size_t kMaxSmem = 227 * 1024; // opt-in dynamic shared memory per CTA on sm_100
+
+} // namespace
+
+struct nsfrb_plan {
+    int nx = 0, ny = 0, npix = 0, nchan = 0, nt = 0, ndm = 0, nw = 0;
+    double tsamp = 0;
+    float threshold = 0;
+    std::vector<double> freqs, dms;
+    std::vector<int32_t> widths;
+    std::vector<int32_t> delays; // [ndm][nchan]
+    std::vector<int32_t> dmax;   // [ndm]
+    // unique trials, sorted by (dmax, first original index)
+    int nuniq = 0;
+    std::vector<int32_t> k_of_u, dmax_u, delays_u;
+    // widths that can hold at least one cell for some trial, original order
+    int nw_used = 0;
+    std::vector<int32_t> widths_used, j_of_used;
+    int wmax_used = 0, dmax_all = 0, dmin_all = 0;
+    int n_groups = 0, n_wb = 0, H = 0, RS = 0, pitch = 0;
+    size_t smem_search = 0, smem_final = 0;
+    int64_t cells_per_pixel = 0, shift_adds_per_pixel = 0;
+    // device
+    float *d_W = nullptr;
+    float *d_base = nullptr;
+    int32_t *d_delays_u = nullptr, *d_dmax_u = nullptr, *d_k_of_u = nullptr, *d_widths = nullptr, *d_j_of_used = nullptr;
+    Partial *d_partials = nullptr;
+    size_t workspace_bytes = 0;
+    // streaming state
+    int64_t n_received = 0;
+    // host-variant staging
+    float *d_in = nullptr;
+    size_t d_in_bytes = 0;
+    float *d_snr = nullptr;
+    int32_t *d_arg = nullptr;
+    nsfrb_cand *d_cands = nullptr;
+    uint32_t d_cands_cap = 0;
+    uint32_t *d_ncands = nullptr;
+    int last_launches = 0;
+    int device = 0;
+    // optional per-kernel timing
+    bool profiling = false;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
+};
+
+namespace {
+
+void free_plan(nsfrb_plan *p)
+{
+    if (!p) return;
+    cudaFree(p->d_W); cudaFree(p->d_base); cudaFree(p->d_delays_u); cudaFree(p->d_dmax_u); cudaFree(p->d_k_of_u);
+    cudaFree(p->d_widths); cudaFree(p->d_j_of_used); cudaFree(p->d_partials); cudaFree(p->d_in); cudaFree(p->d_snr);
+    cudaFree(p->d_arg); cudaFree(p->d_cands); cudaFree(p->d_ncands);
+    for (auto &e : p->ev) if (e) cudaEventDestroy(e);
+    cudaGetLastError();
+    delete p;
+}
+
+template <typename T>
+cudaError_t upload(T **dst, const std::vector<T> &src, size_t *acc)
+{
+    const size_t bytes = std::max<size_t>(src.size(), 1) * sizeof(T);
+    cudaError_t e = cudaMalloc(reinterpret_cast<void **>(dst), bytes);
+    if (e != cudaSuccess) return e;
+    *acc += bytes;
+    if (!src.empty()) e = cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice);
+    return e;
+}
+
+inline void mark(nsfrb_plan *pl, int i, cudaStream_t st)
+{
+    if (pl->profiling && pl->ev[i]) cudaEventRecord(pl->ev[i], st);
+}
+
+// Enqueue search + finalize + compaction over the workspace as it stands.
+int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offset, cudaStream_t st, float *snr_map,
+               int32_t *argmax, nsfrb_cand *cands, uint32_t cap, uint32_t *ncands, int *launches)
+{
+    const int slices = (pl->nw_used > 0) ? pl->n_groups * pl->n_wb : 0;
+    if (slices > 0) {
+        SearchParams sp;
+        sp.W = pl->d_W; sp.delays_u = pl->d_delays_u; sp.dmax_u = pl->d_dmax_u; sp.k_of_u = pl->d_k_of_u;
+        sp.widths = pl->d_widths; sp.partials = pl->d_partials;
+        sp.npix = pl->npix; sp.nchan = pl->nchan; sp.pitch = pl->pitch; sp.ring_L = pl->nt;
+        sp.origin = origin; sp.len = len; sp.raw_end_min = raw_end_min;
+        sp.nuniq = pl->nuniq; sp.nw = pl->nw_used; sp.n_groups = pl->n_groups; sp.n_wb = pl->n_wb;
+        sp.H = pl->H; sp.RS = pl->RS; sp.wmax = pl->wmax_used;
+        CU(launch_search(sp, pl->smem_search, st), "k_search launch");
+        ++*launches;
+    }
+    mark(pl, 2, st);
+    FinalParams fp;
+    fp.W = pl->d_W; fp.delays_u = pl->d_delays_u; fp.dmax_u = pl->d_dmax_u; fp.widths = pl->d_widths;
+    fp.partials = pl->d_partials; fp.snr_map = snr_map; fp.argmax = argmax;
+    fp.npix = pl->npix; fp.nchan = pl->nchan; fp.pitch = pl->pitch; fp.ring_L = pl->nt;
+    fp.origin = origin; fp.len = len; fp.raw_end_min = raw_end_min; fp.slices = slices; fp.t_offset = t_offset;
+    fp.j_of_used = pl->d_j_of_used;
+    CU(launch_finalize(fp, pl->smem_final, st), "k_finalize launch");
+    ++*launches;
+    mark(pl, 3, st);
+    CU(cudaMemsetAsync(ncands, 0, sizeof(uint32_t), st), "memset ncands");
+    CU(launch_compact(snr_map, argmax, pl->npix, pl->threshold, cands, cap, ncands, st), "k_compact launch");
+    ++*launches;
+    mark(pl, 4, st);
+    pl->ev_valid = pl->profiling;
+    return NSFRB_OK;
+}
+
+int check_outputs(const void *snr_map, const void *argmax, const void *cands, uint32_t cap, const void *ncands)
+{
+    if (!snr_map || !argmax || !ncands) return fail(NSFRB_EINVAL, "null output pointer");
+    if (cap > 0 && !cands) return fail(NSFRB_EINVAL, "cands is null but cand_capacity > 0");
+    return NSFRB_OK;
+}
+
+int ensure_host_staging(nsfrb_plan *pl, size_t in_bytes, uint32_t cap)
+{
+    if (pl->d_in_bytes < in_bytes) {
+        cudaFree(pl->d_in); pl->d_in = nullptr; pl->d_in_bytes = 0;
+        CU(cudaMalloc(reinterpret_cast<void **>(&pl->d_in), in_bytes), "staging input alloc");
+        pl->d_in_bytes = in_bytes;
+    }
+    if (!pl->d_snr) CU(cudaMalloc(reinterpret_cast<void **>(&pl->d_snr), (size_t)pl->npix * sizeof(float)), "staging snr alloc");
+    if (!pl->d_arg) CU(cudaMalloc(reinterpret_cast<void **>(&pl->d_arg), 3 * (size_t)pl->npix * sizeof(int32_t)), "staging argmax alloc");
+    if (!pl->d_ncands) CU(cudaMalloc(reinterpret_cast<void **>(&pl->d_ncands), sizeof(uint32_t)), "staging ncands alloc");
+    if (cap > pl->d_cands_cap) {
+        cudaFree(pl->d_cands); pl->d_cands = nullptr; pl->d_cands_cap = 0;
+        CU(cudaMalloc(reinterpret_cast<void **>(&pl->d_cands), (size_t)cap * sizeof(nsfrb_cand)), "staging cands alloc");
+        pl->d_cands_cap = cap;
+    }
+    return NSFRB_OK;
+}
+
+int copy_back(nsfrb_plan *pl, cudaStream_t st, float *snr_h, int32_t *arg_h, nsfrb_cand *cands_h, uint32_t cap,
+              uint32_t *ncands_h)
+{
+    CU(cudaMemcpyAsync(snr_h, pl->d_snr, (size_t)pl->npix * sizeof(float), cudaMemcpyDeviceToHost, st), "D2H snr");
+    CU(cudaMemcpyAsync(arg_h, pl->d_arg, 3 * (size_t)pl->npix * sizeof(int32_t), cudaMemcpyDeviceToHost, st), "D2H argmax");
+    CU(cudaMemcpyAsync(ncands_h, pl->d_ncands, sizeof(uint32_t), cudaMemcpyDeviceToHost, st), "D2H ncands");
+    CU(cudaStreamSynchronize(st), "stream sync");
+    const uint32_t n = std::min(*ncands_h, cap);
+    if (n > 0) {
+        CU(cudaMemcpyAsync(cands_h, pl->d_cands, (size_t)n * sizeof(nsfrb_cand), cudaMemcpyDeviceToHost, st), "D2H cands");
+        CU(cudaStreamSynchronize(st), "stream sync");
+    }
+    return NSFRB_OK;
+}
+
+} // namespace
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+const char *nsfrb_last_error(void) { return g_err.c_str(); }
+const char *nsfrb_version(void) { return "0.1 (sm_100a)"; }
+
+int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
+                      const double *dm_list, int ndm, const int32_t *width_list, int nwidth, float threshold)
+{
+    if (!out) return fail(NSFRB_EINVAL, "out is null");
+    *out = nullptr;
+    if (!freqs_GHz || !dm_list || !width_list) return fail(NSFRB_EINVAL, "null input list");
+    if (nx < 1 || ny < 1 || nchan < 1 || nt < 1 || ndm < 1 || nwidth < 1) return fail(NSFRB_EINVAL, "non-positive size");
+    if ((long long)nx * ny > 0x7fffffffLL / 4) return fail(NSFRB_EINVAL, "image too large");
+    if (!(tsamp_s > 0.0) || !std::isfinite(tsamp_s)) return fail(NSFRB_EINVAL, "tsamp_s must be finite and > 0");
+    if (!std::isfinite(threshold) && !(threshold == INFINITY || threshold == -INFINITY))
+        return fail(NSFRB_EINVAL, "threshold is NaN");
+    for (int c = 0; c < nchan; ++c)
+        if (!std::isfinite(freqs_GHz[c]) || !(freqs_GHz[c] > 0.0)) return fail(NSFRB_EINVAL, "freqs_GHz must be finite and > 0");
+    for (int k = 0; k < ndm; ++k)
+        if (!std::isfinite(dm_list[k]) || dm_list[k] < 0.0) return fail(NSFRB_EINVAL, "dm_list must be finite and >= 0");
+    for (int j = 0; j < nwidth; ++j) {
+        if (width_list[j] < 1) return fail(NSFRB_EINVAL, "width < 1");
+        for (int i = 0; i < j; ++i)
+            if (width_list[i] == width_list[j]) return fail(NSFRB_EINVAL, "duplicate width");
+    }
+
+    nsfrb_plan *pl = new (std::nothrow) nsfrb_plan();
+    if (!pl) return fail(NSFRB_ENOMEM, "host allocation failed");
+    pl->nx = nx; pl->ny = ny; pl->npix = nx * ny; pl->nchan = nchan; pl->nt = nt; pl->ndm = ndm; pl->nw = nwidth;
+    pl->tsamp = tsamp_s; pl->threshold = threshold;
+    pl->freqs.assign(freqs_GHz, freqs_GHz + nchan);
+    pl->dms.assign(dm_list, dm_list + ndm);
+    pl->widths.assign(width_list, width_list + nwidth);
+
+    // ---- a0: delay table, float64 on the host (include/nsfrb.h formula)
+    double f_ref = freqs_GHz[0];
+    for (int c = 1; c < nchan; ++c) f_ref = std::max(f_ref, freqs_GHz[c]);
+    const double inv_ref2 = 1.0 / (f_ref * f_ref);
+    pl->delays.resize((size_t)ndm * nchan);
+    pl->dmax.resize(ndm);
+    for (int k = 0; k < ndm; ++k) {
+        const double scale = 4.15e-3 * dm_list[k];
+        int mx = 0;
+        for (int c = 0; c < nchan; ++c) {
+            const double inv2 = 1.0 / (freqs_GHz[c] * freqs_GHz[c]);
+            const double x = (scale * (inv2 - inv_ref2)) / tsamp_s;
+            const double r = std::floor(x + 0.5);
+            if (!(r < (double)nt)) {
+                free_plan(pl);
+                return fail(NSFRB_EINVAL, "a trial's delay reaches nt: no valid sample left (nt <= dmax_k)");
+            }
+            const int d = (int)r;
+            pl->delays[(size_t)k * nchan + c] = d;
+            mx = std::max(mx, d);
+        }
+        pl->dmax[k] = mx;
+    }
+
+    // ---- unique delay vectors (a duplicate can never win under the lowest-index tie-break)
+    std::vector<int> first;
+    for (int k = 0; k < ndm; ++k) {
+        bool dup = false;
+        for (int u : first)
+            if (std::memcmp(&pl->delays[(size_t)u * nchan], &pl->delays[(size_t)k * nchan], sizeof(int32_t) * nchan) == 0) {
+                dup = true;
+                break;
+            }
+        if (!dup) first.push_back(k);
+    }
+    std::stable_sort(first.begin(), first.end(), [&](int a, int b) { return pl->dmax[a] < pl->dmax[b]; });
+    pl->nuniq = (int)first.size();
+    for (int k : first) {
+        pl->k_of_u.push_back(k);
+        pl->dmax_u.push_back(pl->dmax[k]);
+        pl->delays_u.insert(pl->delays_u.end(), pl->delays.begin() + (size_t)k * nchan,
+                            pl->delays.begin() + (size_t)(k + 1) * nchan);
+    }
+    pl->dmax_all = *std::max_element(pl->dmax.begin(), pl->dmax.end());
+    pl->dmin_all = *std::min_element(pl->dmax.begin(), pl->dmax.end());
+
+    // ---- widths that can hold a cell for at least one trial
+    const int T_longest = nt - pl->dmin_all;
+    for (int j = 0; j < nwidth; ++j)
+        if (width_list[j] <= T_longest) {
+            pl->widths_used.push_back(width_list[j]);
+            pl->j_of_used.push_back(j);
+            pl->wmax_used = std::max(pl->wmax_used, width_list[j]);
+        }
+    pl->nw_used = (int)pl->widths_used.size();
+
+    for (int k = 0; k < ndm; ++k) {
+        const int T = nt - pl->dmax[k];
+        pl->shift_adds_per_pixel += (int64_t)nchan * T;
+        for (int j = 0; j < nwidth; ++j)
+            if (T - width_list[j] + 1 > 0) pl->cells_per_pixel += T - width_list[j] + 1;
+    }
+
+    // ---- kernel geometry
+    pl->n_groups = (pl->nuniq + kSearchWarps - 1) / kSearchWarps;
+    pl->n_wb = std::max(1, (pl->nw_used + kWidthBatch - 1) / kWidthBatch);
+    pl->H = round_up(std::max(pl->wmax_used, 1) + kBlockLen, 32);
+    pl->RS = round_up(kBlockLen + pl->dmax_all, 4);
+    pl->pitch = round_up(nt, 4);
+    pl->smem_search = search_smem_bytes(nchan, pl->RS, pl->H);
+    pl->smem_final = final_smem_bytes(nt);
+    if (pl->smem_search > kMaxSmem || pl->smem_final > kMaxSmem) {
+        char buf[256];
+        snprintf(buf, sizeof buf,
+                 "problem does not fit shared memory: search needs %zu B (nchan*%d + %d*%d floats), finalize %zu B; limit %zu B",
+                 pl->smem_search, pl->RS, kSearchWarps, pl->H, pl->smem_final, kMaxSmem);
+        free_plan(pl);
+        return fail(NSFRB_ENOMEM, buf);
+    }
+    if ((long long)pl->npix * pl->n_groups * pl->n_wb > 0x7fffffffLL) {
+        free_plan(pl);
+        return fail(NSFRB_EINVAL, "too many (pixel, DM group, width batch) tasks for one launch");
+    }
+
+    // ---- device state
+    cudaError_t e = cudaGetDevice(&pl->device);
+    if (e == cudaSuccess) e = configure_kernels(pl->smem_search, pl->smem_final);
+    size_t acc = 0;
+    if (e == cudaSuccess) e = upload(&pl->d_delays_u, pl->delays_u, &acc);
+    if (e == cudaSuccess) e = upload(&pl->d_dmax_u, pl->dmax_u, &acc);
+    if (e == cudaSuccess) e = upload(&pl->d_k_of_u, pl->k_of_u, &acc);
+    if (e == cudaSuccess) e = upload(&pl->d_widths, pl->widths_used, &acc);
+    if (e == cudaSuccess) e = upload(&pl->d_j_of_used, pl->j_of_used, &acc);
+    if (e == cudaSuccess) {
+        const size_t wb = (size_t)pl->npix * nchan * (size_t)pl->pitch * sizeof(float);
+        e = cudaMalloc(reinterpret_cast<void **>(&pl->d_W), wb);
+        if (e == cudaSuccess) { acc += wb; e = cudaMemset(pl->d_W, 0, wb); }
+    }
+    if (e == cudaSuccess) {
+        const size_t pb = (size_t)pl->npix * pl->n_groups * pl->n_wb * sizeof(Partial);
+        e = cudaMalloc(reinterpret_cast<void **>(&pl->d_partials), pb);
+        acc += pb;
+    }
+    if (e == cudaSuccess) {
+        const size_t bb = (size_t)pl->npix * nchan * sizeof(float);
+        e = cudaMalloc(reinterpret_cast<void **>(&pl->d_base), bb);
+        acc += bb;
+    }
+    if (e != cudaSuccess) {
+        const int code = (e == cudaErrorMemoryAllocation) ? NSFRB_ENOMEM : NSFRB_ECUDA;
+        std::string msg = std::string("plan device setup: ") + cudaGetErrorString(e);
+        cudaGetLastError();
+        free_plan(pl);
+        return fail(code, msg);
+    }
+    pl->workspace_bytes = acc;
+    *out = pl;
+    return NSFRB_OK;
+}
+
+int nsfrb_search(nsfrb_plan *pl, const float *cube, void *stream, float *snr_map, int32_t *argmax, nsfrb_cand *cands,
+                 uint32_t cand_capacity, uint32_t *ncands)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (!cube) return fail(NSFRB_EINVAL, "cube is null");
+    if ((reinterpret_cast<uintptr_t>(cube) & 15u) != 0) return fail(NSFRB_EINVAL, "cube is not 16-byte aligned");
+    if (int rc = check_outputs(snr_map, argmax, cands, cand_capacity, ncands)) return rc;
+    if (pl->n_received != 0) return fail(NSFRB_ESTATE, "plan holds streamed samples; call nsfrb_stream_reset first");
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int launches = 0;
+    mark(pl, 0, st);
+    CU(launch_transpose(cube, pl->d_W, pl->npix, pl->nchan, pl->nt, pl->pitch, st), "k_transpose launch");
+    ++launches;
+    mark(pl, 1, st);
+    const int rc = run_search(pl, 0, pl->nt, 0, 0, st, snr_map, argmax, cands, cand_capacity, ncands, &launches);
+    pl->last_launches = launches;
+    return rc;
+}
+
+int nsfrb_stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, void *stream, float *snr_map, int32_t *argmax,
+                      nsfrb_cand *cands, uint32_t cand_capacity, uint32_t *ncands)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (!chunk) return fail(NSFRB_EINVAL, "chunk is null");
+    if ((reinterpret_cast<uintptr_t>(chunk) & 15u) != 0) return fail(NSFRB_EINVAL, "chunk is not 16-byte aligned");
+    if (chunk_nt < 1 || chunk_nt > pl->nt) return fail(NSFRB_EINVAL, "chunk_nt must be in [1, nt]");
+    if (int rc = check_outputs(snr_map, argmax, cands, cand_capacity, ncands)) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int L = pl->nt;
+    const int64_t n_prev = pl->n_received;
+    int launches = 0;
+    mark(pl, 0, st);
+    CU(launch_push(chunk, pl->d_W, pl->d_base, pl->npix, pl->nchan, chunk_nt, pl->pitch, L, (int)(n_prev % L),
+                   n_prev == 0 ? 1 : 0, st),
+       "k_push launch");
+    ++launches;
+    mark(pl, 1, st);
+    const int64_t n = n_prev + chunk_nt;
+    pl->n_received = n;
+    const int64_t lo = std::max<int64_t>(0, n - L);
+    const int rc = run_search(pl, (int)(lo % L), (int)(n - lo), (int)(n_prev - lo), (int)(lo & 0x7fffffff), st, snr_map,
+                              argmax, cands, cand_capacity, ncands, &launches);
+    pl->last_launches = launches;
+    return rc;
+}
+
+int nsfrb_stream_reset(nsfrb_plan *pl)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    pl->n_received = 0;
+    return NSFRB_OK;
+}
+
+int nsfrb_search_host(nsfrb_plan *pl, const float *cube_host, void *stream, float *snr_map_host, int32_t *argmax_host,
+                      nsfrb_cand *cands_host, uint32_t cand_capacity, uint32_t *ncands_host)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (!cube_host) return fail(NSFRB_EINVAL, "cube is null");
+    if (int rc = check_outputs(snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host)) return rc;
+    const size_t bytes = (size_t)pl->nchan * pl->nt * (size_t)pl->npix * sizeof(float);
+    if (int rc = ensure_host_staging(pl, bytes, cand_capacity)) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CU(cudaMemcpyAsync(pl->d_in, cube_host, bytes, cudaMemcpyHostToDevice, st), "H2D cube");
+    if (int rc = nsfrb_search(pl, pl->d_in, stream, pl->d_snr, pl->d_arg, pl->d_cands, cand_capacity, pl->d_ncands)) return rc;
+    return copy_back(pl, st, snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host);
+}
+
+int nsfrb_stream_push_host(nsfrb_plan *pl, const float *chunk_host, int chunk_nt, void *stream, float *snr_map_host,
+                           int32_t *argmax_host, nsfrb_cand *cands_host, uint32_t cand_capacity, uint32_t *ncands_host)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (!chunk_host) return fail(NSFRB_EINVAL, "chunk is null");
+    if (chunk_nt < 1 || chunk_nt > pl->nt) return fail(NSFRB_EINVAL, "chunk_nt must be in [1, nt]");
+    if (int rc = check_outputs(snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host)) return rc;
+    const size_t bytes = (size_t)pl->nchan * chunk_nt * (size_t)pl->npix * sizeof(float);
+    if (int rc = ensure_host_staging(pl, bytes, cand_capacity)) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    CU(cudaMemcpyAsync(pl->d_in, chunk_host, bytes, cudaMemcpyHostToDevice, st), "H2D chunk");
+    if (int rc = nsfrb_stream_push(pl, pl->d_in, chunk_nt, stream, pl->d_snr, pl->d_arg, pl->d_cands, cand_capacity,
+                                   pl->d_ncands))
+        return rc;
+    return copy_back(pl, st, snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host);
+}
+
+int nsfrb_plan_destroy(nsfrb_plan *pl)
+{
+    if (!pl) return NSFRB_OK;
+    cudaDeviceSynchronize();
+    free_plan(pl);
+    return NSFRB_OK;
+}
+
+int nsfrb_plan_get_delays(const nsfrb_plan *pl, int32_t *out)
+{
+    if (!pl || !out) return fail(NSFRB_EINVAL, "null argument");
+    std::memcpy(out, pl->delays.data(), pl->delays.size() * sizeof(int32_t));
+    return NSFRB_OK;
+}
+
+int nsfrb_plan_get_info(const nsfrb_plan *pl, nsfrb_plan_info *info)
+{
+    if (!pl || !info) return fail(NSFRB_EINVAL, "null argument");
+    info->npix = pl->npix; info->nchan = pl->nchan; info->nt = pl->nt; info->ndm = pl->ndm; info->nwidth = pl->nw;
+    info->ndm_unique = pl->nuniq; info->dmax = pl->dmax_all; info->wmax = pl->wmax_used;
+    info->n_groups = pl->n_groups; info->n_width_batches = pl->n_wb; info->series_per_cta = kSearchWarps;
+    info->block_len = kBlockLen; info->ring_len = pl->H; info->search_threads = kSearchWarps * 32;
+    info->search_smem_bytes = (int64_t)pl->smem_search; info->workspace_bytes = (int64_t)pl->workspace_bytes;
+    info->cells_per_pixel = pl->cells_per_pixel; info->shift_adds_per_pixel = pl->shift_adds_per_pixel;
+    return NSFRB_OK;
+}
+
+int nsfrb_plan_last_launches(const nsfrb_plan *pl) { return pl ? pl->last_launches : 0; }
+
+int nsfrb_plan_set_profiling(nsfrb_plan *pl, int on)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (on)
+        for (auto &e : pl->ev)
+            if (!e) CU(cudaEventCreate(&e), "event create");
+    pl->profiling = on != 0;
+    pl->ev_valid = false;
+    return NSFRB_OK;
+}
+
+int nsfrb_plan_get_kernel_ms(nsfrb_plan *pl, float out[4])
+{
+    if (!pl || !out) return fail(NSFRB_EINVAL, "null argument");
+    if (!pl->ev_valid) return fail(NSFRB_ESTATE, "no profiled call yet (nsfrb_plan_set_profiling)");
+    CU(cudaEventSynchronize(pl->ev[4]), "event sync");
+    for (int i = 0; i < 4; ++i) CU(cudaEventElapsedTime(&out[i], pl->ev[i], pl->ev[i + 1]), "event elapsed");
+    return NSFRB_OK;
+}
+
+} // extern "C"
+#pragma GCC visibility pop

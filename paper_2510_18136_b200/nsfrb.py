@@ -1,0 +1,251 @@
+"""Thin ctypes binding over the C-ABI library libnsfrb.so (include/nsfrb.h).
+
+Argument marshalling only: every step of the search runs in the library's CUDA kernels.
+PyTorch supplies device memory and streams.  There is no CPU fallback: loading fails loudly
+if the library has not been built (python -m paper_2510_18136_b200.build).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnsfrb.so")
+
+NSFRB_OK, NSFRB_EINVAL, NSFRB_ENOMEM, NSFRB_ECUDA, NSFRB_ESTATE = 0, -1, -2, -3, -4
+
+
+class NsfrbError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"nsfrb error {code}: {msg}")
+        self.code = code
+
+
+class nsfrb_cand(ctypes.Structure):
+    _fields_ = [("pixel", ctypes.c_int32), ("dm_idx", ctypes.c_int32), ("width_idx", ctypes.c_int32),
+                ("t", ctypes.c_int32), ("snr", ctypes.c_float)]
+
+
+class nsfrb_plan_info(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in (
+        "npix", "nchan", "nt", "ndm", "nwidth", "ndm_unique", "dmax", "wmax", "n_groups", "n_width_batches",
+        "series_per_cta", "block_len", "ring_len", "search_threads")] + [
+        (n, ctypes.c_int64) for n in ("search_smem_bytes", "workspace_bytes", "cells_per_pixel", "shift_adds_per_pixel")]
+
+
+CAND_DTYPE = np.dtype([("pixel", "<i4"), ("dm_idx", "<i4"), ("width_idx", "<i4"), ("t", "<i4"), ("snr", "<f4")])
+assert CAND_DTYPE.itemsize == ctypes.sizeof(nsfrb_cand) == 20
+
+# every symbol include/nsfrb.h declares
+EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stream_reset", "nsfrb_search_host",
+           "nsfrb_stream_push_host", "nsfrb_plan_destroy", "nsfrb_plan_get_delays", "nsfrb_plan_get_info",
+           "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
+           "nsfrb_version")
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libnsfrb.so; raises if it is missing (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2510_18136_b200.build` (needs nvcc); "
+                              "there is no CPU fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i32p, f64p = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int32), ctypes.POINTER(ctypes.c_double)
+        L.nsfrb_plan_create.restype = ctypes.c_int
+        L.nsfrb_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                        f64p, ctypes.c_double, f64p, ctypes.c_int, i32p, ctypes.c_int, ctypes.c_float]
+        out = [vp, vp, vp, ctypes.c_uint32, vp]
+        L.nsfrb_search.restype = ctypes.c_int
+        L.nsfrb_search.argtypes = [vp, vp, vp] + out
+        L.nsfrb_stream_push.restype = ctypes.c_int
+        L.nsfrb_stream_push.argtypes = [vp, vp, ctypes.c_int, vp] + out
+        L.nsfrb_search_host.restype = ctypes.c_int
+        L.nsfrb_search_host.argtypes = [vp, vp, vp] + out
+        L.nsfrb_stream_push_host.restype = ctypes.c_int
+        L.nsfrb_stream_push_host.argtypes = [vp, vp, ctypes.c_int, vp] + out
+        L.nsfrb_stream_reset.restype = ctypes.c_int
+        L.nsfrb_stream_reset.argtypes = [vp]
+        L.nsfrb_plan_destroy.restype = ctypes.c_int
+        L.nsfrb_plan_destroy.argtypes = [vp]
+        L.nsfrb_plan_get_delays.restype = ctypes.c_int
+        L.nsfrb_plan_get_delays.argtypes = [vp, i32p]
+        L.nsfrb_plan_get_info.restype = ctypes.c_int
+        L.nsfrb_plan_get_info.argtypes = [vp, ctypes.POINTER(nsfrb_plan_info)]
+        L.nsfrb_plan_last_launches.restype = ctypes.c_int
+        L.nsfrb_plan_last_launches.argtypes = [vp]
+        L.nsfrb_plan_set_profiling.restype = ctypes.c_int
+        L.nsfrb_plan_set_profiling.argtypes = [vp, ctypes.c_int]
+        L.nsfrb_plan_get_kernel_ms.restype = ctypes.c_int
+        L.nsfrb_plan_get_kernel_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+        L.nsfrb_last_error.restype = ctypes.c_char_p
+        L.nsfrb_version.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def last_error() -> str:
+    return lib().nsfrb_last_error().decode()
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise NsfrbError(rc, last_error())
+
+
+@dataclass
+class SearchResult:
+    snr_map: torch.Tensor   # [npix] float32
+    argmax: torch.Tensor    # [3][npix] int32: dm_idx | width_idx | t
+    cands: torch.Tensor     # [capacity*20] uint8 (raw nsfrb_cand records)
+    ncands: torch.Tensor    # [1] int32 view of the uint32 counter
+
+    def candidates(self) -> np.ndarray:
+        """Structured array of the stored candidates (synchronises)."""
+        n = int(self.ncands.cpu().numpy().view(np.uint32)[0])
+        cap = self.cands.numel() // CAND_DTYPE.itemsize
+        raw = self.cands[: min(n, cap) * CAND_DTYPE.itemsize].cpu().numpy()
+        return raw.view(CAND_DTYPE).copy()
+
+    def n_found(self) -> int:
+        return int(self.ncands.cpu().numpy().view(np.uint32)[0])
+
+
+class Plan:
+    """nsfrb_plan_create / nsfrb_search / nsfrb_stream_push / nsfrb_plan_destroy."""
+
+    def __init__(self, nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, width_list, threshold, cand_capacity=4096):
+        f = np.ascontiguousarray(freqs_GHz, dtype=np.float64)
+        dm = np.ascontiguousarray(dm_list, dtype=np.float64)
+        w = np.ascontiguousarray(width_list, dtype=np.int32)
+        if f.size != nchan:
+            raise ValueError("len(freqs_GHz) != nchan")
+        self._h = ctypes.c_void_p()
+        self.nx, self.ny, self.npix, self.nchan, self.nt = int(nx), int(ny), int(nx) * int(ny), int(nchan), int(nt)
+        self.ndm, self.nwidth = dm.size, w.size
+        self.cand_capacity = int(cand_capacity)
+        _check(lib().nsfrb_plan_create(
+            ctypes.byref(self._h), int(nx), int(ny), int(nchan), int(nt),
+            f.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), float(tsamp_s),
+            dm.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), dm.size,
+            w.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), w.size, float(threshold)))
+        self.device = torch.device("cuda", torch.cuda.current_device())
+
+    @classmethod
+    def for_workload(cls, wl, **kw) -> "Plan":
+        return cls(wl.nx, wl.ny, wl.nchan, wl.nt, wl.freqs_GHz, wl.tsamp_s, wl.dm_list, wl.width_list, wl.threshold, **kw)
+
+    # -- plan facts
+    def delays(self) -> np.ndarray:
+        out = np.empty((self.ndm, self.nchan), dtype=np.int32)
+        _check(lib().nsfrb_plan_get_delays(self._h, out.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))))
+        return out
+
+    def info(self) -> dict:
+        s = nsfrb_plan_info()
+        _check(lib().nsfrb_plan_get_info(self._h, ctypes.byref(s)))
+        return {n: int(getattr(s, n)) for n, _ in s._fields_}
+
+    def last_launches(self) -> int:
+        return int(lib().nsfrb_plan_last_launches(self._h))
+
+    def set_profiling(self, on: bool = True):
+        _check(lib().nsfrb_plan_set_profiling(self._h, int(on)))
+
+    def kernel_ms(self) -> dict:
+        """Device milliseconds of the last call's kernels (needs set_profiling(True)); synchronises."""
+        a = (ctypes.c_float * 4)()
+        _check(lib().nsfrb_plan_get_kernel_ms(self._h, a))
+        return {"layout": a[0], "search": a[1], "finalize": a[2], "compact": a[3]}
+
+    # -- outputs
+    def alloc_outputs(self) -> SearchResult:
+        dev = self.device
+        return SearchResult(
+            torch.empty(self.npix, dtype=torch.float32, device=dev),
+            torch.empty((3, self.npix), dtype=torch.int32, device=dev),
+            torch.empty(max(self.cand_capacity, 1) * CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev),
+            torch.zeros(1, dtype=torch.int32, device=dev))
+
+    @staticmethod
+    def _stream_handle(stream) -> int:
+        s = torch.cuda.current_stream() if stream is None else stream
+        return int(s.cuda_stream)
+
+    def search(self, cube: torch.Tensor, out: SearchResult | None = None, stream=None) -> SearchResult:
+        """nsfrb_search on a device cube [nchan][nt][npix] float32 (asynchronous on `stream`)."""
+        self._check_dev(cube, (self.nchan, self.nt, self.npix))
+        out = out or self.alloc_outputs()
+        _check(lib().nsfrb_search(self._h, cube.data_ptr(), self._stream_handle(stream), out.snr_map.data_ptr(),
+                                  out.argmax.data_ptr(), out.cands.data_ptr(), self.cand_capacity,
+                                  out.ncands.data_ptr()))
+        return out
+
+    def stream_push(self, chunk: torch.Tensor, out: SearchResult | None = None, stream=None) -> SearchResult:
+        """nsfrb_stream_push of a device chunk [nchan][chunk_nt][npix] float32."""
+        if chunk.dim() != 3:
+            raise ValueError("chunk must be [nchan][chunk_nt][npix]")
+        self._check_dev(chunk, (self.nchan, chunk.shape[1], self.npix))
+        out = out or self.alloc_outputs()
+        _check(lib().nsfrb_stream_push(self._h, chunk.data_ptr(), int(chunk.shape[1]), self._stream_handle(stream),
+                                       out.snr_map.data_ptr(), out.argmax.data_ptr(), out.cands.data_ptr(),
+                                       self.cand_capacity, out.ncands.data_ptr()))
+        return out
+
+    def stream_reset(self):
+        _check(lib().nsfrb_stream_reset(self._h))
+
+    # -- host-buffer variants (H2D, search, D2H, synchronise) used for the end-to-end number
+    def _host_out(self):
+        pin = torch.cuda.is_available()
+        return (torch.empty(self.npix, dtype=torch.float32, pin_memory=pin),
+                torch.empty((3, self.npix), dtype=torch.int32, pin_memory=pin),
+                torch.empty(max(self.cand_capacity, 1) * CAND_DTYPE.itemsize, dtype=torch.uint8, pin_memory=pin),
+                torch.zeros(1, dtype=torch.int32, pin_memory=pin))
+
+    def search_host(self, cube_host: torch.Tensor, out=None, stream=None):
+        self._check_host(cube_host, (self.nchan, self.nt, self.npix))
+        out = out or self._host_out()
+        _check(lib().nsfrb_search_host(self._h, cube_host.data_ptr(), self._stream_handle(stream), out[0].data_ptr(),
+                                       out[1].data_ptr(), out[2].data_ptr(), self.cand_capacity, out[3].data_ptr()))
+        return out
+
+    def stream_push_host(self, chunk_host: torch.Tensor, out=None, stream=None):
+        self._check_host(chunk_host, (self.nchan, chunk_host.shape[1], self.npix))
+        out = out or self._host_out()
+        _check(lib().nsfrb_stream_push_host(self._h, chunk_host.data_ptr(), int(chunk_host.shape[1]),
+                                            self._stream_handle(stream), out[0].data_ptr(), out[1].data_ptr(),
+                                            out[2].data_ptr(), self.cand_capacity, out[3].data_ptr()))
+        return out
+
+    # -- checks / lifetime
+    def _check_dev(self, t, shape):
+        if not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+            raise ValueError(f"expected contiguous float32 CUDA tensor of shape {shape}, got {tuple(t.shape)} {t.dtype} {t.device}")
+
+    def _check_host(self, t, shape):
+        if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+            raise ValueError(f"expected contiguous float32 host tensor of shape {shape}")
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().nsfrb_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.destroy()

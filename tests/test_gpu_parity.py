@@ -1,0 +1,241 @@
+"""-m gpu: the CUDA path through the C ABI vs the oracle, element by element (P-rule)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle
+from paper_2510_18136_b200 import workloads as W
+from tests import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+
+
+def _nsfrb():
+    from paper_2510_18136_b200 import nsfrb
+    return nsfrb
+
+
+def _offline(wl, cube, *, pixels=None, capacity=4096, label=None):
+    """Run nsfrb_search on the device cube; compare `pixels` (default all) with the oracle."""
+    nsfrb = _nsfrb()
+    d_orc = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    with nsfrb.Plan.for_workload(wl, cand_capacity=capacity) as plan:
+        assert np.array_equal(plan.delays(), d_orc), "delay table must be bit-exact"
+        res = plan.search(cube)
+        torch.cuda.synchronize()
+        snr = res.snr_map.cpu().numpy()
+        arg = res.argmax.cpu().numpy().T.copy()
+        cands = res.candidates()
+        nfound = res.n_found()
+        info = plan.info()
+    assert info["cells_per_pixel"] == oracle.cells_per_pixel(d_orc, wl.width_list, wl.nt)
+    pix = np.arange(wl.npix) if pixels is None else np.asarray(pixels)
+    sub = cube[:, :, torch.as_tensor(pix, device=cube.device)].cpu().numpy()
+    st = PU.check(sub, d_orc, wl.width_list, snr[pix], arg[pix], wl.threshold, label=label or wl.name)
+    cs = PU.check_candidates(st["oracle"], pix, cands, nfound, wl.threshold, capacity, all_pixels_checked=pixels is None)
+    # stored candidate records repeat the maps exactly
+    for c in cands:
+        p = int(c["pixel"])
+        assert c["snr"] == snr[p] and (c["dm_idx"], c["width_idx"], c["t"]) == tuple(arg[p])
+        assert c["snr"] > wl.threshold
+    return st, cs, snr, arg
+
+
+def _inject_all(wl, cube, d):
+    pulses = W.injection_table(wl, d)
+    W.inject(cube, pulses, d)
+    return pulses
+
+
+# ----------------------------------------------------------------------------- config 1
+def test_c1_as_specified():
+    wl = W.config("c1")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    cube = W.make_cube(wl, "cuda")
+    W.inject(cube, W.injection_table(wl, d), d, extra_delays=oracle.delays(wl.freqs_GHz, wl.tsamp_s, [500.0])[0])
+    st, cs, snr, arg = _offline(wl, cube)
+    p = 20 * 32 + 11
+    assert abs(snr[p] - 5.728493) < 1e-3 and tuple(arg[p]) == (0, 2, 31)
+    assert cs["found"] == 0            # an empty candidate list is the right answer here
+    assert st["adjudicated"] <= 0.1 * st["n"]
+
+
+def test_c1b_threshold5_has_one_candidate():
+    from dataclasses import replace
+    wl = replace(W.config("c1"), threshold=5.0)
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    cube = W.make_cube(wl, "cuda")
+    W.inject(cube, W.injection_table(wl, d), d, extra_delays=oracle.delays(wl.freqs_GHz, wl.tsamp_s, [500.0])[0])
+    st, cs, snr, arg = _offline(wl, cube)
+    assert cs["found"] == 1
+
+
+def test_c1c_long_series_pulse_on_grid():
+    # nt = 2048, DM 600 on the trial grid: BASELINE's S0 = A w nchan / (sigma sqrt(w nchan)) regime
+    from dataclasses import replace
+    wl = replace(W.config("c1"), nt=2048, name="c1c")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    rng = np.random.default_rng(0)
+    cube = torch.from_numpy(rng.standard_normal((wl.nchan, wl.nt, wl.npix)).astype(np.float32)).cuda()
+    W.inject(cube, [W.Pulse(pixel=651, dm_idx=3, width_idx=2, t0=1000, width=4, s0=8.49, amp=1.5)], d)
+    st, cs, snr, arg = _offline(wl, cube)
+    assert tuple(arg[651][:2]) == (3, 2) and abs(arg[651][2] - 1000) <= 1
+    assert 6.5 < snr[651] < 10.5 and cs["found"] >= 1
+
+
+# ----------------------------------------------------------------------------- scaled C3, C4, C5
+@pytest.mark.parametrize("name,nx,ny,nt", [
+    ("c3", 12, 8, None),      # full 4096-sample series, 32 DMs x 24 widths, sky term
+    ("c3", 7, 5, 1000),       # ragged: nt not a multiple of the block, npix not a multiple of 32
+    ("c4", 40, 25, None),     # 64 DMs (44 distinct vectors), Fibonacci widths, channel gains
+    ("c5", 8, 6, None),       # 64 channels, 256 DMs, 32 widths, RFI spikes
+    ("c5", 5, 3, 1500),       # widths up to 1200 on a 1500-sample cube
+])
+def test_scaled_configs(name, nx, ny, nt):
+    wl = W.config(name).scaled(nx, ny, nt, n_pulses=min(W.config(name).n_pulses, nx * ny // 3))
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    cube = W.make_cube(wl, "cuda")
+    pulses = _inject_all(wl, cube, d)
+    st, cs, snr, arg = _offline(wl, cube)
+    assert st["exact"] >= 0.75 * st["n"], st
+    # injected single pulses with nominal S0 >= 12 are recovered at their trial DM (or a duplicate's lowest index)
+    hits = 0
+    strong = [pu for pu in pulses if pu.s0 >= 12 and not pu.train_period]
+    for pu in strong:
+        if np.array_equal(d[arg[pu.pixel][0]], d[pu.dm_idx]) and abs(arg[pu.pixel][2] - pu.t0) <= max(2, pu.width // 4):
+            hits += 1
+    assert hits >= 0.6 * len(strong), (hits, len(strong))
+
+
+# ----------------------------------------------------------------------------- streaming (C2)
+def _stream_case(wl, n_push, eval_at, chunk_sizes=None, capacity=1024):
+    nsfrb = _nsfrb()
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    src = W.ChunkSource(wl, d, n_push, "cuda")
+    so = oracle.StreamOracle(wl.nchan, wl.npix, wl.nt, d, wl.width_list)
+    stats = []
+    with nsfrb.Plan.for_workload(wl, cand_capacity=capacity) as plan:
+        out = plan.alloc_outputs()
+        for i in range(n_push):
+            if chunk_sizes is None:
+                chunk = src.next()
+            else:
+                c = chunk_sizes[i % len(chunk_sizes)]
+                chunk = torch.randn((wl.nchan, c, wl.npix), device="cuda", generator=src.g)
+            plan.stream_push(chunk, out)
+            torch.cuda.synchronize()
+            ch = chunk.cpu().numpy()
+            n_prev = so.n
+            so.n += ch.shape[1]
+            so.hist = np.concatenate([so.hist, ch], axis=1)[:, -so.L:, :]
+            if i in eval_at:
+                lo = max(0, so.n - so.L)
+                snr = out.snr_map.cpu().numpy()
+                arg = out.argmax.cpu().numpy().T.copy()
+                st = PU.check(so.hist, d, wl.width_list, snr, arg, wl.threshold, raw_end_min=n_prev - lo,
+                              t_offset=lo, label=f"{wl.name} push {i}")
+                PU.check_candidates(st["oracle"], np.arange(wl.npix), out.candidates(), out.n_found(), wl.threshold,
+                                    capacity)
+                stats.append(st)
+        # offline search is refused while the plan holds streamed samples
+        cube = torch.zeros((wl.nchan, wl.nt, wl.npix), device="cuda")
+        with pytest.raises(nsfrb.NsfrbError) as ei:
+            plan.search(cube)
+        assert ei.value.code == nsfrb.NSFRB_ESTATE
+        plan.stream_reset()
+        plan.search(cube)
+        torch.cuda.synchronize()
+    return stats
+
+
+def test_stream_c2_scaled():
+    wl = W.config("c2").scaled(12, 8)
+    # first pushes (ring nearly empty), mid fill, the pushes around the ring wrap (1536/25 = 61.44), steady state
+    stats = _stream_case(wl, 68, eval_at={0, 1, 2, 7, 30, 48, 60, 61, 62, 63, 67})
+    assert sum(s["exact"] for s in stats) >= 0.75 * sum(s["n"] - s["undefined"] for s in stats)
+
+
+def test_stream_small_ring_variable_chunks():
+    from dataclasses import replace
+    wl = replace(W.config("c2").scaled(9, 5, nt=300), width_list=np.asarray([1, 2, 5, 16, 40, 120, 250], np.int32))
+    _stream_case(wl, 40, eval_at=set(range(40)), chunk_sizes=[25, 1, 7, 60, 300, 13])
+
+
+def test_stream_equals_offline_on_ring_contents():
+    nsfrb = _nsfrb()
+    wl = W.config("c2").scaled(8, 4, nt=256)
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    g = torch.Generator(device="cuda").manual_seed(5)
+    data = torch.randn((wl.nchan, 20 * 25, wl.npix), device="cuda", generator=g)
+    with nsfrb.Plan.for_workload(wl) as plan:
+        for i in range(20):
+            out = plan.stream_push(data[:, i * 25:(i + 1) * 25, :].contiguous())
+        torch.cuda.synchronize()
+        s_stream = out.snr_map.cpu().numpy()
+    lo = 20 * 25 - wl.nt
+    ring = data[:, lo:, :].contiguous().cpu().numpy()
+    r = oracle.search(ring, d, wl.width_list, raw_end_min=wl.nt - 25, t_offset=lo)
+    assert np.all(np.abs(s_stream - r.snr) <= PU.tol(r.snr))
+
+
+# ----------------------------------------------------------------------------- edge and degenerate cases
+def test_degenerate_pixels_and_duplicate_unsorted_dms():
+    from dataclasses import replace
+    base = W.config("c1")
+    # unsorted DM list with duplicates (exact ties must resolve to the lowest index, R17)
+    dms = np.asarray([600.0, 0.0, 1400.0, 600.0, 200.0, 0.0, 1000.0, 3.0])
+    wl = replace(base, nx=9, ny=7, nt=300, dm_list=dms, width_list=np.asarray([3, 1, 400, 17, 2], np.int32), name="edge")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    assert np.array_equal(d[7], d[1])  # DM 3 has the delay vector of DM 0
+    rng = np.random.default_rng(3)
+    a = rng.standard_normal((wl.nchan, wl.nt, wl.npix)).astype(np.float32)
+    a[:, :, 0] = 0.0                      # all-zero pixel: sigma = 0 -> S = 0, argmax (first defined cell)
+    a[:, :, 1] = 3.0                      # constant pixel
+    a[:, :, 2] += 1000.0                  # large DC offset (invariance; per-channel baseline removal)
+    a[:, :, 3] *= 1e-3                    # small scale
+    a[:, :, 4] *= 1e3                     # large scale
+    a[:, 100:104, 5] += 5.0               # zero-DM pulse: DM 0 appears at k=1 and k=5 and k=7's vector
+    cube = torch.from_numpy(a).cuda()
+    st, cs, snr, arg = _offline(wl, cube)
+    assert snr[0] == 0.0 and snr[1] == 0.0
+    assert tuple(arg[0]) == tuple(st["oracle"].argmax[0]) and tuple(arg[1]) == tuple(st["oracle"].argmax[1])
+    assert arg[5][0] == 1                 # lowest index among the identical trials {1, 5, 7}
+
+
+def test_no_cell_defined_and_single_channel():
+    from dataclasses import replace
+    nsfrb = _nsfrb()
+    wl = replace(W.config("c1"), nx=5, ny=3, nt=40, width_list=np.asarray([41, 100], np.int32), name="nocell")
+    cube = torch.randn((wl.nchan, wl.nt, wl.npix), device="cuda")
+    with nsfrb.Plan.for_workload(wl) as plan:
+        res = plan.search(cube)
+        torch.cuda.synchronize()
+        assert torch.all(torch.isneginf(res.snr_map)) and torch.all(res.argmax == -1) and res.n_found() == 0
+    wl1 = replace(W.config("c1"), nx=6, ny=6, nchan=1, nt=77, freqs_GHz=np.asarray([1.4]), name="1chan")
+    cube = torch.randn((1, 77, 36), device="cuda")
+    _offline(wl1, cube)
+
+
+def test_candidate_overflow_reports_total():
+    from dataclasses import replace
+    wl = replace(W.config("c1"), threshold=2.0, name="overflow")
+    cube = W.make_cube(wl, "cuda")
+    st, cs, snr, arg = _offline(wl, cube, capacity=7)
+    assert cs["found"] > 7
+
+
+def test_host_buffer_variants_match_device_path():
+    nsfrb = _nsfrb()
+    wl = W.config("c1")
+    cube = W.make_cube(wl, "cpu").pin_memory()
+    with nsfrb.Plan.for_workload(wl) as plan:
+        h = plan.search_host(cube)
+        dres = plan.search(cube.cuda())
+        torch.cuda.synchronize()
+        assert torch.equal(h[0], dres.snr_map.cpu()) and torch.equal(h[1], dres.argmax.cpu())
+        assert int(h[3].numpy().view(np.uint32)[0]) == dres.n_found()
+        hp = plan.stream_push_host(cube[:, :25, :].contiguous().pin_memory())
+        plan.stream_reset()
+        dp = plan.stream_push(cube[:, :25, :].contiguous().cuda())
+        torch.cuda.synchronize()
+        assert torch.equal(hp[0], dp.snr_map.cpu()) and torch.equal(hp[1], dp.argmax.cpu())
