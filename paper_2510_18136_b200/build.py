@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnsfrb.so")
-SOURCES = ["nsfrb_api.cu", "nsfrb_kernels.cu"]
+SOURCES = ["nsfrb_api.cu", "nsfrb_kernels.cu", "nsfrb_search.cu"]
 HEADERS = [os.path.join(CSRC, "nsfrb_internal.h"), os.path.join(os.path.dirname(HERE), "include", "nsfrb.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",

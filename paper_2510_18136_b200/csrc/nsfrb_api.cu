@@ -56,12 +56,14 @@ struct nsfrb_plan {
     int nw_used = 0;
     std::vector<int32_t> widths_used, j_of_used;
     int wmax_used = 0, dmax_all = 0, dmin_all = 0;
-    int n_groups = 0, n_wb = 0, H = 0, RS = 0, pitch = 0;
+    int n_groups = 0, n_wb = 0, H = 0, RS = 0, pitch = 0, tab_cap = 0;
+    std::vector<int32_t> dd_tab, dd_off; // per-group dedispersion change lists
     size_t smem_search = 0, smem_final = 0;
     int64_t cells_per_pixel = 0, shift_adds_per_pixel = 0;
     // device
     float *d_W = nullptr;
     float *d_base = nullptr;
+    int32_t *d_dd_tab = nullptr, *d_dd_off = nullptr;
     int32_t *d_delays_u = nullptr, *d_dmax_u = nullptr, *d_k_of_u = nullptr, *d_widths = nullptr, *d_j_of_used = nullptr;
     Partial *d_partials = nullptr;
     size_t workspace_bytes = 0;
@@ -89,6 +91,7 @@ void free_plan(nsfrb_plan *p)
 {
     if (!p) return;
     cudaFree(p->d_W); cudaFree(p->d_base); cudaFree(p->d_delays_u); cudaFree(p->d_dmax_u); cudaFree(p->d_k_of_u);
+    cudaFree(p->d_dd_tab); cudaFree(p->d_dd_off);
     cudaFree(p->d_widths); cudaFree(p->d_j_of_used); cudaFree(p->d_partials); cudaFree(p->d_in); cudaFree(p->d_snr);
     cudaFree(p->d_arg); cudaFree(p->d_cands); cudaFree(p->d_ncands);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
@@ -112,6 +115,53 @@ inline void mark(nsfrb_plan *pl, int i, cudaStream_t st)
     if (pl->profiling && pl->ev[i]) cudaEventRecord(pl->ev[i], st);
 }
 
+// Dedispersion record streams, one per group of kSearchWarps unique trials (sorted by dmax), read by
+// phase 1 of k_search.  All records are 4-int aligned.  Offsets index the raw tile raw[c*RS + i].
+//   [0..3]   pos(half 0), pos(half 1), 0, 0
+//   half:    {nser, 0, 0, 0} then nser trial records (a half is 8 consecutive trials of the group)
+//   trial:   {n, 0, 0, 0} + n offsets c*RS + d[u][c]  (padded to 4 ints): D = sum_c raw[off_c + t]
+//        or  {n, 1, 0, 0} + n*4 (new, old) offset pairs: D += sum raw[new + t] - raw[old + t]
+//            for the channels whose delay differs from the previous trial (padding pairs are (0,0)).
+void build_dd_tables(nsfrb_plan *pl)
+{
+    const int nchan = pl->nchan, RS = pl->RS;
+    pl->dd_tab.clear();
+    pl->dd_off.assign(1, 0);
+    int cap = 0;
+    for (int g = 0; g < pl->n_groups; ++g) {
+        std::vector<int32_t> t(4, 0);
+        const int u0 = g * kSearchWarps, n = std::min(kSearchWarps, pl->nuniq - u0);
+        for (int h = 0; h < 2; ++h) {
+            t[h] = (int32_t)t.size();
+            const int first = h * 8, nser = std::max(0, std::min(8, n - first));
+            t.insert(t.end(), {nser, 0, 0, 0});
+            for (int s = 0; s < nser; ++s) {
+                const int32_t *d = &pl->delays_u[(size_t)(u0 + first + s) * nchan];
+                std::vector<int32_t> pairs;
+                if (s > 0) {
+                    const int32_t *dp = d - nchan;
+                    for (int c = 0; c < nchan; ++c)
+                        if (d[c] != dp[c]) { pairs.push_back(c * RS + d[c]); pairs.push_back(c * RS + dp[c]); }
+                }
+                const int np4 = (int)((pairs.size() / 2 + 3) / 4);
+                if (s > 0 && 2 * 4 * np4 < nchan) {
+                    pairs.resize((size_t)np4 * 8, 0);
+                    t.insert(t.end(), {np4, 1, 0, 0});
+                    t.insert(t.end(), pairs.begin(), pairs.end());
+                } else {
+                    t.insert(t.end(), {nchan, 0, 0, 0});
+                    for (int c = 0; c < nchan; ++c) t.push_back(c * RS + d[c]);
+                    while (t.size() % 4) t.push_back(0);
+                }
+            }
+        }
+        cap = std::max(cap, (int)t.size());
+        pl->dd_tab.insert(pl->dd_tab.end(), t.begin(), t.end());
+        pl->dd_off.push_back((int32_t)pl->dd_tab.size());
+    }
+    pl->tab_cap = round_up(std::max(cap, 4), 4);
+}
+
 // Enqueue search + finalize + compaction over the workspace as it stands.
 int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offset, cudaStream_t st, float *snr_map,
                int32_t *argmax, nsfrb_cand *cands, uint32_t cap, uint32_t *ncands, int *launches)
@@ -120,11 +170,11 @@ int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offse
     if (slices > 0) {
         SearchParams sp;
         sp.W = pl->d_W; sp.delays_u = pl->d_delays_u; sp.dmax_u = pl->d_dmax_u; sp.k_of_u = pl->d_k_of_u;
-        sp.widths = pl->d_widths; sp.partials = pl->d_partials;
+        sp.widths = pl->d_widths; sp.partials = pl->d_partials; sp.dd_tab = pl->d_dd_tab; sp.dd_off = pl->d_dd_off;
         sp.npix = pl->npix; sp.nchan = pl->nchan; sp.pitch = pl->pitch; sp.ring_L = pl->nt;
         sp.origin = origin; sp.len = len; sp.raw_end_min = raw_end_min;
         sp.nuniq = pl->nuniq; sp.nw = pl->nw_used; sp.n_groups = pl->n_groups; sp.n_wb = pl->n_wb;
-        sp.H = pl->H; sp.RS = pl->RS; sp.wmax = pl->wmax_used;
+        sp.H = pl->H; sp.RS = pl->RS; sp.wmax = pl->wmax_used; sp.tab_cap = pl->tab_cap;
         CU(launch_search(sp, pl->smem_search, st), "k_search launch");
         ++*launches;
     }
@@ -289,10 +339,11 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const
     // ---- kernel geometry
     pl->n_groups = (pl->nuniq + kSearchWarps - 1) / kSearchWarps;
     pl->n_wb = std::max(1, (pl->nw_used + kWidthBatch - 1) / kWidthBatch);
-    pl->H = round_up(std::max(pl->wmax_used, 1) + kBlockLen, 32);
+    pl->H = round_up(std::max(pl->wmax_used, 1) + kBlockLen + 32, 32);
     pl->RS = round_up(kBlockLen + pl->dmax_all, 4);
     pl->pitch = round_up(nt, 4);
-    pl->smem_search = search_smem_bytes(nchan, pl->RS, pl->H);
+    build_dd_tables(pl);
+    pl->smem_search = search_smem_bytes(nchan, pl->RS, pl->H, pl->tab_cap);
     pl->smem_final = final_smem_bytes(nt);
     if (pl->smem_search > kMaxSmem || pl->smem_final > kMaxSmem) {
         char buf[256];
@@ -309,9 +360,12 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const
 
     // ---- device state
     cudaError_t e = cudaGetDevice(&pl->device);
-    if (e == cudaSuccess) e = configure_kernels(pl->smem_search, pl->smem_final);
+    if (e == cudaSuccess) e = configure_kernels(pl->smem_final);
+    if (e == cudaSuccess) e = configure_search(pl->smem_search);
     size_t acc = 0;
     if (e == cudaSuccess) e = upload(&pl->d_delays_u, pl->delays_u, &acc);
+    if (e == cudaSuccess) e = upload(&pl->d_dd_tab, pl->dd_tab, &acc);
+    if (e == cudaSuccess) e = upload(&pl->d_dd_off, pl->dd_off, &acc);
     if (e == cudaSuccess) e = upload(&pl->d_dmax_u, pl->dmax_u, &acc);
     if (e == cudaSuccess) e = upload(&pl->d_k_of_u, pl->k_of_u, &acc);
     if (e == cudaSuccess) e = upload(&pl->d_widths, pl->widths_used, &acc);

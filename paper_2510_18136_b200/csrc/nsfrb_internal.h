@@ -28,6 +28,7 @@ struct Partial {
 constexpr int kBlockLen = 256;   // dedispersed samples per time block (8 per lane)
 constexpr int kWidthBatch = 32;  // widths one search CTA tracks in registers
 constexpr int kSearchWarps = 16; // warps per search CTA = DM trials held on chip per CTA
+constexpr int kStageStride = 288; // floats per trial in the dedispersion staging tile: t + 4*(t>>5), t < 256
 
 struct SearchParams {
     const float *W;          // [npix][nchan][pitch]  time-contiguous, baseline removed
@@ -35,6 +36,8 @@ struct SearchParams {
     const int32_t *dmax_u;   // [nuniq]
     const int32_t *k_of_u;   // [nuniq]               lowest original dm index of the trial
     const int32_t *widths;   // [nw]
+    const int32_t *dd_tab;   // dedispersion change lists, one record stream per group (see build_dd_tables)
+    const int32_t *dd_off;   // [n_groups+1] offsets into dd_tab
     Partial *partials;       // [npix][n_groups*n_wb]
     int32_t npix, nchan, pitch;
     int32_t ring_L;      // slots per (pixel, channel) row = plan nt
@@ -42,7 +45,8 @@ struct SearchParams {
     int32_t len;         // valid raw samples (nt offline; min(n, L) streaming)
     int32_t raw_end_min; // S5: windows must end (raw frame) at or after this relative index
     int32_t nuniq, nw, n_groups, n_wb;
-    int32_t H;           // prefix history per series (multiple of 32, >= wmax + kBlockLen)
+    int32_t H;           // prefix history per series (multiple of 32, >= wmax + kBlockLen + 32)
+    int32_t tab_cap;     // ints reserved in shared memory for one group's change lists (multiple of 4)
     int32_t RS;          // raw block row stride in floats
     int32_t wmax;
 };
@@ -68,8 +72,9 @@ cudaError_t launch_search(const SearchParams &p, size_t smem_bytes, cudaStream_t
 cudaError_t launch_finalize(const FinalParams &p, size_t smem_bytes, cudaStream_t st);
 cudaError_t launch_compact(const float *snr_map, const int32_t *argmax, int npix, float threshold,
                            nsfrb_cand *cands, uint32_t cap, uint32_t *ncands, cudaStream_t st);
-cudaError_t configure_kernels(size_t search_smem, size_t final_smem);
-size_t search_smem_bytes(int nchan, int RS, int H);
+cudaError_t configure_kernels(size_t final_smem);
+cudaError_t configure_search(size_t search_smem);
+size_t search_smem_bytes(int nchan, int RS, int H, int tab_cap);
 size_t final_smem_bytes(int nt);
 
 } // namespace nsfrb
