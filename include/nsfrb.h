@@ -27,6 +27,7 @@
 #ifndef NSFRB_H
 #define NSFRB_H
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -150,6 +151,19 @@ int nsfrb_plan_last_launches(const nsfrb_plan *plan);
  */
 int nsfrb_plan_set_profiling(nsfrb_plan *plan, int on);
 int nsfrb_plan_get_kernel_ms(nsfrb_plan *plan, float out[4]);
+
+/*
+ * Harness access to the plan-specialised real-time kernel: for the plan the first ten
+ * arguments describe (as nsfrb_plan_create) and a first chunk of chunk_nt samples, writes either the CUDA
+ * source the library compiles at the first nsfrb_stream_push (want_cubin = 0) or its sm_100a cubin
+ * (want_cubin = 1, compiled with NVRTC) to out[capacity] (host) and the byte count to *needed; call with
+ * out = NULL to size the buffer.  variant = NULL or "" selects the default tile shape, else
+ * "KK,GPC,SEG,TT[,MINB]".  Needs no CUDA device.
+ */
+int nsfrb_jit_stream_kernel(int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
+                            const double *dm_list, int ndm, const int32_t *width_list, int nwidth,
+                            int chunk_nt, const char *variant, int want_cubin,
+                            char *out, size_t capacity, size_t *needed);
 
 /* Thread-local text of the last error; never NULL. */
 const char *nsfrb_last_error(void);

@@ -41,63 +41,20 @@ constexpr size_t kMaxSmem = 227 * 1024; // opt-in dynamic shared memory per CTA 
 
 } // namespace
 
-struct nsfrb_plan {
-    int nx = 0, ny = 0, npix = 0, nchan = 0, nt = 0, ndm = 0, nw = 0;
-    double tsamp = 0;
-    float threshold = 0;
-    std::vector<double> freqs, dms;
-    std::vector<int32_t> widths;
-    std::vector<int32_t> delays; // [ndm][nchan]
-    std::vector<int32_t> dmax;   // [ndm]
-    // unique trials, sorted by (dmax, first original index)
-    int nuniq = 0;
-    std::vector<int32_t> k_of_u, dmax_u, delays_u;
-    // widths that can hold at least one cell for some trial, original order
-    int nw_used = 0;
-    std::vector<int32_t> widths_used, j_of_used;
-    int wmax_used = 0, dmax_all = 0, dmin_all = 0;
-    int n_groups = 0, n_wb = 0, H = 0, RS = 0, pitch = 0, tab_cap = 0;
-    std::vector<int32_t> dd_tab, dd_off; // per-group dedispersion change lists
-    size_t smem_search = 0, smem_final = 0;
-    int64_t cells_per_pixel = 0, shift_adds_per_pixel = 0;
-    // device
-    float *d_W = nullptr;
-    float *d_base = nullptr;
-    int32_t *d_dd_tab = nullptr, *d_dd_off = nullptr;
-    int32_t *d_delays_u = nullptr, *d_dmax_u = nullptr, *d_k_of_u = nullptr, *d_widths = nullptr, *d_j_of_used = nullptr;
-    Partial *d_partials = nullptr;
-    size_t workspace_bytes = 0;
-    // streaming state
-    int64_t n_received = 0;
-    // host-variant staging
-    float *d_in = nullptr;
-    size_t d_in_bytes = 0;
-    float *d_snr = nullptr;
-    int32_t *d_arg = nullptr;
-    nsfrb_cand *d_cands = nullptr;
-    uint32_t d_cands_cap = 0;
-    uint32_t *d_ncands = nullptr;
-    int last_launches = 0;
-    int device = 0;
-    // optional per-kernel timing
-    bool profiling = false;
-    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
-    bool ev_valid = false;
-};
-
-namespace {
-
-void free_plan(nsfrb_plan *p)
+void nsfrb::free_plan(nsfrb_plan *p)
 {
     if (!p) return;
-    cudaFree(p->d_W); cudaFree(p->d_base); cudaFree(p->d_delays_u); cudaFree(p->d_dmax_u); cudaFree(p->d_k_of_u);
+    cudaFree(p->d_W); cudaFree(p->d_delays_u); cudaFree(p->d_dmax_u); cudaFree(p->d_k_of_u);
     cudaFree(p->d_dd_tab); cudaFree(p->d_dd_off);
     cudaFree(p->d_widths); cudaFree(p->d_j_of_used); cudaFree(p->d_partials); cudaFree(p->d_in); cudaFree(p->d_snr);
     cudaFree(p->d_arg); cudaFree(p->d_cands); cudaFree(p->d_ncands);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
+    stream_free(p);
     cudaGetLastError();
     delete p;
 }
+
+namespace {
 
 template <typename T>
 cudaError_t upload(T **dst, const std::vector<T> &src, size_t *acc)
@@ -244,8 +201,13 @@ extern "C" {
 const char *nsfrb_last_error(void) { return g_err.c_str(); }
 const char *nsfrb_version(void) { return "0.1 (sm_100a)"; }
 
-int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
-                      const double *dm_list, int ndm, const int32_t *width_list, int nwidth, float threshold)
+} // extern "C"
+#pragma GCC visibility pop
+
+// Validation and every host-side table of a plan (no CUDA call): shared by nsfrb_plan_create and the
+// JIT harness entry points, which must work on a machine without a GPU.
+int nsfrb::plan_host_init(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
+                          const double *dm_list, int ndm, const int32_t *width_list, int nwidth, float threshold)
 {
     if (!out) return fail(NSFRB_EINVAL, "out is null");
     *out = nullptr;
@@ -328,6 +290,10 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const
             pl->wmax_used = std::max(pl->wmax_used, width_list[j]);
         }
     pl->nw_used = (int)pl->widths_used.size();
+    pl->stream_worder.resize(pl->nw_used);
+    std::iota(pl->stream_worder.begin(), pl->stream_worder.end(), 0);
+    std::sort(pl->stream_worder.begin(), pl->stream_worder.end(),
+              [&](int a, int b) { return pl->widths_used[a] < pl->widths_used[b]; });
 
     for (int k = 0; k < ndm; ++k) {
         const int T = nt - pl->dmax[k];
@@ -358,6 +324,20 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const
         return fail(NSFRB_EINVAL, "too many (pixel, DM group, width batch) tasks for one launch");
     }
 
+    *out = pl;
+    return NSFRB_OK;
+}
+
+#pragma GCC visibility push(default)
+extern "C" {
+
+int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
+                      const double *dm_list, int ndm, const int32_t *width_list, int nwidth, float threshold)
+{
+    nsfrb_plan *pl = nullptr;
+    if (int rc = plan_host_init(&pl, nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, ndm, width_list, nwidth, threshold))
+        return rc;
+    *out = nullptr;
     // ---- device state
     cudaError_t e = cudaGetDevice(&pl->device);
     if (e == cudaSuccess) e = configure_kernels(pl->smem_final);
@@ -371,19 +351,9 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const
     if (e == cudaSuccess) e = upload(&pl->d_widths, pl->widths_used, &acc);
     if (e == cudaSuccess) e = upload(&pl->d_j_of_used, pl->j_of_used, &acc);
     if (e == cudaSuccess) {
-        const size_t wb = (size_t)pl->npix * nchan * (size_t)pl->pitch * sizeof(float);
-        e = cudaMalloc(reinterpret_cast<void **>(&pl->d_W), wb);
-        if (e == cudaSuccess) { acc += wb; e = cudaMemset(pl->d_W, 0, wb); }
-    }
-    if (e == cudaSuccess) {
         const size_t pb = (size_t)pl->npix * pl->n_groups * pl->n_wb * sizeof(Partial);
         e = cudaMalloc(reinterpret_cast<void **>(&pl->d_partials), pb);
         acc += pb;
-    }
-    if (e == cudaSuccess) {
-        const size_t bb = (size_t)pl->npix * nchan * sizeof(float);
-        e = cudaMalloc(reinterpret_cast<void **>(&pl->d_base), bb);
-        acc += bb;
     }
     if (e != cudaSuccess) {
         const int code = (e == cudaErrorMemoryAllocation) ? NSFRB_ENOMEM : NSFRB_ECUDA;
@@ -406,6 +376,17 @@ int nsfrb_search(nsfrb_plan *pl, const float *cube, void *stream, float *snr_map
     if (int rc = check_outputs(snr_map, argmax, cands, cand_capacity, ncands)) return rc;
     if (pl->n_received != 0) return fail(NSFRB_ESTATE, "plan holds streamed samples; call nsfrb_stream_reset first");
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (!pl->d_W) { // time-contiguous copy of the cube, allocated on first use
+        const size_t wb = (size_t)pl->npix * pl->nchan * (size_t)pl->pitch * sizeof(float);
+        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&pl->d_W), wb);
+        if (e == cudaSuccess) e = cudaMemset(pl->d_W, 0, wb);
+        if (e != cudaSuccess) {
+            cudaFree(pl->d_W);
+            pl->d_W = nullptr;
+            return e == cudaErrorMemoryAllocation ? fail(NSFRB_ENOMEM, "workspace allocation failed") : fail_cuda(e, "workspace alloc");
+        }
+        pl->workspace_bytes += wb;
+    }
     int launches = 0;
     mark(pl, 0, st);
     CU(launch_transpose(cube, pl->d_W, pl->npix, pl->nchan, pl->nt, pl->pitch, st), "k_transpose launch");
@@ -425,28 +406,25 @@ int nsfrb_stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, void *st
     if (chunk_nt < 1 || chunk_nt > pl->nt) return fail(NSFRB_EINVAL, "chunk_nt must be in [1, nt]");
     if (int rc = check_outputs(snr_map, argmax, cands, cand_capacity, ncands)) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const int L = pl->nt;
-    const int64_t n_prev = pl->n_received;
     int launches = 0;
     mark(pl, 0, st);
-    CU(launch_push(chunk, pl->d_W, pl->d_base, pl->npix, pl->nchan, chunk_nt, pl->pitch, L, (int)(n_prev % L),
-                   n_prev == 0 ? 1 : 0, st),
-       "k_push launch");
+    std::string err;
+    if (int rc = stream_push(pl, chunk, chunk_nt, st, snr_map, argmax, &launches, err)) return fail(rc, err);
+    mark(pl, 3, st);
+    CU(cudaMemsetAsync(ncands, 0, sizeof(uint32_t), st), "memset ncands");
+    CU(launch_compact(snr_map, argmax, pl->npix, pl->threshold, cands, cand_capacity, ncands, st), "k_compact launch");
     ++launches;
-    mark(pl, 1, st);
-    const int64_t n = n_prev + chunk_nt;
-    pl->n_received = n;
-    const int64_t lo = std::max<int64_t>(0, n - L);
-    const int rc = run_search(pl, (int)(lo % L), (int)(n - lo), (int)(n_prev - lo), (int)(lo & 0x7fffffff), st, snr_map,
-                              argmax, cands, cand_capacity, ncands, &launches);
+    mark(pl, 4, st);
+    pl->ev_valid = pl->profiling;
     pl->last_launches = launches;
-    return rc;
+    return NSFRB_OK;
 }
 
 int nsfrb_stream_reset(nsfrb_plan *pl)
 {
     if (!pl) return fail(NSFRB_EINVAL, "plan is null");
     pl->n_received = 0;
+    stream_reset(pl);
     return NSFRB_OK;
 }
 
@@ -505,6 +483,31 @@ int nsfrb_plan_get_info(const nsfrb_plan *pl, nsfrb_plan_info *info)
     info->block_len = kBlockLen; info->ring_len = pl->H; info->search_threads = kSearchWarps * 32;
     info->search_smem_bytes = (int64_t)pl->smem_search; info->workspace_bytes = (int64_t)pl->workspace_bytes;
     info->cells_per_pixel = pl->cells_per_pixel; info->shift_adds_per_pixel = pl->shift_adds_per_pixel;
+    return NSFRB_OK;
+}
+
+int nsfrb_jit_stream_kernel(int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s, const double *dm_list,
+                            int ndm, const int32_t *width_list, int nwidth, int chunk_nt, const char *variant, int want_cubin,
+                            char *out, size_t capacity, size_t *needed)
+{
+    if (!needed) return fail(NSFRB_EINVAL, "needed is null");
+    nsfrb_plan *pl = nullptr;
+    if (int rc = plan_host_init(&pl, nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, ndm, width_list, nwidth, 0.f)) return rc;
+    std::string src, err;
+    int rc = stream_source(pl, chunk_nt, variant, src, err);
+    free_plan(pl);
+    if (rc) return fail(rc, err);
+    std::vector<char> bin;
+    const char *data = src.data();
+    size_t n = src.size();
+    if (want_cubin) {
+        std::string log;
+        if ((rc = stream_compile(src, bin, log))) return fail(rc, log);
+        data = bin.data();
+        n = bin.size();
+    }
+    *needed = n;
+    if (out && capacity >= n) std::memcpy(out, data, n);
     return NSFRB_OK;
 }
 

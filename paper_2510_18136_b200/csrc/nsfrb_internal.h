@@ -5,6 +5,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <string>
+#include <vector>
+
 #include "../../include/nsfrb.h"
 
 namespace nsfrb {
@@ -51,6 +54,8 @@ struct SearchParams {
     int32_t wmax;
 };
 
+struct StreamState;
+
 struct FinalParams {
     const float *W;
     const int32_t *delays_u;
@@ -64,10 +69,76 @@ struct FinalParams {
     int32_t t_offset; // added to the reported t (streaming: lo mod 2^31)
 };
 
+} // namespace nsfrb
+
+// The plan: host tables + device workspace.  Opaque to callers (include/nsfrb.h).
+struct nsfrb_plan {
+    int nx = 0, ny = 0, npix = 0, nchan = 0, nt = 0, ndm = 0, nw = 0;
+    double tsamp = 0;
+    float threshold = 0;
+    std::vector<double> freqs, dms;
+    std::vector<int32_t> widths;
+    std::vector<int32_t> delays; // [ndm][nchan]
+    std::vector<int32_t> dmax;   // [ndm]
+    // unique trials, sorted by (dmax, first original index)
+    int nuniq = 0;
+    std::vector<int32_t> k_of_u, dmax_u, delays_u;
+    // widths that can hold at least one cell for some trial, original order
+    int nw_used = 0;
+    std::vector<int32_t> widths_used, j_of_used;
+    std::vector<int32_t> stream_worder; // indices into widths_used, ascending width (k_stream's W_TAB order)
+    int wmax_used = 0, dmax_all = 0, dmin_all = 0;
+    int n_groups = 0, n_wb = 0, H = 0, RS = 0, pitch = 0, tab_cap = 0;
+    std::vector<int32_t> dd_tab, dd_off; // per-group dedispersion change lists
+    size_t smem_search = 0, smem_final = 0;
+    int64_t cells_per_pixel = 0, shift_adds_per_pixel = 0;
+    // device
+    float *d_W = nullptr;
+    int32_t *d_dd_tab = nullptr, *d_dd_off = nullptr;
+    int32_t *d_delays_u = nullptr, *d_dmax_u = nullptr, *d_k_of_u = nullptr, *d_widths = nullptr, *d_j_of_used = nullptr;
+    nsfrb::Partial *d_partials = nullptr;
+    size_t workspace_bytes = 0;
+    // streaming state
+    int64_t n_received = 0;
+    // host-variant staging
+    float *d_in = nullptr;
+    size_t d_in_bytes = 0;
+    float *d_snr = nullptr;
+    int32_t *d_arg = nullptr;
+    nsfrb_cand *d_cands = nullptr;
+    uint32_t d_cands_cap = 0;
+    uint32_t *d_ncands = nullptr;
+    int last_launches = 0;
+    int device = 0;
+    // optional per-kernel timing
+    bool profiling = false;
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
+    // real-time path (nsfrb_stream.cu): ring, provisional means, plan-specialised kernel
+    nsfrb::StreamState *stream = nullptr;
+};
+
+namespace nsfrb {
+
+int plan_host_init(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
+                   const double *dm_list, int ndm, const int32_t *width_list, int nwidth, float threshold);
+void free_plan(nsfrb_plan *p);
+
+// ---- real-time path (nsfrb_stream.cu)
+void stream_free(nsfrb_plan *p);
+void stream_reset(nsfrb_plan *p);
+// a8 + k_stream passes + reduction over slices; outputs as nsfrb_stream_push.  Returns an NSFRB_* code and
+// leaves the message in `err`.
+int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t st, float *snr_map, int32_t *argmax,
+                int *launches, std::string &err);
+// Source text (prologue + kernel) and cubin of the plan's k_stream for a first chunk of chunk_nt samples;
+// no CUDA device needed.  `variant` = "" for the default tile shape or "KK,GPC,SEG,TT,MINB".
+int stream_source(const nsfrb_plan *pl, int chunk_nt, const char *variant, std::string &src, std::string &err);
+int stream_compile(const std::string &src, std::vector<char> &cubin, std::string &log);
+
+
 cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, int nt, int pitch,
                              cudaStream_t st);
-cudaError_t launch_push(const float *chunk, float *W, float *base, int npix, int nchan, int chunk_nt,
-                        int pitch, int ring_L, int slot0, int set_base, cudaStream_t st);
 cudaError_t launch_search(const SearchParams &p, size_t smem_bytes, cudaStream_t st);
 cudaError_t launch_finalize(const FinalParams &p, size_t smem_bytes, cudaStream_t st);
 cudaError_t launch_compact(const float *snr_map, const int32_t *argmax, int npix, float threshold,

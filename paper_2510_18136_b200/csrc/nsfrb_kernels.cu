@@ -1,6 +1,6 @@
 // sm_100a kernels of the NSFRB search hot path (steps a1..a8 of DESIGN.md):
-//   k_transpose / k_push : cube or chunk [chan][time][pixel] -> workspace W[pixel][chan][time]
-//                          (time-contiguous, per-channel baseline removed); a8 ring update
+//   k_transpose          : cube [chan][time][pixel] -> workspace W[pixel][chan][time]
+//                          (time-contiguous, per-channel baseline removed)
 //   k_search             : (nsfrb_search.cu) dedispersion (a2), mean/variance (a1, a3), prefix sum
 //                          (a4), boxcar + peak over time (a5), S/N + reduction over (DM, width)
 //                          of one DM group (a6, first half)
@@ -55,39 +55,6 @@ __global__ void __launch_bounds__(256) k_transpose(const float *__restrict__ cub
     for (int r = threadIdx.y; r < 32; r += 8) {
         const int p = p0 + r, t = t0 + threadIdx.x;
         if (t < nt && p < npix) W[((size_t)p * nchan + c) * (size_t)pitch + t] = tile[threadIdx.x][r];
-    }
-}
-
-// chunk[c][i][p] -> W[p][c][(slot0 + i) mod L] - base[c][p]; the first push defines base.
-__global__ void __launch_bounds__(256) k_push(const float *__restrict__ chunk, float *__restrict__ W,
-                                              float *__restrict__ base, int npix, int nchan, int chunk_nt,
-                                              int pitch, int ring_L, int slot0, int set_base)
-{
-    __shared__ float tile[32][33];
-    const int c = blockIdx.y;
-    const int p0 = blockIdx.x * 32;
-    const size_t chan0 = (size_t)c * chunk_nt * (size_t)npix;
-    const int pr = p0 + threadIdx.x;
-    float b = 0.f;
-    if (pr < npix) {
-        b = set_base ? __ldg(chunk + chan0 + pr) : base[(size_t)c * npix + pr];
-        if (set_base && threadIdx.y == 0) base[(size_t)c * npix + pr] = b;
-    }
-    for (int i0 = 0; i0 < chunk_nt; i0 += 32) {
-        for (int r = threadIdx.y; r < 32; r += 8) {
-            const int i = i0 + r;
-            if (i < chunk_nt && pr < npix) tile[r][threadIdx.x] = __ldg(chunk + chan0 + (size_t)i * npix + pr) - b;
-        }
-        __syncthreads();
-        for (int r = threadIdx.y; r < 32; r += 8) {
-            const int p = p0 + r, i = i0 + threadIdx.x;
-            if (i < chunk_nt && p < npix) {
-                int slot = slot0 + i;
-                if (slot >= ring_L) slot -= ring_L;
-                W[((size_t)p * nchan + c) * (size_t)pitch + slot] = tile[threadIdx.x][r];
-            }
-        }
-        __syncthreads();
     }
 }
 
@@ -244,14 +211,6 @@ cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, i
 {
     dim3 grid((npix + 31) / 32, (nt + 31) / 32, nchan), block(32, 8);
     k_transpose<<<grid, block, 0, st>>>(cube, W, npix, nchan, nt, pitch);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_push(const float *chunk, float *W, float *base, int npix, int nchan, int chunk_nt, int pitch,
-                        int ring_L, int slot0, int set_base, cudaStream_t st)
-{
-    dim3 grid((npix + 31) / 32, nchan), block(32, 8);
-    k_push<<<grid, block, 0, st>>>(chunk, W, base, npix, nchan, chunk_nt, pitch, ring_L, slot0, set_base);
     return cudaGetLastError();
 }
 
