@@ -9,19 +9,24 @@
 //
 // Prologue (see nsfrb_jit.cu: make_stream_prologue):
 //   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB     integers
-//   E_TAB[NU][NCHAN]   reverse-frame delays  e[u][c] = dmax_u - d[u][c]   (unique trials, DM ascending)
+//   D_TAB[NU][NCHAN]   integer delays d[u][c] of the unique trials, DM ascending
 //   DMAX_TAB[NU]       dmax_u                 K_OF_U[NU]  lowest original dm index of the trial
 //   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index
 //
 // Reverse frame.  The ring holds raw samples rho in [0, len); s = len-1-rho counts back from the
 // newest one.  Series u has T_u = len - dmax_u samples; its r-th sample from the end (r = 1..T_u) is
-//     D_u(r) = sum_c R[c][s = (r-1) + e[u][c]]
-// i.e. a dedispersion in reversed time with delays e, aligned over u at the ring's newest edge.
+//     D_u(r) = sum_c R[c][s = (r-1) + dmax_u - d[u][c]]
+// i.e. a dedispersion in reversed time.  The KK trials of a thread march together in the GROUP frame
+// rg = r - delta_u, delta_u = DMAXG - dmax_u (DMAXG = the group's largest dmax): there trial u reads
+// s = (rg-1) + e[u][c], e[u][c] = DMAXG - d[u][c], so consecutive trials differ only in the channels
+// whose delay differs (differential dedispersion keeps working), every trial of the group ends at the
+// same group step len - DMAXG, and the delta_u newest samples of trial u are covered by a masked lead-in.
 // With Q_u(r) = sum_{r'<=r} (D_u(r') - mu0_u) (suffix sums of the series), the boxcar of width w whose
 // window excludes the newest i samples is B(i, w) = Q(i+w) - Q(i); rule S5 (only windows whose last
 // raw sample arrived in this push) keeps exactly i in [0, chunk_nt) for every trial.  One backward
 // march therefore needs, per (pixel, trial): Q (register), Q at the C ends (shared memory, Qe) and
-// the running max per width (shared memory, M) -- no prefix history, no P ring.
+// the running max per width (M: one width at a time in registers, the rest in an L2-resident
+// workspace -- wide widths have disjoint start ranges) -- no prefix history, no P ring.
 //
 // Mapping.  Lane = pixel (the ring is pixel-contiguous: every load is one coalesced 128-byte row
 // segment).  Thread = 1 pixel x KK consecutive trials x 1 of SEG time segments.  A tile is TT steps:
@@ -31,8 +36,8 @@
 // a width's start range also evaluate its cells (a5).  Segments are cut between start ranges, so a
 // width belongs to one segment and its maxima are relative to that segment's offset, added at the end.
 // End of march: delta = S1/T, var = S2/T - delta^2, S = (M + Off - w delta)/(sigma sqrt(w)), reduced over
-// widths, trials and DM groups of the CTA (a6).  Raw rows for tile n+1 are requested before tile n
-// is computed (register double buffer).
+// widths, trials and DM groups of the CTA (a6).  The rows of tile n+1 are requested as soon as tile n's
+// dedispersion has consumed its rows (same registers), PFD tiles further ahead they are prefetched to L2.
 #ifndef NSFRB_STREAM_KERNEL_CUH
 #define NSFRB_STREAM_KERNEL_CUH
 
@@ -49,7 +54,9 @@ struct StreamParams {
     int len;     // valid raw samples in the ring
     int i0, C;   // this pass evaluates ends i in [i0, i0+C)
     int nslice, slice0;
-    int rfast;          // steps r <= rfast are valid for every trial (len - dmax_all, >= 0)
+    float *mws;         // running maxima  [pixel block][supergroup][GPC*KK][NW][32]  (global, L2-resident)
+    int *aws;           // their end indices, same shape
+    float *sws;         // segment totals S1, S2  [pixel block][supergroup][2][GPC*KK][SEG][32]
     int bound[9];       // segment q < SEG marches steps (bound[q], bound[q+1]], multiples of TT (SEG <= 8)
 };
 
@@ -75,7 +82,20 @@ template <int I, int N, class F> __device__ __forceinline__ void sfor(F &&f)
 // repeating the last trial, whose results are discarded)
 template <int G> struct GT {
     static __host__ __device__ constexpr int u(int kk) { return (G * KK + kk < NU) ? G * KK + kk : NU - 1; }
-    static __host__ __device__ constexpr int e(int kk, int c) { return E_TAB[u(kk)][c]; }
+    static __host__ __device__ constexpr int dmaxg()
+    {
+        int m = DMAX_TAB[u(0)];
+        for (int k = 1; k < KK; ++k) m = DMAX_TAB[u(k)] > m ? DMAX_TAB[u(k)] : m;
+        return m;
+    }
+    static __host__ __device__ constexpr int e(int kk, int c) { return dmaxg() - D_TAB[u(kk)][c]; }
+    static __host__ __device__ constexpr int delta(int kk) { return dmaxg() - DMAX_TAB[u(kk)]; } // own step = group step + delta
+    static __host__ __device__ constexpr int dspread()
+    {
+        int m = 0;
+        for (int k = 0; k < KK; ++k) m = delta(k) > m ? delta(k) : m;
+        return m;
+    }
     static __host__ __device__ constexpr int emin(int c)
     {
         int m = e(0, c);
@@ -102,13 +122,14 @@ template <int G> struct GT {
 constexpr int kThreads = 32 * GPC * SEG;
 constexpr int kTrialsPerCta = GPC * KK;
 
-// shared memory: Qe[kTrialsPerCta][CMAX][32], M[kTrialsPerCta][NW][32], A (uint8) same shape as M,
-// S1[kTrialsPerCta][SEG][32], S2 same, then the cross-group reduction scratch
+// shared memory: Qe[kTrialsPerCta][CMAX][32], the cross-group reduction scratch, and per (group, segment)
+// the range of widths that segment evaluated.  Segment totals S1, S2 [kTrialsPerCta][SEG][32] go through
+// the global workspace sws (written once per thread).
 constexpr int kQeFloats = kTrialsPerCta * CMAX * 32;
-constexpr int kMFloats = kTrialsPerCta * NW * 32;
 constexpr int kSegFloats = kTrialsPerCta * SEG * 32;
 constexpr int kRedFloats = GPC * 32 * 4;
-constexpr int kSmemBytes = (kQeFloats + kMFloats + 2 * kSegFloats + kRedFloats) * 4 + kMFloats /*A bytes*/;
+constexpr int kRangeInts = GPC * SEG * 2;
+constexpr int kSmemBytes = (kQeFloats + kRedFloats + kRangeInts) * 4;
 
 __device__ __forceinline__ float ldrow(const float *p) { return __ldg(p); }
 
@@ -116,18 +137,50 @@ template <int G> struct Worker {
     using T = GT<G>;
     const float *rp; // &ring[top_row][0][pixel]
     float *qe;       // &Qe[gl*KK][0][lane]
-    float *ms;       // &M [gl*KK][0][lane]
-    unsigned char *as; // &A[gl*KK][0][lane]
-    int lane, i0, C, len;
+    float *mg;       // &mws[block][gl*KK][0][lane]
+    int *ag;         // &aws[block][gl*KK][0][lane]
+    int i0, C, len;
     float carry[T::CARRY];
     float mu[KK], Q[KK], S2[KK];
     int ja, jb; // widths [ja, jb) can have cells in the current tile
+    // register cache of one width's running maxima (the rest live in mws/aws)
+    int jc, jfirst, jseen;
+    float mc[KK];
+    int ac[KK];
 
-    // element m of channel c's window at tile base rb lives at reverse raw index s = rb + m + emin(c)
-    template <int C_, int M_> __device__ __forceinline__ const float *addr(int rb) const
+    __device__ __forceinline__ void flush()
     {
-        return rp + ((long long)C_ - (long long)(M_ + T::emin(C_)) * NCHAN) * NPIX - (long long)rb * NCHAN * NPIX;
+        if (jc >= 0) {
+            float *mj = mg + jc * 32;
+            int *aj = ag + jc * 32;
+            sfor<0, KK>([&](auto kk) {
+                if constexpr (G * KK + V(kk) < NU) {
+                    mj[V(kk) * NW * 32] = mc[V(kk)];
+                    aj[V(kk) * NW * 32] = ac[V(kk)];
+                }
+            });
+        }
     }
+    __device__ __forceinline__ void fetch(int j)
+    {
+        flush();
+        if (j > jseen) { // first visit (widths are visited in ascending order)
+            sfor<0, KK>([&](auto kk) { mc[V(kk)] = -kInf; ac[V(kk)] = 0; });
+            jseen = j;
+            if (jfirst < 0) jfirst = j;
+        } else {
+            const float *mj = mg + j * 32;
+            const int *aj = ag + j * 32;
+            sfor<0, KK>([&](auto kk) {
+                if constexpr (G * KK + V(kk) < NU) {
+                    mc[V(kk)] = mj[V(kk) * NW * 32];
+                    ac[V(kk)] = aj[V(kk) * NW * 32];
+                }
+            });
+        }
+        jc = j;
+    }
+
     __device__ __forceinline__ void load_new(float (&buf)[NCHAN * TT], int rb) const
     {
         const float *b = rp - (long long)rb * NCHAN * NPIX;
@@ -135,6 +188,17 @@ template <int G> struct Worker {
             sfor<0, TT>([&](auto tt) {
                 constexpr long long off = ((long long)V(c) - (long long)(T::span(V(c)) + V(tt) + T::emin(V(c))) * NCHAN) * NPIX;
                 buf[V(c) * TT + V(tt)] = ldrow(b + off);
+            });
+        });
+    }
+    // ask L2 for the rows of the tile PFD tiles ahead (no registers held; the later loads hit L2)
+    __device__ __forceinline__ void prefetch_l2(int rb) const
+    {
+        const float *b = rp - (long long)rb * NCHAN * NPIX;
+        sfor<0, NCHAN>([&](auto c) {
+            sfor<0, TT>([&](auto tt) {
+                constexpr long long off = ((long long)V(c) - (long long)(T::span(V(c)) + V(tt) + T::emin(V(c))) * NCHAN) * NPIX;
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(b + off));
             });
         });
     }
@@ -149,17 +213,16 @@ template <int G> struct Worker {
         });
     }
 
-    // one tile: steps rb+1 .. rb+TT.  cur = the TT new rows of every channel; nxt receives the next tile's.
-    template <bool CELLS, bool MASKED>
-    __device__ __forceinline__ void tile(float (&cur)[NCHAN * TT], float (&nxt)[NCHAN * TT], int rb, bool prefetch)
+    // One tile: group steps rb+1 .. rb+TT.  On entry cur holds the TT new rows of every channel; on exit
+    // (if `more`) the rows of the next tile have been requested into the same registers.
+    template <bool CELLS, bool MASKED, bool QE> __device__ __forceinline__ void tile(float (&cur)[NCHAN * TT], int rb, bool more, bool pf)
     {
-        if (prefetch) load_new(nxt, rb + TT);
         auto Wn = [&](auto c, auto m) -> float {
             if constexpr (V(m) < T::span(V(c))) return carry[T::coff(V(c)) + V(m)];
             else return cur[V(c) * TT + (V(m) - T::span(V(c)))];
         };
-        float D[TT];
-        float Qs[KK][TT];
+        // a2: first trial = plain channel sum, every next one differentially
+        float Dv[KK][TT];
         sfor<0, KK>([&](auto kk) {
             if constexpr (V(kk) == 0) {
                 sfor<0, TT>([&](auto tt) {
@@ -168,7 +231,7 @@ template <int G> struct Worker {
                         const float v = Wn(c, IC<V(tt) + T::o(0, V(c))>{});
                         if constexpr ((V(c) & 1) == 0) a0 += v; else a1 += v;
                     });
-                    D[V(tt)] = a0 + a1;
+                    Dv[0][V(tt)] = a0 + a1;
                 });
             } else {
                 sfor<0, TT>([&](auto tt) {
@@ -177,58 +240,81 @@ template <int G> struct Worker {
                         if constexpr (T::o(V(kk), V(c)) != T::o(V(kk) - 1, V(c)))
                             a += Wn(c, IC<V(tt) + T::o(V(kk), V(c))>{}) - Wn(c, IC<V(tt) + T::o(V(kk) - 1, V(c))>{});
                     });
-                    D[V(tt)] += a;
+                    Dv[V(kk)][V(tt)] = Dv[V(kk) - 1][V(tt)] + a;
                 });
             }
-            // a1, a3, a4: centred sample, suffix sum, sum of squares
+        });
+        // carry the halo: next tile's element m is this tile's element m + TT
+        {
+            float nc[T::CARRY];
+            sfor<0, NCHAN>([&](auto c) {
+                sfor<0, T::span(V(c))>([&](auto m) { nc[T::coff(V(c)) + V(m)] = Wn(c, IC<V(m) + TT>{}); });
+            });
+            sfor<0, T::CARRY>([&](auto i) { carry[V(i)] = nc[V(i)]; });
+        }
+        if (more) load_new(cur, rb + TT); // rows of the next tile; their latency overlaps what follows
+        if (PFD > 0 && pf) prefetch_l2(rb + PFD * TT);
+        // a1, a3, a4: centred sample, suffix sum (left in Dv), sum of squares
+        sfor<0, KK>([&](auto kk) {
             sfor<0, TT>([&](auto tt) {
-                float x = D[V(tt)] - mu[V(kk)];
-                if constexpr (MASKED) x = ((rb + 1 + V(tt)) <= len - DMAX_TAB[T::u(V(kk))]) ? x : 0.f;
+                float x = Dv[V(kk)][V(tt)] - mu[V(kk)];
+                if constexpr (MASKED) {
+                    const int ro = rb + 1 + V(tt) + T::delta(V(kk)); // step in the trial's own frame
+                    x = (ro >= 1 && ro <= len - DMAX_TAB[T::u(V(kk))]) ? x : 0.f;
+                }
                 Q[V(kk)] += x;
                 S2[V(kk)] = fmaf(x, x, S2[V(kk)]);
-                Qs[V(kk)][V(tt)] = Q[V(kk)];
+                Dv[V(kk)][V(tt)] = Q[V(kk)];
             });
-            if constexpr (CELLS) {
-                if (G * KK + V(kk) < NU) {
-                    // Q at the ends of this pass: Qe[ii] = Q(i0 + ii)
+        });
+        if constexpr (QE) {
+            // Q at the ends of this pass: Qe[ii] = Q(i0 + ii), own frame
+            float *qb = qe + (rb + 1 - i0) * 32;
+            sfor<0, KK>([&](auto kk) {
+                if constexpr (G * KK + V(kk) < NU)
                     sfor<0, TT>([&](auto tt) {
-                        const int ii = rb + 1 + V(tt) - i0;
-                        if (ii >= 0 && ii < C) qe[(V(kk) * CMAX + ii) * 32] = Qs[V(kk)][V(tt)];
+                        const unsigned ii = (unsigned)(rb + 1 - i0 + V(tt) + T::delta(V(kk)));
+                        if (ii < (unsigned)C) qb[(V(kk) * CMAX + V(tt) + T::delta(V(kk))) * 32] = Dv[V(kk)][V(tt)];
+                    });
+            });
+        }
+        if constexpr (CELLS) {
+            // a5: widths whose start range [w+i0, w+i0+C-1] (own frame) meets this tile
+            while (ja < NW && W_TAB[ja] + i0 + C - 1 < rb + 1) ++ja;
+            if (jb < ja) jb = ja;
+            while (jb < NW && W_TAB[jb] + i0 <= rb + TT + T::dspread()) ++jb;
+            for (int j = ja; j < jb; ++j) {
+                if (j != jc) fetch(j);
+                const int ib = rb + 1 - W_TAB[j] - i0; // end index (relative to i0) of group step rb+1 at delta = 0
+                const float *qb = qe + ib * 32;        // &Qe[0][ib]: every access below is a static offset from it
+                const bool inside = !MASKED && ib >= 0 && ib + TT - 1 + T::dspread() < C;
+                if (inside) { // every cell of the tile is defined: no range checks
+                    sfor<0, KK>([&](auto kk) {
+                        if constexpr (G * KK + V(kk) < NU)
+                            sfor<0, TT>([&](auto tt) {
+                                const float v = Dv[V(kk)][V(tt)] - qb[(V(kk) * CMAX + V(tt) + T::delta(V(kk))) * 32];
+                                if (v >= mc[V(kk)]) { mc[V(kk)] = v; ac[V(kk)] = ib + V(tt) + T::delta(V(kk)); }
+                            });
+                    });
+                } else {
+                    sfor<0, KK>([&](auto kk) {
+                        if constexpr (G * KK + V(kk) < NU)
+                            sfor<0, TT>([&](auto tt) {
+                                const int ii = ib + V(tt) + T::delta(V(kk));
+                                bool in = (unsigned)ii < (unsigned)C;
+                                if constexpr (MASKED) {
+                                    const int ro = rb + 1 + V(tt) + T::delta(V(kk));
+                                    in = in && ro >= 1 && ro <= len - DMAX_TAB[T::u(V(kk))];
+                                }
+                                if (in) {
+                                    const float v = Dv[V(kk)][V(tt)] - qb[(V(kk) * CMAX + V(tt) + T::delta(V(kk))) * 32];
+                                    if (v >= mc[V(kk)]) { mc[V(kk)] = v; ac[V(kk)] = ii; } // later step = earlier start
+                                }
+                            });
                     });
                 }
             }
-        });
-        if constexpr (CELLS) {
-            // a5: widths whose start range [w+i0, w+i0+C-1] meets this tile
-            while (ja < NW && W_TAB[ja] + i0 + C - 1 < rb + 1) ++ja;
-            while (jb < NW && W_TAB[jb] + i0 <= rb + TT) ++jb;
-            for (int j = ja; j < jb; ++j) {
-                const int ib = rb + 1 - W_TAB[j] - i0; // end index (relative to i0) of step rb+1
-                sfor<0, KK>([&](auto kk) {
-                    if (G * KK + V(kk) < NU) {
-                        float m = ms[(V(kk) * NW + j) * 32];
-                        int a = as[(V(kk) * NW + j) * 32];
-                        sfor<0, TT>([&](auto tt) {
-                            const int ii = ib + V(tt);
-                            bool in = (ii >= 0) && (ii < C);
-                            if constexpr (MASKED) in = in && ((rb + 1 + V(tt)) <= len - DMAX_TAB[T::u(V(kk))]);
-                            if (in) {
-                                const float v = Qs[V(kk)][V(tt)] - qe[(V(kk) * CMAX + ii) * 32];
-                                if (v >= m) { m = v; a = ii; } // later step = earlier start: ties go to the smaller t
-                            }
-                        });
-                        ms[(V(kk) * NW + j) * 32] = m;
-                        as[(V(kk) * NW + j) * 32] = (unsigned char)a;
-                    }
-                });
-            }
         }
-        // carry the halo: next tile's element m is this tile's element m + TT
-        float nc[T::CARRY];
-        sfor<0, NCHAN>([&](auto c) {
-            sfor<0, T::span(V(c))>([&](auto m) { nc[T::coff(V(c)) + V(m)] = Wn(c, IC<V(m) + TT>{}); });
-        });
-        sfor<0, T::CARRY>([&](auto i) { carry[V(i)] = nc[V(i)]; });
     }
 };
 
@@ -245,87 +331,94 @@ __device__ __forceinline__ bool better(float s, int k, int j, int t, float bs, i
     return t < bt;
 }
 
-template <int G> __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, int gl, int seg, int lane, int pix, bool live)
+template <int G>
+__device__ __forceinline__ void run_group(const StreamParams &P, float *smem, int gl, int seg, int lane, int pix, bool live)
 {
     using T = GT<G>;
     float *Qe = smem;
-    float *Ms = Qe + kQeFloats;
-    float *S1s = Ms + kMFloats;
+    float *red = Qe + kQeFloats;
+    float *S1s = P.sws + ((long long)blockIdx.x * NSUPER + blockIdx.y) * 2 * kSegFloats;
     float *S2s = S1s + kSegFloats;
-    float *red = S2s + kSegFloats;
-    unsigned char *As = reinterpret_cast<unsigned char *>(red + kRedFloats);
+    int *rng = reinterpret_cast<int *>(red + kRedFloats);
 
     Worker<G> w;
-    w.lane = lane; w.i0 = P.i0; w.C = P.C; w.len = P.len;
+    w.i0 = P.i0; w.C = P.C; w.len = P.len;
     w.rp = P.ring + ((long long)P.top_row * NCHAN) * NPIX + pix;
     w.qe = Qe + (gl * KK) * CMAX * 32 + lane;
-    w.ms = Ms + (gl * KK) * NW * 32 + lane;
-    w.as = As + (gl * KK) * NW * 32 + lane;
-    w.ja = 0; w.jb = 0;
+    {
+        const long long blk = ((long long)blockIdx.x * NSUPER + blockIdx.y) * kTrialsPerCta + gl * KK;
+        w.mg = P.mws + blk * NW * 32 + lane;
+        w.ag = P.aws + blk * NW * 32 + lane;
+    }
+    w.ja = 0; w.jb = 0; w.jc = -1; w.jfirst = -1; w.jseen = -1;
     sfor<0, KK>([&](auto kk) {
         w.mu[V(kk)] = P.mu0[(long long)T::u(V(kk)) * NPIX + pix];
         w.Q[V(kk)] = 0.f;
         w.S2[V(kk)] = 0.f;
+        w.mc[V(kk)] = -kInf;
+        w.ac[V(kk)] = 0;
     });
-    // this thread initialises the M/A slots of its trials for the widths of its segment ... all segments
-    // share the slots, so segment 0 initialises everything before the first barrier
-    if (seg == 0) {
-        for (int j = 0; j < NW; ++j)
-            sfor<0, KK>([&](auto kk) {
-                w.ms[(V(kk) * NW + j) * 32] = -kInf;
-                w.as[(V(kk) * NW + j) * 32] = 0;
-            });
-        if (P.i0 == 0) sfor<0, KK>([&](auto kk) { w.qe[(V(kk) * CMAX) * 32] = 0.f; });
-    }
+    if (seg == 0 && P.i0 == 0) sfor<0, KK>([&](auto kk) { w.qe[(V(kk) * CMAX) * 32] = 0.f; });
 
-    const int r_begin = P.bound[seg], r_end = P.bound[seg + 1];
-    const int qe_end = P.i0 + P.C; // steps < qe_end store Qe (they all lie in segment 0)
+    // group frame: segment 0 starts with the masked lead-in that covers the newest delta_u samples
+    constexpr int kLead = (T::dspread() + TT - 1) / TT * TT;
+    const int r_begin = seg == 0 ? -kLead : P.bound[seg], r_end = P.bound[seg + 1];
+    const int r_fast_end = P.len - T::dmaxg(); // last group step (valid for every trial of the group)
+    const int qe_end = P.i0 + P.C;             // group steps < qe_end may store Qe (they lie in segment 0)
+    const bool pf = true;
     bool synced = false;
     if (r_begin < r_end) {
-        float bufA[NCHAN * TT], bufB[NCHAN * TT];
+        float cur[NCHAN * TT];
         w.load_carry(r_begin);
-        w.load_new(bufA, r_begin);
+        w.load_new(cur, r_begin);
         int rb = r_begin;
-        bool flip = false;
         while (rb < r_end) {
-            const bool pf = rb + TT < r_end;
-            const bool masked = rb + TT > P.rfast;
-            // does the tile store ends or touch a start range?
+            if (seg == 0 && !synced && rb >= qe_end) { // every Qe of this pass is written
+                bar_named(1, kThreads);
+                synced = true;
+            }
+            const bool masked = rb < 0 || rb + TT > r_fast_end;
             bool cells = rb < qe_end;
             if (!cells) {
                 int ja = w.ja;
                 while (ja < NW && W_TAB[ja] + P.i0 + P.C - 1 < rb + 1) ++ja;
                 w.ja = ja;
-                cells = ja < NW && W_TAB[ja] + P.i0 <= rb + TT;
+                cells = ja < NW && W_TAB[ja] + P.i0 <= rb + TT + T::dspread();
             }
-            if (cells && seg != 0 && !synced) { // Qe is complete once segment 0 has passed qe_end
-                bar_named(1, kThreads);
-                synced = true;
-            }
-            if (!flip) {
-                if (masked) w.template tile<true, true>(bufA, bufB, rb, pf);
-                else if (cells) w.template tile<true, false>(bufA, bufB, rb, pf);
-                else w.template tile<false, false>(bufA, bufB, rb, pf);
+            if (masked || cells) {
+                if (cells && seg != 0 && !synced) { // Qe is complete once segment 0 has passed qe_end
+                    bar_named(1, kThreads);
+                    synced = true;
+                }
+                if (masked) w.template tile<true, true, true>(cur, rb, rb + TT < r_end, pf);
+                else if (rb < qe_end) w.template tile<true, false, true>(cur, rb, rb + TT < r_end, pf);
+                else w.template tile<true, false, false>(cur, rb, rb + TT < r_end, pf);
+                rb += TT;
             } else {
-                if (masked) w.template tile<true, true>(bufB, bufA, rb, pf);
-                else if (cells) w.template tile<true, false>(bufB, bufA, rb, pf);
-                else w.template tile<false, false>(bufB, bufA, rb, pf);
-            }
-            flip = !flip;
-            rb += TT;
-            if (seg == 0 && !synced && rb >= qe_end) {
-                bar_named(1, kThreads);
-                synced = true;
+                // plain run: up to the next start range, the masked tail or the end of the segment
+                const int wnext = w.ja < NW ? W_TAB[w.ja] + P.i0 - T::dspread() : 0x3fffffff;
+                int stop = r_end;
+                if (r_fast_end - TT + 1 < stop) stop = r_fast_end - TT + 1; // rb < stop  <=>  rb + TT <= r_fast_end
+                if (wnext - TT < stop) stop = wnext - TT;                   // rb < stop  <=>  rb + TT < wnext
+                do {
+                    w.template tile<false, false, false>(cur, rb, rb + TT < r_end, pf);
+                    rb += TT;
+                } while (rb < stop);
             }
         }
     }
+    w.flush();
     if (!synced) bar_named(1, kThreads);
 
-    // segment totals
+    // segment totals and the widths this segment evaluated
     sfor<0, KK>([&](auto kk) {
         S1s[((gl * KK + V(kk)) * SEG + seg) * 32 + lane] = w.Q[V(kk)];
         S2s[((gl * KK + V(kk)) * SEG + seg) * 32 + lane] = w.S2[V(kk)];
     });
+    if (lane == 0) {
+        rng[(gl * SEG + seg) * 2 + 0] = w.jfirst;
+        rng[(gl * SEG + seg) * 2 + 1] = w.jseen;
+    }
     bar_named(2, kThreads);
 
     // a6: exact mean/variance, normalise, reduce over widths and trials (segment-0 threads)
@@ -349,21 +442,22 @@ template <int G> __device__ __forceinline__ void run_group(const StreamParams &P
                     const float var = fmaxf(fmaf(-delta, delta, s2 * invT), 0.f);
                     const float sigma = sqrtf(var);
                     if (P.slice0 == 0 && live) P.mu0[(long long)u * NPIX + pix] = w.mu[V(kk)] + delta;
-                    for (int j = 0; j < NW; ++j) {
-                        const float m = w.ms[(V(kk) * NW + j) * 32];
-                        if (m > -kInf) {
-                            const int wj = W_TAB[j];
-                            const int rj = wj + P.i0; // first start step of the width: fixes its segment
-                            float o = 0.f;
-                            sfor<1, SEG>([&](auto q) { if (rj > P.bound[V(q)]) o = off[V(q)]; });
-                            const float fw = (float)wj;
-                            const float B = fmaf(-fw, delta, m + o);
-                            const float S = sigma > 0.f ? B / (sigma * sqrtf(fw)) : 0.f;
-                            const int ii = P.i0 + (int)w.as[(V(kk) * NW + j) * 32];
-                            const int t = Tk - ii - wj;
-                            if (better(S, K_OF_U[u], J_OF_W[j], t, bs, bk, bj, bt)) { bs = S; bk = K_OF_U[u]; bj = J_OF_W[j]; bt = t; }
-                        }
-                    }
+                    sfor<0, SEG>([&](auto q) {
+                        const int j0 = rng[(gl * SEG + V(q)) * 2 + 0], j1 = rng[(gl * SEG + V(q)) * 2 + 1];
+                        if (j0 >= 0)
+                            for (int j = j0; j <= j1; ++j) {
+                                const float m = w.mg[(V(kk) * NW + j) * 32];
+                                if (m > -kInf) {
+                                    const int wj = W_TAB[j];
+                                    const float fw = (float)wj;
+                                    const float B = fmaf(-fw, delta, m + off[V(q)]);
+                                    const float S = sigma > 0.f ? B / (sigma * sqrtf(fw)) : 0.f;
+                                    const int ii = P.i0 + w.ag[(V(kk) * NW + j) * 32];
+                                    const int t = Tk - ii - wj;
+                                    if (better(S, K_OF_U[u], J_OF_W[j], t, bs, bk, bj, bt)) { bs = S; bk = K_OF_U[u]; bj = J_OF_W[j]; bt = t; }
+                                }
+                            }
+                    });
                 }
             }
         });
@@ -387,7 +481,8 @@ template <int G> __device__ __forceinline__ void run_group(const StreamParams &P
     }
 }
 
-template <int G0, int N> __device__ __forceinline__ void dispatch(int g, const StreamParams &P, float *smem, int gl, int seg, int lane, int pix, bool live)
+template <int G0, int N>
+__device__ __forceinline__ void dispatch(int g, const StreamParams &P, float *smem, int gl, int seg, int lane, int pix, bool live)
 {
     if constexpr (N == 1) {
         run_group<G0>(P, smem, gl, seg, lane, pix, live);
@@ -404,11 +499,11 @@ extern "C" __global__ void __launch_bounds__(sk::kThreads, MINB) k_stream(const 
     extern __shared__ __align__(16) float smem[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int gl = warp / SEG, seg = warp - gl * SEG;
-    // pixel blocks past NPIX clamp to the last pixel (loads stay in bounds; the store is skipped)
+    // lanes past NPIX work on the last pixel (loads stay in bounds) and skip their stores
     int pix = blockIdx.x * 32 + lane;
     const bool live = pix < NPIX;
     if (!live) pix = NPIX - 1;
-    const int g = blockIdx.y * GPC + gl; // DM group of this warp; NSUPER*GPC groups exist (padded)
+    const int g = blockIdx.y * GPC + gl; // DM group of this warp; NSUPER*GPC groups exist (the last may be padding)
     sk::dispatch<0, NSUPER * GPC>(g, P, smem, gl, seg, lane, pix, live);
 }
 
