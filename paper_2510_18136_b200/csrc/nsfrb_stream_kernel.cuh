@@ -8,7 +8,7 @@
 // ahead of time with the BASELINE config-2 prologue as a build check.
 //
 // Prologue (see nsfrb_jit.cu: make_stream_prologue):
-//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB     integers
+//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD DBUF   integers
 //   D_TAB[NU][NCHAN]   integer delays d[u][c] of the unique trials, DM ascending
 //   DMAX_TAB[NU]       dmax_u                 K_OF_U[NU]  lowest original dm index of the trial
 //   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index
@@ -28,8 +28,9 @@
 // the running max per width (M: one width at a time in registers, the rest in an L2-resident
 // workspace -- wide widths have disjoint start ranges) -- no prefix history, no P ring.
 //
-// Mapping.  Lane = pixel (the ring is pixel-contiguous: every load is one coalesced 128-byte row
-// segment).  Thread = 1 pixel x KK consecutive trials x 1 of SEG time segments.  A tile is TT steps:
+// Mapping.  Lane = pixel.  The ring is stored per block of 32 pixels, [block][row][chan][32]: every load is
+// one coalesced 128-byte segment and a warp streams through one contiguous region (a tile's new rows are
+// TT*NCHAN*128 contiguous bytes), which is what HBM row buffers and the TLB want.  Thread = 1 pixel x KK consecutive trials x 1 of SEG time segments.  A tile is TT steps:
 // the thread holds the raw window of every channel in registers (TT new rows + a carried halo of
 // span_c = max_kk e - min_kk e rows), forms D for its first trial as the plain channel sum and every
 // next trial differentially (a2), then x = D - mu0, Q += x, S2 += x^2 (a1, a3, a4).  Tiles that touch
@@ -47,7 +48,7 @@ struct SPartial { // per (pixel, slice): slice = pass * NSUPER + supergroup
 };
 
 struct StreamParams {
-    const float *ring; // [rows][NCHAN][NPIX], baseline removed, every sample stored at slot and slot+L
+    const float *ring; // [pixel block][ROWS][NCHAN][32], baseline removed, every sample stored at slot and slot+L
     float *mu0;        // [NU][NPIX] provisional means (the previous push's exact means); updated
     SPartial *partials;
     int top_row; // row of the newest sample
@@ -141,7 +142,7 @@ template <int G> struct Worker {
     int *ag;         // &aws[block][gl*KK][0][lane]
     int i0, C, len;
     float carry[T::CARRY];
-    float mu[KK], Q[KK], S2[KK];
+    float mu[KK], dmu[KK], Q[KK], S2[KK]; // mu: provisional means (mu[0] and the differences dmu are live in the loop)
     int ja, jb; // widths [ja, jb) can have cells in the current tile
     // register cache of one width's running maxima (the rest live in mws/aws)
     int jc, jfirst, jseen;
@@ -183,31 +184,37 @@ template <int G> struct Worker {
 
     __device__ __forceinline__ void load_new(float (&buf)[NCHAN * TT], int rb) const
     {
-        const float *b = rp - (long long)rb * NCHAN * NPIX;
+        const float *b = rp - (long long)rb * (NCHAN * 32);
         sfor<0, NCHAN>([&](auto c) {
             sfor<0, TT>([&](auto tt) {
-                constexpr long long off = ((long long)V(c) - (long long)(T::span(V(c)) + V(tt) + T::emin(V(c))) * NCHAN) * NPIX;
+                constexpr int off = (V(c) - (T::span(V(c)) + V(tt) + T::emin(V(c))) * NCHAN) * 32;
+#if HACK == 2
+                buf[V(c) * TT + V(tt)] = __int_as_float(0x3f800000 + rb * 64 + off); // EXPERIMENT: no memory traffic
+#elif HACK == 1
+                buf[V(c) * TT + V(tt)] = ldrow(rp + off - (rb & 15) * (NCHAN * 32)); // EXPERIMENT: L1-resident rows
+#else
                 buf[V(c) * TT + V(tt)] = ldrow(b + off);
+#endif
             });
         });
     }
     // ask L2 for the rows of the tile PFD tiles ahead (no registers held; the later loads hit L2)
     __device__ __forceinline__ void prefetch_l2(int rb) const
     {
-        const float *b = rp - (long long)rb * NCHAN * NPIX;
+        const float *b = rp - (long long)rb * (NCHAN * 32);
         sfor<0, NCHAN>([&](auto c) {
             sfor<0, TT>([&](auto tt) {
-                constexpr long long off = ((long long)V(c) - (long long)(T::span(V(c)) + V(tt) + T::emin(V(c))) * NCHAN) * NPIX;
+                constexpr int off = (V(c) - (T::span(V(c)) + V(tt) + T::emin(V(c))) * NCHAN) * 32;
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(b + off));
             });
         });
     }
     __device__ __forceinline__ void load_carry(int rb)
     {
-        const float *b = rp - (long long)rb * NCHAN * NPIX;
+        const float *b = rp - (long long)rb * (NCHAN * 32);
         sfor<0, NCHAN>([&](auto c) {
             sfor<0, T::span(V(c))>([&](auto m) {
-                constexpr long long off = ((long long)V(c) - (long long)(V(m) + T::emin(V(c))) * NCHAN) * NPIX;
+                constexpr int off = (V(c) - (V(m) + T::emin(V(c))) * NCHAN) * 32;
                 carry[T::coff(V(c)) + V(m)] = ldrow(b + off);
             });
         });
@@ -215,8 +222,14 @@ template <int G> struct Worker {
 
     // One tile: group steps rb+1 .. rb+TT.  On entry cur holds the TT new rows of every channel; on exit
     // (if `more`) the rows of the next tile have been requested into the same registers.
-    template <bool CELLS, bool MASKED, bool QE> __device__ __forceinline__ void tile(float (&cur)[NCHAN * TT], int rb, bool more, bool pf)
+    // `cells`: the tile stores ends or meets a start range (one code body serves plain and cell tiles: the
+    // hot instruction footprint of an SM has to stay within the ~32 KB the instruction cache streams well)
+    template <bool MASKED> __device__ __forceinline__ void tile(float (&cur)[NCHAN * TT], int rb, bool more, bool pf, bool cells)
     {
+#if DBUF
+        float nxt[NCHAN * TT];
+        if (more) load_new(nxt, rb + TT);
+#endif
         auto Wn = [&](auto c, auto m) -> float {
             if constexpr (V(m) < T::span(V(c))) return carry[T::coff(V(c)) + V(m)];
             else return cur[V(c) * TT + (V(m) - T::span(V(c)))];
@@ -226,7 +239,7 @@ template <int G> struct Worker {
         sfor<0, KK>([&](auto kk) {
             if constexpr (V(kk) == 0) {
                 sfor<0, TT>([&](auto tt) {
-                    float a0 = 0.f, a1 = 0.f;
+                    float a0 = -mu[0], a1 = 0.f; // centred on the provisional mean of trial 0
                     sfor<0, NCHAN>([&](auto c) {
                         const float v = Wn(c, IC<V(tt) + T::o(0, V(c))>{});
                         if constexpr ((V(c) & 1) == 0) a0 += v; else a1 += v;
@@ -235,7 +248,7 @@ template <int G> struct Worker {
                 });
             } else {
                 sfor<0, TT>([&](auto tt) {
-                    float a = 0.f;
+                    float a = dmu[V(kk)]; // mu0[kk-1] - mu0[kk]: keeps every trial centred on its own provisional mean
                     sfor<0, NCHAN>([&](auto c) {
                         if constexpr (T::o(V(kk), V(c)) != T::o(V(kk) - 1, V(c)))
                             a += Wn(c, IC<V(tt) + T::o(V(kk), V(c))>{}) - Wn(c, IC<V(tt) + T::o(V(kk) - 1, V(c))>{});
@@ -252,12 +265,14 @@ template <int G> struct Worker {
             });
             sfor<0, T::CARRY>([&](auto i) { carry[V(i)] = nc[V(i)]; });
         }
+#if !DBUF
         if (more) load_new(cur, rb + TT); // rows of the next tile; their latency overlaps what follows
+#endif
         if (PFD > 0 && pf) prefetch_l2(rb + PFD * TT);
         // a1, a3, a4: centred sample, suffix sum (left in Dv), sum of squares
         sfor<0, KK>([&](auto kk) {
             sfor<0, TT>([&](auto tt) {
-                float x = Dv[V(kk)][V(tt)] - mu[V(kk)];
+                float x = Dv[V(kk)][V(tt)];
                 if constexpr (MASKED) {
                     const int ro = rb + 1 + V(tt) + T::delta(V(kk)); // step in the trial's own frame
                     x = (ro >= 1 && ro <= len - DMAX_TAB[T::u(V(kk))]) ? x : 0.f;
@@ -267,7 +282,7 @@ template <int G> struct Worker {
                 Dv[V(kk)][V(tt)] = Q[V(kk)];
             });
         });
-        if constexpr (QE) {
+        if (cells && rb < i0 + C) {
             // Q at the ends of this pass: Qe[ii] = Q(i0 + ii), own frame
             float *qb = qe + (rb + 1 - i0) * 32;
             sfor<0, KK>([&](auto kk) {
@@ -278,7 +293,7 @@ template <int G> struct Worker {
                     });
             });
         }
-        if constexpr (CELLS) {
+        if (cells) {
             // a5: widths whose start range [w+i0, w+i0+C-1] (own frame) meets this tile
             while (ja < NW && W_TAB[ja] + i0 + C - 1 < rb + 1) ++ja;
             if (jb < ja) jb = ja;
@@ -315,6 +330,9 @@ template <int G> struct Worker {
                 }
             }
         }
+#if DBUF
+        if (more) sfor<0, NCHAN * TT>([&](auto i) { cur[V(i)] = nxt[V(i)]; });
+#endif
     }
 };
 
@@ -343,7 +361,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
 
     Worker<G> w;
     w.i0 = P.i0; w.C = P.C; w.len = P.len;
-    w.rp = P.ring + ((long long)P.top_row * NCHAN) * NPIX + pix;
+    w.rp = P.ring + ((long long)blockIdx.x * ROWS + P.top_row) * (NCHAN * 32) + lane;
     w.qe = Qe + (gl * KK) * CMAX * 32 + lane;
     {
         const long long blk = ((long long)blockIdx.x * NSUPER + blockIdx.y) * kTrialsPerCta + gl * KK;
@@ -355,9 +373,11 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
         w.mu[V(kk)] = P.mu0[(long long)T::u(V(kk)) * NPIX + pix];
         w.Q[V(kk)] = 0.f;
         w.S2[V(kk)] = 0.f;
+        w.dmu[V(kk)] = 0.f;
         w.mc[V(kk)] = -kInf;
         w.ac[V(kk)] = 0;
     });
+    sfor<1, KK>([&](auto kk) { w.dmu[V(kk)] = w.mu[V(kk) - 1] - w.mu[V(kk)]; });
     if (seg == 0 && P.i0 == 0) sfor<0, KK>([&](auto kk) { w.qe[(V(kk) * CMAX) * 32] = 0.f; });
 
     // group frame: segment 0 starts with the masked lead-in that covers the newest delta_u samples
@@ -365,46 +385,43 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     const int r_begin = seg == 0 ? -kLead : P.bound[seg], r_end = P.bound[seg + 1];
     const int r_fast_end = P.len - T::dmaxg(); // last group step (valid for every trial of the group)
     const int qe_end = P.i0 + P.C;             // group steps < qe_end may store Qe (they lie in segment 0)
-    const bool pf = true;
+    const bool pf = gl == 0; // the DM groups of a pixel block read the same rows: one of them prefetches
     bool synced = false;
     if (r_begin < r_end) {
         float cur[NCHAN * TT];
         w.load_carry(r_begin);
         w.load_new(cur, r_begin);
         int rb = r_begin;
+        int plain_until = r_begin; // exclusive
         while (rb < r_end) {
             if (seg == 0 && !synced && rb >= qe_end) { // every Qe of this pass is written
                 bar_named(1, kThreads);
                 synced = true;
             }
             const bool masked = rb < 0 || rb + TT > r_fast_end;
-            bool cells = rb < qe_end;
-            if (!cells) {
-                int ja = w.ja;
-                while (ja < NW && W_TAB[ja] + P.i0 + P.C - 1 < rb + 1) ++ja;
-                w.ja = ja;
-                cells = ja < NW && W_TAB[ja] + P.i0 <= rb + TT + T::dspread();
-            }
-            if (masked || cells) {
+            bool cells = rb >= plain_until; // tiles below plain_until are known to hold no end and no start
+            if (cells) {
+                cells = rb < qe_end;
+                if (!cells) {
+                    int ja = w.ja;
+                    while (ja < NW && W_TAB[ja] + P.i0 + P.C - 1 < rb + 1) ++ja;
+                    w.ja = ja;
+                    const int wnext = ja < NW ? W_TAB[ja] + P.i0 - T::dspread() : 0x3fffffff; // first step of the next start range
+                    cells = wnext <= rb + TT;
+                    if (!cells) { // a plain run begins: nothing stays cached across it
+                        plain_until = wnext - TT; // rb < plain_until  <=>  rb + TT < wnext
+                        w.flush();
+                        w.jc = -1;
+                    }
+                }
                 if (cells && seg != 0 && !synced) { // Qe is complete once segment 0 has passed qe_end
                     bar_named(1, kThreads);
                     synced = true;
                 }
-                if (masked) w.template tile<true, true, true>(cur, rb, rb + TT < r_end, pf);
-                else if (rb < qe_end) w.template tile<true, false, true>(cur, rb, rb + TT < r_end, pf);
-                else w.template tile<true, false, false>(cur, rb, rb + TT < r_end, pf);
-                rb += TT;
-            } else {
-                // plain run: up to the next start range, the masked tail or the end of the segment
-                const int wnext = w.ja < NW ? W_TAB[w.ja] + P.i0 - T::dspread() : 0x3fffffff;
-                int stop = r_end;
-                if (r_fast_end - TT + 1 < stop) stop = r_fast_end - TT + 1; // rb < stop  <=>  rb + TT <= r_fast_end
-                if (wnext - TT < stop) stop = wnext - TT;                   // rb < stop  <=>  rb + TT < wnext
-                do {
-                    w.template tile<false, false, false>(cur, rb, rb + TT < r_end, pf);
-                    rb += TT;
-                } while (rb < stop);
             }
+            if (masked) w.template tile<true>(cur, rb, rb + TT < r_end, pf, true);
+            else w.template tile<false>(cur, rb, rb + TT < r_end, pf, cells);
+            rb += TT;
         }
     }
     w.flush();
