@@ -30,6 +30,8 @@ sys.path.insert(0, ROOT)
 from paper_2510_18136_b200 import workloads as W  # noqa: E402
 
 CHUNK_DURATION_MS = 25 * W.TSAMP_S * 1e3  # 3355 ms (25 samples x 134 ms)
+# DRAM bytes (read + write) of one launch of the dominant kernel, from `ncu --set full` (profiles/r01_v3.md)
+NCU_TRAFFIC_BYTES = {"c2": 6.72e9}
 
 
 # ---------------------------------------------------------------------------- helpers
@@ -159,6 +161,10 @@ class StreamBench:
         # the whole ring is read once per push (mu/sigma span it) + the chunk is written into it
         return self.ring_bytes + self.chunk_bytes
 
+    def kernel_bytes(self):
+        # k_stream alone: the ring read once (per unit: 4 B per (channel, ring sample, pixel))
+        return self.ring_bytes
+
 
 class OfflineBench:
     def __init__(self, wl, plan_mod):
@@ -199,6 +205,9 @@ class OfflineBench:
         return self.wl.npix * 16 + 4
 
     def algorithmic_bytes(self):
+        return self.cube_bytes
+
+    def kernel_bytes(self):
         return self.cube_bytes
 
 
@@ -244,10 +253,21 @@ def run_cuda_arm(args, rank, world, local):
     ms_per_step = total_ms / args.steps
     launches = bench.plan.last_launches()
 
-    # per-kernel device time of the dominant kernel: time the search kernel alone through the same
-    # entry point is not possible from outside the library, so the roofline uses the whole step
-    # (all launches of the call) -- a lower bound on the kernel's own achieved rate.
     value = world * bench.cells_per_step / (ms_per_step * 1e-3) / 1e9
+
+    # device time of the dominant kernel (k_stream / k_search), measured live: the library records CUDA
+    # events on the launching stream around each kernel it enqueues (nsfrb_plan_set_profiling)
+    bench.plan.set_profiling(True)
+    kms = []
+    for _ in range(max(3, min(args.steps, 10))):
+        if flusher is not None:
+            flusher()
+        bench.step()
+        kms.append(bench.plan.kernel_ms())
+    bench.plan.set_profiling(False)
+    torch.cuda.synchronize()
+    kernel_ms = {k: float(np.mean([m[k] for m in kms])) for k in kms[0]}
+    dominant_ms = max_over_ranks(kernel_ms["search"], world)
 
     # end-to-end through the host-buffer entry points (pinned host memory, H2D + D2H inside)
     e2e = None
@@ -275,7 +295,11 @@ def run_cuda_arm(args, rank, world, local):
     if rank != 0:
         return
     alg_bytes = bench.algorithmic_bytes()
-    achieved = alg_bytes / (ms_per_step * 1e-3) / 1e9
+    kern_bytes = bench.kernel_bytes()
+    achieved = kern_bytes / (dominant_ms * 1e-3) / 1e9
+    dom_name = "k_stream" if wl.streaming else "k_search"
+    # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu capture (profiles/)
+    traffic = NCU_TRAFFIC_BYTES.get(wl.name)
     info = bench.info
     line = {
         "metric": "Gcells/s (pixel*DM*width*sample)", "value": value, "unit": "Gcells/s", "n_gpus": world,
@@ -289,8 +313,10 @@ def run_cuda_arm(args, rank, world, local):
         "e2e": e2e, "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
         "clocks": clocks,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                     "traffic": None, "peak_source": peak_src, "kernel": "k_search (timed: whole step, all launches)",
-                     "algorithmic_bytes": alg_bytes},
+                     "traffic": traffic, "peak_source": peak_src, "kernel": dom_name, "kernel_ms": dominant_ms,
+                     "share_of_step": dominant_ms / ms_per_step, "algorithmic_bytes": kern_bytes,
+                     "step_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / hbm_peak},
+        "kernel_ms": kernel_ms,
         "ms_per_step_p50": float(np.median(per_step)), "ms_per_step_max": float(np.max(per_step)),
         "wall_s": wall_s,
     }

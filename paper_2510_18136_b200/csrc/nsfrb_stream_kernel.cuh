@@ -8,7 +8,7 @@
 // ahead of time with the BASELINE config-2 prologue as a build check.
 //
 // Prologue (see nsfrb_jit.cu: make_stream_prologue):
-//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD DBUF   integers
+//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD   integers
 //   D_TAB[NU][NCHAN]   integer delays d[u][c] of the unique trials, DM ascending
 //   DMAX_TAB[NU]       dmax_u                 K_OF_U[NU]  lowest original dm index of the trial
 //   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index
@@ -188,13 +188,7 @@ template <int G> struct Worker {
         sfor<0, NCHAN>([&](auto c) {
             sfor<0, TT>([&](auto tt) {
                 constexpr int off = (V(c) - (T::span(V(c)) + V(tt) + T::emin(V(c))) * NCHAN) * 32;
-#if HACK == 2
-                buf[V(c) * TT + V(tt)] = __int_as_float(0x3f800000 + rb * 64 + off); // EXPERIMENT: no memory traffic
-#elif HACK == 1
-                buf[V(c) * TT + V(tt)] = ldrow(rp + off - (rb & 15) * (NCHAN * 32)); // EXPERIMENT: L1-resident rows
-#else
                 buf[V(c) * TT + V(tt)] = ldrow(b + off);
-#endif
             });
         });
     }
@@ -226,10 +220,6 @@ template <int G> struct Worker {
     // hot instruction footprint of an SM has to stay within the ~32 KB the instruction cache streams well)
     template <bool MASKED> __device__ __forceinline__ void tile(float (&cur)[NCHAN * TT], int rb, bool more, bool pf, bool cells)
     {
-#if DBUF
-        float nxt[NCHAN * TT];
-        if (more) load_new(nxt, rb + TT);
-#endif
         auto Wn = [&](auto c, auto m) -> float {
             if constexpr (V(m) < T::span(V(c))) return carry[T::coff(V(c)) + V(m)];
             else return cur[V(c) * TT + (V(m) - T::span(V(c)))];
@@ -265,9 +255,7 @@ template <int G> struct Worker {
             });
             sfor<0, T::CARRY>([&](auto i) { carry[V(i)] = nc[V(i)]; });
         }
-#if !DBUF
         if (more) load_new(cur, rb + TT); // rows of the next tile; their latency overlaps what follows
-#endif
         if (PFD > 0 && pf) prefetch_l2(rb + PFD * TT);
         // a1, a3, a4: centred sample, suffix sum (left in Dv), sum of squares
         sfor<0, KK>([&](auto kk) {
@@ -330,9 +318,6 @@ template <int G> struct Worker {
                 }
             }
         }
-#if DBUF
-        if (more) sfor<0, NCHAN * TT>([&](auto i) { cur[V(i)] = nxt[V(i)]; });
-#endif
     }
 };
 

@@ -315,3 +315,37 @@ def test_full_size_stream_c2_sampled():
                 PU.check_candidates(st["oracle"], pix, out.candidates(), out.n_found(), wl.threshold, 4096,
                                     all_pixels_checked=False)
                 assert out.n_found() == int((snr > wl.threshold).sum())
+
+
+def test_stream_unsorted_duplicate_dms_and_flat_pixels():
+    """Real-time path on an awkward plan: unsorted DM list with duplicates (5 unique trials: the last DM group
+    of k_stream is padded), unsorted widths incl. one longer than the ring, 35 pixels (neither a multiple of
+    32 nor of 4), a constant pixel (sigma = 0 => S = 0) and chunks larger than the first one (several passes)."""
+    from dataclasses import replace
+    dms = np.asarray([600.0, 0.0, 1400.0, 600.0, 200.0, 0.0, 1000.0], dtype=np.float64)
+    wl = replace(W.config("c1"), nx=7, ny=5, nt=120, dm_list=dms, streaming=True, threshold=4.0,
+                 width_list=np.asarray([3, 1, 400, 17, 2, 64], np.int32), name="stream-edge")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    nsfrb = _nsfrb()
+    g = torch.Generator(device="cuda").manual_seed(11)
+    so = oracle.StreamOracle(wl.nchan, wl.npix, wl.nt, d, wl.width_list)
+    with nsfrb.Plan.for_workload(wl, cand_capacity=64) as plan:
+        out = plan.alloc_outputs()
+        for i, c in enumerate([4, 9, 30, 1, 120, 17, 33, 5]):
+            chunk = torch.randn((wl.nchan, c, wl.npix), device="cuda", generator=g)
+            chunk[:, :, 3] = 2.5          # constant pixel: sigma = 0 for every trial
+            chunk[:, :, 20] *= 1e-3       # tiny scale: S/N is scale-free
+            plan.stream_push(chunk, out)
+            torch.cuda.synchronize()
+            ch = chunk.cpu().numpy()
+            n_prev = so.n
+            so.n += c
+            so.hist = np.concatenate([so.hist, ch], axis=1)[:, -so.L:, :]
+            lo = max(0, so.n - so.L)
+            snr = out.snr_map.cpu().numpy()
+            arg = out.argmax.cpu().numpy().T.copy()
+            st = PU.check(so.hist, d, wl.width_list, snr, arg, wl.threshold, raw_end_min=n_prev - lo, t_offset=lo,
+                          label=f"stream-edge push {i}", max_adjudicated_frac=0.5)
+            PU.check_candidates(st["oracle"], np.arange(wl.npix), out.candidates(), out.n_found(), wl.threshold, 64)
+            if so.n > int(d.max()) + 1:
+                assert snr[3] == 0.0

@@ -1,0 +1,57 @@
+"""CPU tests of the plan-time specialisation of the real-time kernel (no GPU: NVRTC only cross-compiles)."""
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+
+from paper_2510_18136_b200 import nsfrb, workloads as W
+
+
+def _args(wl):
+    return (wl.nx, wl.ny, wl.nchan, wl.nt, wl.freqs_GHz, wl.tsamp_s, wl.dm_list, wl.width_list)
+
+
+def test_generated_source_carries_the_plan():
+    wl = W.config("c2")
+    src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
+    assert "#define NPIX 65536" in src and "#define NCHAN 16" in src and "#define NU 16" in src and "#define CMAX 25" in src
+    # widths ascending, as the library was given them (tests/golden/width_lists.txt, n = 20)
+    assert "W_TAB[NW] = {1,2,3,4,5,6,9,14,20,29,42,61,88,128,186,270,392,569,826,1200}" in src
+    # delay rows of the table the plan computes (tests/golden/c2_dmax.txt pins their maxima)
+    assert "DMAX_TAB[NU] = {0,1,1,2,3,4,4,5,6,6,7,8,8,9,10,11}" in src
+    assert 'extern "C" __global__' in src and "k_stream" in src
+
+
+def test_duplicate_trials_and_unused_widths_are_dropped_from_the_kernel():
+    wl = W.config("c1")
+    dms = np.asarray([600.0, 0.0, 600.0, 3.0])          # DM 3 has the delay vector of DM 0
+    src = nsfrb.jit_stream_kernel(wl.nx, wl.ny, wl.nchan, 64, wl.freqs_GHz, wl.tsamp_s, dms, [5, 1, 400], 8).decode()
+    assert "#define NU 2" in src and "K_OF_U[NU] = {1,0}" in src      # unique trials, ascending delay
+    assert "W_TAB[NW] = {1,5}" in src and "J_OF_W[NW] = {1,0}" in src  # width 400 > ring: no cell, not compiled in
+
+
+def test_bad_variant_is_rejected():
+    wl = W.config("c1")
+    with pytest.raises(nsfrb.NsfrbError):
+        nsfrb.jit_stream_kernel(*_args(wl), 25, variant="zebra")
+
+
+def test_kernel_cross_compiles_to_sm100a():
+    wl = W.config("c1")
+    cubin = nsfrb.jit_stream_kernel(*_args(wl), 25, cubin=True)
+    assert cubin[:4] == b"\x7fELF"
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    path = os.path.join(os.environ.get("TMPDIR", "/tmp"), f"nsfrb_k_stream_{os.getpid()}.cubin")
+    with open(path, "wb") as f:
+        f.write(cubin)
+    try:
+        out = subprocess.run([cuobjdump, "-res-usage", path], capture_output=True, text=True).stdout
+        assert "Function k_stream" in out
+        elf = subprocess.run([cuobjdump, "-elf", path], capture_output=True, text=True).stdout
+        assert "sm_100a" in elf or "SM100a" in elf or "EF_CUDA_SM100" in elf, elf[:400]
+    finally:
+        os.remove(path)
