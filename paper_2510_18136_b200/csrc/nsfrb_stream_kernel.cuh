@@ -11,7 +11,7 @@
 //   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD   integers
 //   D_TAB[NU][NCHAN]   integer delays d[u][c] of the unique trials, DM ascending
 //   DMAX_TAB[NU]       dmax_u                 K_OF_U[NU]  lowest original dm index of the trial
-//   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index
+//   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index   RSQ_W[NW]  1/sqrt(width)
 //
 // Reverse frame.  The ring holds raw samples rho in [0, len); s = len-1-rho counts back from the
 // newest one.  Series u has T_u = len - dmax_u samples; its r-th sample from the end (r = 1..T_u) is
@@ -443,6 +443,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     const float delta = s1 * invT;
                     const float var = fmaxf(fmaf(-delta, delta, s2 * invT), 0.f);
                     const float sigma = sqrtf(var);
+                    const float rsig = sigma > 0.f ? 1.f / sigma : 0.f; // sigma = 0 => S = 0 (definition)
                     if (P.slice0 == 0 && live) P.mu0[(long long)u * NPIX + pix] = w.mu[V(kk)] + delta;
                     sfor<0, SEG>([&](auto q) {
                         const int j0 = rng[(gl * SEG + V(q)) * 2 + 0], j1 = rng[(gl * SEG + V(q)) * 2 + 1];
@@ -451,9 +452,8 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                                 const float m = w.mg[(V(kk) * NW + j) * 32];
                                 if (m > -kInf) {
                                     const int wj = W_TAB[j];
-                                    const float fw = (float)wj;
-                                    const float B = fmaf(-fw, delta, m + off[V(q)]);
-                                    const float S = sigma > 0.f ? B / (sigma * sqrtf(fw)) : 0.f;
+                                    const float B = fmaf(-(float)wj, delta, m + off[V(q)]);
+                                    const float S = (B * RSQ_W[j]) * rsig; // RSQ_W[j] = 1/sqrt(w_j), correctly rounded
                                     const int ii = P.i0 + w.ag[(V(kk) * NW + j) * 32];
                                     const int t = Tk - ii - wj;
                                     if (better(S, K_OF_U[u], J_OF_W[j], t, bs, bk, bj, bt)) { bs = S; bk = K_OF_U[u]; bj = J_OF_W[j]; bt = t; }
@@ -468,8 +468,13 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
         reinterpret_cast<int *>(red)[(gl * 32 + lane) * 4 + 2] = bj;
         reinterpret_cast<int *>(red)[(gl * 32 + lane) * 4 + 3] = bt;
     }
+    // only the (group 0, segment 0) warp consumes the reduction scratch: the others arrive and leave
+    if (!(seg == 0 && gl == 0)) {
+        asm volatile("bar.arrive 3, %0;" ::"r"(kThreads) : "memory");
+        return;
+    }
     bar_named(3, kThreads);
-    if (seg == 0 && gl == 0 && live) {
+    if (live) {
         sfor<1, GPC>([&](auto g2) {
             const float s = red[(V(g2) * 32 + lane) * 4 + 0];
             const int k = reinterpret_cast<int *>(red)[(V(g2) * 32 + lane) * 4 + 1];
