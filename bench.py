@@ -376,10 +376,19 @@ def run_reference_arm(args, rank, world):
     else:
         per_pixel_cells = oracle.cells_per_pixel(d, wl.width_list, wl.nt)
         est = per_pixel_cells * 1.2e-9 + wl.nchan * wl.nt * len(wl.dm_list) * 1e-9
-    n_pix = int(max(cores, min(wl.npix, 3.0 * cores / est)))  # ~3 s per step
-    g = torch.Generator().manual_seed(wl.seed)
-    data = torch.randn((wl.nchan, wl.nt, n_pix), generator=g).numpy()
     kw = dict(raw_end_min=wl.nt - wl.chunk_nt) if wl.streaming else {}
+    # bounded sample: calibrate on a few pixels, then size the per-step sample so that the whole
+    # --steps/--warmup run takes about two minutes
+    g = torch.Generator().manual_seed(wl.seed)
+    n0 = max(cores, 8)
+    probe = torch.randn((wl.nchan, wl.nt, n0), generator=g).numpy()
+    t0 = time.perf_counter()
+    oracle.search(probe, d, wl.width_list, nthreads=cores, **kw)
+    dt0 = max(time.perf_counter() - t0, 1e-4)
+    per_step_budget = 120.0 / max(args.steps + args.warmup, 1)
+    n_pix = int(max(cores, min(wl.npix, n0 * per_step_budget / dt0)))
+    del est
+    data = torch.randn((wl.nchan, wl.nt, n_pix), generator=g).numpy()
     times = []
     for i in range(args.warmup + args.steps):
         t0 = time.perf_counter()

@@ -111,6 +111,10 @@ int nsfrb_search(nsfrb_plan *plan, const float *cube, void *stream,
  *   arrived in this push are evaluated: n_prev <= t + w_j - 1 + dmax_k < n, t >= lo;
  *   reported t is the absolute sample index since the first push (mod 2^31).
  * 1 <= chunk_nt <= nt.  Outputs as nsfrb_search.
+ * The first push of a plan compiles the plan-specialised kernel with NVRTC (seconds to a minute, growing with
+ * ndm*nchan) and allocates the ring (2*(nt + guard)*nchan*npix*4 B); a compile failure returns NSFRB_ECUDA with
+ * the compiler log.  Compiled kernels are cached on disk (NSFRB_JIT_CACHE=<dir>, default /tmp/nsfrb_jit_cache;
+ * NSFRB_JIT_CACHE=0 disables).  Chunks longer than the plan's first chunk are searched in several passes.
  */
 int nsfrb_stream_push(nsfrb_plan *plan, const float *chunk, int chunk_nt, void *stream,
                       float *snr_map, int32_t *argmax,
