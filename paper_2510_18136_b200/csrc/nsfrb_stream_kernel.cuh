@@ -136,7 +136,8 @@ __device__ __forceinline__ float ldrow(const float *p) { return __ldg(p); }
 
 template <int G> struct Worker {
     using T = GT<G>;
-    const float *rp; // &ring[top_row][0][pixel]
+    const float *rp;  // &ring[block][top_row][0][lane]
+    const float *rp0; // the same for lane 0
     float *qe;       // &Qe[gl*KK][0][lane]
     float *mg;       // &mws[block][gl*KK][0][lane]
     int *ag;         // &aws[block][gl*KK][0][lane]
@@ -192,16 +193,13 @@ template <int G> struct Worker {
             });
         });
     }
-    // ask L2 for the rows of the tile PFD tiles ahead (no registers held; the later loads hit L2)
+    // ask L2 for the TT raw rows (all channels: TT*NCHAN*128 contiguous bytes in the blocked ring) that the tile
+    // PFD tiles ahead will need first -- one bulk prefetch, no registers held; the later loads hit L2
     __device__ __forceinline__ void prefetch_l2(int rb) const
     {
-        const float *b = rp - (long long)rb * (NCHAN * 32);
-        sfor<0, NCHAN>([&](auto c) {
-            sfor<0, TT>([&](auto tt) {
-                constexpr int off = (V(c) - (T::span(V(c)) + V(tt) + T::emin(V(c))) * NCHAN) * 32;
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(b + off));
-            });
-        });
+        constexpr int emax_all = []() { int m = 0; for (int c = 0; c < NCHAN; ++c) m = T::emax(c) > m ? T::emax(c) : m; return m; }();
+        const float *lo = rp0 - (long long)(rb + emax_all + TT - 1) * (NCHAN * 32); // oldest of the TT rows, channel 0, lane 0
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(lo), "r"(TT * NCHAN * 128) : "memory");
     }
     __device__ __forceinline__ void load_carry(int rb)
     {
@@ -346,7 +344,8 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
 
     Worker<G> w;
     w.i0 = P.i0; w.C = P.C; w.len = P.len;
-    w.rp = P.ring + ((long long)blockIdx.x * ROWS + P.top_row) * (NCHAN * 32) + lane;
+    w.rp0 = P.ring + ((long long)blockIdx.x * ROWS + P.top_row) * (NCHAN * 32);
+    w.rp = w.rp0 + lane;
     w.qe = Qe + (gl * KK) * CMAX * 32 + lane;
     {
         const long long blk = ((long long)blockIdx.x * NSUPER + blockIdx.y) * kTrialsPerCta + gl * KK;
@@ -370,7 +369,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     const int r_begin = seg == 0 ? -kLead : P.bound[seg], r_end = P.bound[seg + 1];
     const int r_fast_end = P.len - T::dmaxg(); // last group step (valid for every trial of the group)
     const int qe_end = P.i0 + P.C;             // group steps < qe_end may store Qe (they lie in segment 0)
-    const bool pf = gl == 0; // the DM groups of a pixel block read the same rows: one of them prefetches
+    const bool pf = gl == 0 && lane == 0; // the DM groups of a pixel block read the same rows: one thread prefetches
     bool synced = false;
     if (r_begin < r_end) {
         float cur[NCHAN * TT];
