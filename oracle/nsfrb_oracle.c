@@ -318,3 +318,22 @@ int64_t nsfrb_oracle_cells_per_pixel(int nchan, int nt, const int32_t *delays, i
     }
     return n;
 }
+
+/* NEXT 2: time binning of the image stack, PAPER.md:L77/L81 ("bins images to 0.67 s (x5) and 10.05 s
+ * (x75)" before re-searching with the same widths and, by footnote 12 L98, the same shift table at 5x the DM).
+ * Reading R24: out[c][u][p] = sum_{i<factor} in[c][u*factor + i][p] for u < floor(nt/factor); the
+ * trailing nt mod factor samples are dropped; a sum, not a mean (the S/N of O5 is scale-free).  float64 accumulate,
+ * result rounded once to float32 (the search takes a float32 cube). */
+int nsfrb_oracle_bin(const float *in, int nchan, int nt, int64_t npix, int factor, float *out)
+{
+    if (!in || !out || nchan < 1 || nt < 1 || npix < 1 || factor < 1) return -1;
+    const int nb = nt / factor;
+    for (int c = 0; c < nchan; ++c)
+        for (int u = 0; u < nb; ++u)
+            for (int64_t p = 0; p < npix; ++p) {
+                double s = 0.0;
+                for (int i = 0; i < factor; ++i) s += (double)in[((size_t)c * nt + (size_t)u * factor + i) * npix + p];
+                out[((size_t)c * nb + u) * npix + p] = (float)s;
+            }
+    return 0;
+}

@@ -51,6 +51,8 @@ def _load():
             f32p, ctypes.c_int64, ctypes.c_int, ctypes.c_int, i32p, ctypes.c_int, i32p, ctypes.c_int,
             ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int64,
         ]
+        lib.nsfrb_oracle_bin.restype = ctypes.c_int
+        lib.nsfrb_oracle_bin.argtypes = [f32p, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_int, f32p]
         lib.nsfrb_oracle_cells_per_pixel.restype = ctypes.c_int64
         lib.nsfrb_oracle_cells_per_pixel.argtypes = [ctypes.c_int, ctypes.c_int, i32p, ctypes.c_int, i32p, ctypes.c_int]
         _lib = lib
@@ -145,6 +147,18 @@ def cells_per_pixel(delay_table, widths, nt) -> int:
     w = np.ascontiguousarray(widths, dtype=np.int32)
     return int(_load().nsfrb_oracle_cells_per_pixel(d.shape[1], int(nt), _p(d, ctypes.c_int32), d.shape[0],
                                                     _p(w, ctypes.c_int32), w.size))
+
+
+def bin_time(cube, factor: int) -> np.ndarray:
+    """NEXT 2 / reading R24: sum of `factor` consecutive samples, floor(nt/factor) outputs."""
+    a = np.ascontiguousarray(cube, dtype=np.float32)
+    nchan, nt, npix = a.shape
+    out = np.empty((nchan, nt // int(factor), npix), dtype=np.float32)
+    if out.size:
+        rc = _load().nsfrb_oracle_bin(_p(a, ctypes.c_float), nchan, nt, npix, int(factor), _p(out, ctypes.c_float))
+        if rc != 0:
+            raise ValueError("nsfrb_oracle_bin: bad arguments")
+    return out
 
 
 class StreamOracle:

@@ -396,3 +396,42 @@ def test_multithreaded_oracle_is_identical():
     sel = np.asarray([5, 0, 36, 5])
     c = oracle.search(cube, d, w, pixels=sel, nthreads=3)
     assert np.array_equal(c.snr, a.snr[sel]) and np.array_equal(c.argmax, a.argmax[sel])
+
+
+# ----------------------------------------------------------------------------- NEXT 2: time binning (R24)
+def test_bin_time_pins():
+    """oracle.bin_time against what the definition fixes (reading R24): a constant cube bins to
+    factor x constant, factor 1 is the identity, trailing samples are dropped, it equals a reshape-sum (library
+    routine), it composes (x5 then x15 == x75, the paper's two binned timescales) and conserves the total."""
+    rng = np.random.default_rng(77)
+    a = rng.standard_normal((3, 157, 5)).astype(np.float32)
+    assert np.array_equal(oracle.bin_time(a, 1), a)
+    assert np.array_equal(oracle.bin_time(np.full((2, 10, 3), 1.5, np.float32), 5), np.full((2, 2, 3), 7.5, np.float32))
+    b5 = oracle.bin_time(a, 5)
+    assert b5.shape == (3, 31, 5)                      # floor(157/5); samples 155, 156 dropped
+    ref = a[:, :155, :].astype(np.float64).reshape(3, 31, 5, 5).sum(axis=2)
+    assert np.allclose(b5, ref, rtol=0, atol=1e-6)
+    assert np.array_equal(b5, ref.astype(np.float32))  # one rounding of the float64 sum
+    x = rng.integers(-8, 9, size=(2, 150, 4)).astype(np.float32)   # integers: every sum is exact in float32
+    assert np.array_equal(oracle.bin_time(oracle.bin_time(x, 5), 15), oracle.bin_time(x, 75))
+    assert oracle.bin_time(x, 75).sum() == x.sum()
+    assert oracle.bin_time(a, 200).shape == (3, 0, 5)  # factor > nt: nothing left
+
+
+def test_binned_search_reuses_the_delay_table():
+    """Footnote 12: searching the x5-binned cube at 5x the DMs uses the same integer shifts, so a
+    pulse injected at trial k of the fine grid with 5x the delays and 5x the width is recovered at the same (k, j)."""
+    f = np.linspace(1.311, 1.499, 8)
+    dms = np.linspace(0.0, 1400.0, 8)
+    d1 = oracle.delays(f, 0.1342, dms)
+    d5 = oracle.delays(f, 5 * 0.1342, 5 * dms)
+    assert np.array_equal(d1, d5)
+    nt, k, w, t0 = 1200, 5, 4, 100                    # in binned units; the cube is built at the fine sampling
+    cube = np.zeros((8, nt, 1), np.float32)
+    for c in range(8):
+        s = 5 * (t0 + d5[k][c])
+        cube[c, s:s + 5 * w, 0] = 1.0
+    r = oracle.search(oracle.bin_time(cube, 5), d5, [1, 2, 4, 8, 16])
+    assert tuple(r.argmax[0]) == (k, 2, t0)
+    Tk = nt // 5 - d5[k].max()
+    assert abs(r.snr[0] - np.sqrt(Tk - w)) < 1e-9      # noise-free closed form, as in the unbinned pin
