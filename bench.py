@@ -408,6 +408,30 @@ def run_reference_arm(args, rank, world):
         "gpu_launches": 0}))
 
 
+def run_bin_arm(args):
+    """--op bin: NEXT 2's binning kernel on the C3-shaped cube (x5, the paper's 0.67 s timescale): HBM-bound,
+    algorithmic bytes = cube read once + binned cube written once."""
+    from paper_2510_18136_b200 import nsfrb
+    torch.cuda.set_device(0)
+    hbm_peak, peak_src, _ = measured_peaks()
+    wl = W.config(args.workload if args.workload != "c2" else "c3")
+    factor = args.bin_factor
+    cube = torch.randn((wl.nchan, wl.nt, wl.npix), device="cuda", generator=torch.Generator(device="cuda").manual_seed(wl.seed))
+    out = torch.empty((wl.nchan, wl.nt // factor, wl.npix), device="cuda")
+    per_step = time_steps(lambda: nsfrb.bin_time(cube, factor, out), args.steps, args.warmup)
+    ms = float(np.mean(per_step))
+    nbytes = cube.numel() * 4 + out.numel() * 4
+    print(json.dumps({"metric": "GB/s (time binning, NEXT 2)", "value": nbytes / (ms * 1e-3) / 1e9, "unit": "GB/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+                      "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"{wl.name}-shaped cube binned x{factor}", "nchan": wl.nchan, "nt": wl.nt,
+                                 "npix": wl.npix, "l2": "inputs larger than L2"},
+                      "gpu_launches": args.steps,
+                      "roofline": {"bound": "hbm", "achieved": nbytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                                   "frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": None, "peak_source": peak_src,
+                                   "kernel": "k_bin", "algorithmic_bytes": nbytes}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -417,10 +441,15 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--op", default="search", choices=["search", "bin"], help="bin: time the binning kernel (NEXT 2)")
+    ap.add_argument("--bin-factor", type=int, default=5)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     rank, world, local = dist_setup(args.gpus)
-    if args.impl == "reference":
+    if args.op == "bin" and args.impl == "cuda":
+        if rank == 0:
+            run_bin_arm(args)
+    elif args.impl == "reference":
         run_reference_arm(args, rank, world)
     else:
         run_cuda_arm(args, rank, world, local)

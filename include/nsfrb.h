@@ -157,6 +157,16 @@ int nsfrb_plan_set_profiling(nsfrb_plan *plan, int on);
 int nsfrb_plan_get_kernel_ms(nsfrb_plan *plan, float out[4]);
 
 /*
+ * Time binning for the paper's longer timescales (images are binned x5 to 0.67 s and x75 to
+ * 10.05 s and searched again with the same widths; by footnote 12, L98, a plan created with 5*tsamp and 5*dm has
+ * the same shift table).  out[c][u][p] = sum_{i<factor} cube[c][u*factor+i][p] for u < nt/factor (integer
+ * division; trailing samples are dropped; a sum, not a mean -- the S/N is scale-free).
+ *   cube  device, [nchan][nt][npix] float32, read only;  out  device, [nchan][nt/factor][npix], must not alias cube
+ * Asynchronous on `stream`.  NSFRB_EINVAL for null pointers or non-positive sizes/factor.
+ */
+int nsfrb_bin_time(const float *cube, int nchan, int nt, int64_t npix, int factor, float *out, void *stream);
+
+/*
  * Harness access to the plan-specialised real-time kernel: for the plan the first ten
  * arguments describe (as nsfrb_plan_create) and a first chunk of chunk_nt samples, writes either the CUDA
  * source the library compiles at the first nsfrb_stream_push (want_cubin = 0) or its sm_100a cubin

@@ -511,6 +511,16 @@ int nsfrb_jit_stream_kernel(int nx, int ny, int nchan, int nt, const double *fre
     return NSFRB_OK;
 }
 
+int nsfrb_bin_time(const float *cube, int nchan, int nt, int64_t npix, int factor, float *out, void *stream)
+{
+    if (!cube || !out) return fail(NSFRB_EINVAL, "null pointer");
+    if (nchan < 1 || nt < 1 || npix < 1 || factor < 1) return fail(NSFRB_EINVAL, "non-positive size or factor");
+    if (nchan > 65535) return fail(NSFRB_EINVAL, "too many channels");
+    if (cube == out) return fail(NSFRB_EINVAL, "in-place binning is not supported");
+    CU(launch_bin(cube, out, nchan, nt, (long long)npix, factor, static_cast<cudaStream_t>(stream)), "k_bin launch");
+    return NSFRB_OK;
+}
+
 int nsfrb_plan_last_launches(const nsfrb_plan *pl) { return pl ? pl->last_launches : 0; }
 
 int nsfrb_plan_set_profiling(nsfrb_plan *pl, int on)

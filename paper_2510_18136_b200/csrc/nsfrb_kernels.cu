@@ -198,6 +198,42 @@ __global__ void __launch_bounds__(256) k_compact(const float *__restrict__ snr_m
 }
 
 // ------------------------------------------------------------------------------------------
+// NEXT 2: time binning out[c][u][p] = sum_{i<factor} in[c][u*factor+i][p]  (reading R24).
+// One thread owns one output vector (1 or 4 pixels) and walks `factor` input rows: coalesced, every input
+// byte read once -- HBM-bound by construction.
+// ------------------------------------------------------------------------------------------
+template <typename V>
+__global__ void __launch_bounds__(256) k_bin(const V *__restrict__ in, V *__restrict__ out, int nt, int nb, long long npv,
+                                             int factor)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npv) return;
+    const int c = blockIdx.z;
+    for (int u = blockIdx.y; u < nb; u += gridDim.y) {
+        const V *src = in + ((size_t)c * nt + (size_t)u * factor) * npv + p;
+        V acc = __ldcs(src);
+        for (int i = 1; i < factor; ++i) {
+            const V v = __ldcs(src + (size_t)i * npv);
+            if constexpr (sizeof(V) == 16) { acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w; }
+            else acc += v;
+        }
+        out[((size_t)c * nb + u) * npv + p] = acc;
+    }
+}
+
+cudaError_t launch_bin(const float *in, float *out, int nchan, int nt, long long npix, int factor, cudaStream_t st)
+{
+    const int nb = nt / factor;
+    if (nb < 1) return cudaSuccess;
+    const bool v4 = (npix % 4 == 0) && (((reinterpret_cast<uintptr_t>(in) | reinterpret_cast<uintptr_t>(out)) & 15u) == 0);
+    const long long npv = v4 ? npix / 4 : npix;
+    dim3 grid((unsigned)((npv + 255) / 256), (unsigned)(nb < 65535 ? nb : 65535), (unsigned)nchan);
+    if (v4) k_bin<float4><<<grid, 256, 0, st>>>(reinterpret_cast<const float4 *>(in), reinterpret_cast<float4 *>(out), nt, nb, npv, factor);
+    else k_bin<float><<<grid, 256, 0, st>>>(in, out, nt, nb, npv, factor);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
 // host-side launchers
 // ------------------------------------------------------------------------------------------
 size_t final_smem_bytes(int nt) { return ((size_t)nt + 2) * sizeof(float); }

@@ -44,7 +44,7 @@ assert CAND_DTYPE.itemsize == ctypes.sizeof(nsfrb_cand) == 20
 EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stream_reset", "nsfrb_search_host",
            "nsfrb_stream_push_host", "nsfrb_plan_destroy", "nsfrb_plan_get_delays", "nsfrb_plan_get_info",
            "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
-           "nsfrb_version", "nsfrb_jit_stream_kernel")
+           "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time")
 
 _lib = None
 
@@ -88,6 +88,8 @@ def lib() -> ctypes.CDLL:
         L.nsfrb_jit_stream_kernel.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, f64p, ctypes.c_double,
                                               f64p, ctypes.c_int, i32p, ctypes.c_int, ctypes.c_int, ctypes.c_char_p,
                                               ctypes.c_int, vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t)]
+        L.nsfrb_bin_time.restype = ctypes.c_int
+        L.nsfrb_bin_time.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_int, vp, vp]
         L.nsfrb_last_error.restype = ctypes.c_char_p
         L.nsfrb_version.restype = ctypes.c_char_p
         _lib = L
@@ -135,6 +137,20 @@ def jit_stream_kernel(nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, width_list
     buf = ctypes.create_string_buffer(need.value)
     _check(lib().nsfrb_jit_stream_kernel(*args, buf, need.value, ctypes.byref(need)))
     return buf.raw[: need.value]
+
+
+def bin_time(cube: torch.Tensor, factor: int, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+    """nsfrb_bin_time on a device cube [nchan][nt][npix] float32 -> [nchan][nt // factor][npix] (asynchronous)."""
+    if not cube.is_cuda or cube.dtype != torch.float32 or not cube.is_contiguous() or cube.dim() != 3:
+        raise ValueError("expected a contiguous float32 CUDA tensor [nchan][nt][npix]")
+    nchan, nt, npix = cube.shape
+    if out is None:
+        out = torch.empty((nchan, nt // int(factor) if factor >= 1 else 0, npix), dtype=torch.float32, device=cube.device)
+    if factor >= 1 and nt // int(factor) == 0:
+        return out  # nothing left to compute
+    s = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().nsfrb_bin_time(cube.data_ptr(), nchan, nt, npix, int(factor), out.data_ptr(), int(s.cuda_stream)))
+    return out
 
 
 class Plan:

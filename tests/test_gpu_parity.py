@@ -349,3 +349,49 @@ def test_stream_unsorted_duplicate_dms_and_flat_pixels():
             PU.check_candidates(st["oracle"], np.arange(wl.npix), out.candidates(), out.n_found(), wl.threshold, 64)
             if so.n > int(d.max()) + 1:
                 assert snr[3] == 0.0
+
+
+# ----------------------------------------------------------------------------- NEXT 2: binned timescales
+@pytest.mark.parametrize("npix", [37, 64])
+def test_bin_time_matches_oracle(npix):
+    nsfrb = _nsfrb()
+    g = torch.Generator(device="cuda").manual_seed(21)
+    ints = torch.randint(-8, 9, (3, 301, npix), device="cuda", generator=g).float()   # exact in float32
+    gauss = torch.randn((3, 301, npix), device="cuda", generator=g)
+    for factor in (1, 5, 7, 75, 301, 400):
+        got = nsfrb.bin_time(ints, factor)
+        torch.cuda.synchronize()
+        assert np.array_equal(got.cpu().numpy(), oracle.bin_time(ints.cpu().numpy(), factor)), factor
+        got = nsfrb.bin_time(gauss, factor).cpu().numpy()
+        ref = oracle.bin_time(gauss.cpu().numpy(), factor)
+        assert got.shape == ref.shape and np.all(np.abs(got - ref) <= 1e-6 * factor * 4), factor
+    with pytest.raises(nsfrb.NsfrbError):
+        nsfrb.bin_time(ints, 0)
+
+
+def test_three_timescale_search_paper_grid():
+    """The search as the paper runs it: 16 DM trials x log2 widths 1..16 at the native sampling,
+    again on the x5-binned stack with 5x the DMs (same shift table, fn. 12), and widths only (DM 0) on the x75-binned
+    stack -- each leg compared with the oracle on the oracle-binned cube."""
+    from dataclasses import replace
+    nsfrb = _nsfrb()
+    base = replace(W.config("c2").scaled(8, 6, nt=3000), streaming=False, width_list=np.asarray([1, 2, 4, 8, 16], np.int32),
+                   dm_list=np.linspace(171.0, 4000.0, 16), threshold=6.0, name="paper-grid")
+    g = torch.Generator(device="cuda").manual_seed(31)
+    cube = torch.randn((base.nchan, base.nt, base.npix), device="cuda", generator=g)
+    cube[:, 1500:1500 + 40, 7] += 0.6            # a 5.4 s pulse at DM 0: best seen at the 0.67 s timescale
+    cube[:, 600:600 + 900, 20] += 0.15           # a 2 min pulse (in a 40-bin x75 series it inflates its own sigma, L130)
+    d1 = oracle.delays(base.freqs_GHz, base.tsamp_s, base.dm_list)
+    best = {}
+    for factor, dms in ((1, base.dm_list), (5, 5 * base.dm_list), (75, np.asarray([0.0]))):
+        wl = replace(base, nt=base.nt // factor, tsamp_s=base.tsamp_s * factor, dm_list=dms, name=f"paper-grid x{factor}")
+        d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+        if factor == 5:
+            assert np.array_equal(d, d1)         # footnote 12: the same shift table
+        binned = nsfrb.bin_time(cube, factor) if factor > 1 else cube
+        ref_binned = oracle.bin_time(cube.cpu().numpy(), factor)
+        assert np.all(np.abs(binned.cpu().numpy() - ref_binned) <= 1e-5 * factor)
+        st, cs, snr, arg = _offline(wl, binned.contiguous(), label=wl.name)
+        best[factor] = snr
+    # the 40-sample pulse exceeds the 16-sample native boxcars: the x5 leg recovers more of it (L77)
+    assert best[5][7] > best[1][7]
