@@ -77,9 +77,10 @@ typedef struct {
  *   for nsfrb_stream_push.  freqs_GHz: host [nchan], finite, > 0, any order.  tsamp_s > 0.
  *   dm_list: host [ndm], finite, >= 0.  width_list: host [nwidth], each >= 1, distinct.
  *   Every trial must keep at least one sample: nt > max_c d[k][c] for all k.
- * All host arrays are copied.  The plan allocates nchan*nt*npix*4 B of device workspace
- * (the time-contiguous copy of the cube, which doubles as the streaming ring) plus small
- * tables, on the current CUDA device.
+ * All host arrays are copied.  Device memory is allocated on the current CUDA device when first needed: small
+ * tables at creation; nchan*nt*npix*4 B (the time-contiguous copy of the cube) at the first nsfrb_search; the
+ * ring, 2*(nt + guard)*nchan*npix*4 B, plus a workspace of ~10 B per (pixel, trial, width) at the first
+ * nsfrb_stream_push.
  */
 int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt,
                       const double *freqs_GHz, double tsamp_s,

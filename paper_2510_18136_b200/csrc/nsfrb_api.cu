@@ -481,7 +481,7 @@ int nsfrb_plan_get_info(const nsfrb_plan *pl, nsfrb_plan_info *info)
     info->ndm_unique = pl->nuniq; info->dmax = pl->dmax_all; info->wmax = pl->wmax_used;
     info->n_groups = pl->n_groups; info->n_width_batches = pl->n_wb; info->series_per_cta = kSearchWarps;
     info->block_len = kBlockLen; info->ring_len = pl->H; info->search_threads = kSearchWarps * 32;
-    info->search_smem_bytes = (int64_t)pl->smem_search; info->workspace_bytes = (int64_t)pl->workspace_bytes;
+    info->search_smem_bytes = (int64_t)pl->smem_search; info->workspace_bytes = (int64_t)(pl->workspace_bytes + stream_bytes(pl));
     info->cells_per_pixel = pl->cells_per_pixel; info->shift_adds_per_pixel = pl->shift_adds_per_pixel;
     return NSFRB_OK;
 }

@@ -127,6 +127,7 @@ void free_plan(nsfrb_plan *p);
 // ---- real-time path (nsfrb_stream.cu)
 void stream_free(nsfrb_plan *p);
 void stream_reset(nsfrb_plan *p);
+size_t stream_bytes(const nsfrb_plan *p); // device bytes the real-time path holds (0 before the first push)
 // a8 + k_stream passes + reduction over slices; outputs as nsfrb_stream_push.  Returns an NSFRB_* code and
 // leaves the message in `err`.
 int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t st, float *snr_map, int32_t *argmax,
