@@ -301,6 +301,26 @@ def run_cuda_arm(args, rank, world, local):
     # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu capture (profiles/)
     traffic = NCU_TRAFFIC_BYTES.get(wl.name)
     info = bench.info
+    roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+            "traffic": traffic, "peak_source": peak_src, "kernel": dom_name, "kernel_ms": dominant_ms,
+            "share_of_step": dominant_ms / ms_per_step, "algorithmic_bytes": kern_bytes,
+            "step_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / hbm_peak}
+    if not wl.streaming:
+        # BASELINE.json's roofline: the slower of (cube bytes once / HBM) and (shift-adds + prefix adds) / FP32 issue
+        # rate.  FP32 issue peak = 148 SMs x 128 lanes x SM clock (measured 123-134 lane-ops/clk/SM).
+        sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+        alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e12  # T lane-ops/s
+        prefix_adds = sum(wl.nt - int(x) for x in bench.delays.max(axis=1))
+        alu_ops = (info["shift_adds_per_pixel"] + prefix_adds) * wl.npix
+        t_hbm, t_alu = kern_bytes / (hbm_peak * 1e9), alu_ops / (alu_peak * 1e12)
+        if t_alu > t_hbm:
+            ach = alu_ops / (dominant_ms * 1e-3) / 1e12
+            roof.update({"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "T lane-ops/s", "frac": ach / alu_peak,
+                         "peak_source": "148 SMs x 128 FP32 lanes x sm_max_mhz (DESIGN.md sec. 7)",
+                         "algorithmic_ops": alu_ops, "contract_roofline_ms": t_alu * 1e3,
+                         "step_frac": alu_ops / (ms_per_step * 1e-3) / 1e12 / alu_peak})
+        else:
+            roof["contract_roofline_ms"] = t_hbm * 1e3
     line = {
         "metric": "Gcells/s (pixel*DM*width*sample)", "value": value, "unit": "Gcells/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -312,10 +332,7 @@ def run_cuda_arm(args, rank, world, local):
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "e2e": e2e, "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                     "traffic": traffic, "peak_source": peak_src, "kernel": dom_name, "kernel_ms": dominant_ms,
-                     "share_of_step": dominant_ms / ms_per_step, "algorithmic_bytes": kern_bytes,
-                     "step_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / hbm_peak},
+        "roofline": roof,
         "kernel_ms": kernel_ms,
         "ms_per_step_p50": float(np.median(per_step)), "ms_per_step_max": float(np.max(per_step)),
         "wall_s": wall_s,

@@ -340,8 +340,6 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const
     *out = nullptr;
     // ---- device state
     cudaError_t e = cudaGetDevice(&pl->device);
-    if (e == cudaSuccess) e = configure_kernels(pl->smem_final);
-    if (e == cudaSuccess) e = configure_search(pl->smem_search);
     size_t acc = 0;
     if (e == cudaSuccess) e = upload(&pl->d_delays_u, pl->delays_u, &acc);
     if (e == cudaSuccess) e = upload(&pl->d_dd_tab, pl->dd_tab, &acc);

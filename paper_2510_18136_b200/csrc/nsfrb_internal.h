@@ -145,8 +145,6 @@ cudaError_t launch_finalize(const FinalParams &p, size_t smem_bytes, cudaStream_
 cudaError_t launch_compact(const float *snr_map, const int32_t *argmax, int npix, float threshold,
                            nsfrb_cand *cands, uint32_t cap, uint32_t *ncands, cudaStream_t st);
 cudaError_t launch_bin(const float *in, float *out, int nchan, int nt, long long npix, int factor, cudaStream_t st);
-cudaError_t configure_kernels(size_t final_smem);
-cudaError_t configure_search(size_t search_smem);
 size_t search_smem_bytes(int nchan, int RS, int H, int tab_cap);
 size_t final_smem_bytes(int nt);
 

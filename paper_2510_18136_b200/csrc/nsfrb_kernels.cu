@@ -238,11 +238,6 @@ cudaError_t launch_bin(const float *in, float *out, int nchan, int nt, long long
 // ------------------------------------------------------------------------------------------
 size_t final_smem_bytes(int nt) { return ((size_t)nt + 2) * sizeof(float); }
 
-cudaError_t configure_kernels(size_t final_smem)
-{
-    return cudaFuncSetAttribute(k_finalize, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)final_smem);
-}
-
 cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, int nt, int pitch, cudaStream_t st)
 {
     dim3 grid((npix + 31) / 32, (nt + 31) / 32, nchan), block(32, 8);
@@ -252,6 +247,15 @@ cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, i
 
 cudaError_t launch_finalize(const FinalParams &p, size_t smem_bytes, cudaStream_t st)
 {
+    static size_t granted[64] = {0}; // per-device function attribute shared by all plans: only ever raise it
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64 && smem_bytes > granted[dev]) {
+        e = cudaFuncSetAttribute(k_finalize, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+        if (e != cudaSuccess) return e;
+        granted[dev] = smem_bytes;
+    }
     k_finalize<<<p.npix, 256, smem_bytes, st>>>(p);
     return cudaGetLastError();
 }

@@ -441,15 +441,20 @@ size_t search_smem_bytes(int nchan, int RS, int H, int tab_cap)
     return n * sizeof(float) + 16;
 }
 
-cudaError_t configure_search(size_t search_smem)
-{
-    return cudaFuncSetAttribute(k_search, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)search_smem);
-}
-
 cudaError_t launch_search(const SearchParams &p, size_t smem_bytes, cudaStream_t st)
 {
     const long long blocks = (long long)p.npix * p.n_groups * p.n_wb;
     if (blocks <= 0 || blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    // the opt-in shared-memory size is a per-device function attribute: several plans share it, so only ever raise it
+    static size_t granted[64] = {0};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev >= 0 && dev < 64 && smem_bytes > granted[dev]) {
+        e = cudaFuncSetAttribute(k_search, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+        if (e != cudaSuccess) return e;
+        granted[dev] = smem_bytes;
+    }
     k_search<<<(unsigned)blocks, NW * 32, smem_bytes, st>>>(p);
     return cudaGetLastError();
 }

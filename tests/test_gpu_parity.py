@@ -395,3 +395,18 @@ def test_three_timescale_search_paper_grid():
         best[factor] = snr
     # the 40-sample pulse exceeds the 16-sample native boxcars: the x5 leg recovers more of it (L77)
     assert best[5][7] > best[1][7]
+
+
+def test_two_plans_with_different_shared_memory_needs_coexist():
+    """The opt-in shared-memory size is a per-function attribute: creating a second, smaller plan must not break
+    launches of the first (regression: 'k_search launch: invalid argument')."""
+    nsfrb = _nsfrb()
+    big = W.config("c3").scaled(6, 4, nt=600, n_pulses=0)
+    small = W.config("c1")
+    cube = W.make_cube(big, "cuda")
+    with nsfrb.Plan.for_workload(big) as p1:
+        with nsfrb.Plan(small.nx, small.ny, small.nchan, small.nt, small.freqs_GHz, small.tsamp_s, [500.0], [1], 6.0) as p2:
+            p2.search(W.make_cube(small, "cuda"))
+        r = p1.search(cube)
+        torch.cuda.synchronize()
+        assert np.isfinite(r.snr_map.cpu().numpy()).all()
