@@ -180,6 +180,12 @@ int nsfrb_jit_stream_kernel(int nx, int ny, int nchan, int nt, const double *fre
                             int chunk_nt, const char *variant, int want_cubin,
                             char *out, size_t capacity, size_t *needed);
 
+/* The same for the plan-specialised offline kernel k_search3 (compiled at the first nsfrb_search of a plan with at
+ * most 32 usable widths; NSFRB_SEARCH_JIT=0 selects the generic k_search instead). */
+int nsfrb_jit_search_kernel(int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
+                            const double *dm_list, int ndm, const int32_t *width_list, int nwidth,
+                            int want_cubin, char *out, size_t capacity, size_t *needed);
+
 /* Thread-local text of the last error; never NULL. */
 const char *nsfrb_last_error(void);
 

@@ -14,9 +14,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnsfrb.so")
 SOURCES = ["nsfrb_api.cu", "nsfrb_kernels.cu", "nsfrb_search.cu", "nsfrb_stream.cu"]
-JIT_SRC = os.path.join(CSRC, "nsfrb_stream_kernel.cuh")   # compiled at plan time (NVRTC); embedded as text
-JIT_INC = os.path.join(CSRC, "nsfrb_stream_kernel_src.inc")
-HEADERS = [JIT_SRC, os.path.join(CSRC, "nsfrb_internal.h"), os.path.join(os.path.dirname(HERE), "include", "nsfrb.h")]
+JIT_SRCS = [os.path.join(CSRC, "nsfrb_stream_kernel.cuh"),   # compiled at plan time (NVRTC); embedded as text
+            os.path.join(CSRC, "nsfrb_search_kernel.cuh")]
+HEADERS = JIT_SRCS + [os.path.join(CSRC, "nsfrb_internal.h"), os.path.join(os.path.dirname(HERE), "include", "nsfrb.h")]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC,-fvisibility=hidden", "-shared", "-cudart", "static",
@@ -41,11 +41,12 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
-        with open(JIT_SRC) as f:
-            text = f.read()
-        assert ')NSFRBSRC"' not in text
-        with open(JIT_INC, "w") as f:   # the kernel source as one raw string literal
-            f.write('R"NSFRBSRC(\n' + text + ')NSFRBSRC"\n')
+        for src_path in JIT_SRCS:   # each kernel source as one raw string literal
+            with open(src_path) as f:
+                text = f.read()
+            assert ')NSFRBSRC"' not in text
+            with open(src_path[:-len(".cuh")] + "_src.inc", "w") as f:
+                f.write('R"NSFRBSRC(\n' + text + ')NSFRBSRC"\n')
         tmp = LIB + f".tmp{os.getpid()}"
         cmd = [_nvcc(), *NVCC_FLAGS] + (["-Xptxas", "-v"] if verbose else []) + \
               ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]

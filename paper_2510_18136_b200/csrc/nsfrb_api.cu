@@ -50,6 +50,7 @@ void nsfrb::free_plan(nsfrb_plan *p)
     cudaFree(p->d_arg); cudaFree(p->d_cands); cudaFree(p->d_ncands);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     stream_free(p);
+    search3_free(p);
     cudaGetLastError();
     delete p;
 }
@@ -132,7 +133,12 @@ int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offse
         sp.origin = origin; sp.len = len; sp.raw_end_min = raw_end_min;
         sp.nuniq = pl->nuniq; sp.nw = pl->nw_used; sp.n_groups = pl->n_groups; sp.n_wb = pl->n_wb;
         sp.H = pl->H; sp.RS = pl->RS; sp.wmax = pl->wmax_used; sp.tab_cap = pl->tab_cap;
-        CU(launch_search(sp, pl->smem_search, st), "k_search launch");
+        if (search3_usable(pl)) { // plan-specialised kernel (same algorithm, compiled per plan)
+            std::string err;
+            if (int rc = search3_launch(pl, st, err)) return fail(rc, err);
+        } else {
+            CU(launch_search(sp, pl->smem_search, st), "k_search launch");
+        }
         ++*launches;
     }
     mark(pl, 2, st);
@@ -493,6 +499,31 @@ int nsfrb_jit_stream_kernel(int nx, int ny, int nchan, int nt, const double *fre
     if (int rc = plan_host_init(&pl, nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, ndm, width_list, nwidth, 0.f)) return rc;
     std::string src, err;
     int rc = stream_source(pl, chunk_nt, variant, src, err);
+    free_plan(pl);
+    if (rc) return fail(rc, err);
+    std::vector<char> bin;
+    const char *data = src.data();
+    size_t n = src.size();
+    if (want_cubin) {
+        std::string log;
+        if ((rc = stream_compile(src, bin, log))) return fail(rc, log);
+        data = bin.data();
+        n = bin.size();
+    }
+    *needed = n;
+    if (out && capacity >= n) std::memcpy(out, data, n);
+    return NSFRB_OK;
+}
+
+int nsfrb_jit_search_kernel(int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s, const double *dm_list,
+                            int ndm, const int32_t *width_list, int nwidth, int want_cubin, char *out, size_t capacity,
+                            size_t *needed)
+{
+    if (!needed) return fail(NSFRB_EINVAL, "needed is null");
+    nsfrb_plan *pl = nullptr;
+    if (int rc = plan_host_init(&pl, nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, ndm, width_list, nwidth, 0.f)) return rc;
+    std::string src, err;
+    int rc = search3_source(pl, src, err);
     free_plan(pl);
     if (rc) return fail(rc, err);
     std::vector<char> bin;

@@ -55,6 +55,7 @@ struct SearchParams {
 };
 
 struct StreamState;
+struct Search3State;
 
 struct FinalParams {
     const float *W;
@@ -116,6 +117,8 @@ struct nsfrb_plan {
     bool ev_valid = false;
     // real-time path (nsfrb_stream.cu): ring, provisional means, plan-specialised kernel
     nsfrb::StreamState *stream = nullptr;
+    // offline path: plan-specialised k_search3 (nsfrb_search_kernel.cuh), compiled at the first nsfrb_search
+    nsfrb::Search3State *search3 = nullptr;
 };
 
 namespace nsfrb {
@@ -123,6 +126,13 @@ namespace nsfrb {
 int plan_host_init(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
                    const double *dm_list, int ndm, const int32_t *width_list, int nwidth, float threshold);
 void free_plan(nsfrb_plan *p);
+
+// ---- plan-specialised offline kernel (nsfrb_stream.cu holds the NVRTC plumbing for both kernels)
+// True if the plan can use k_search3 (at most 32 usable widths; NSFRB_SEARCH_JIT=0 forces the generic k_search).
+bool search3_usable(const nsfrb_plan *pl);
+int search3_source(const nsfrb_plan *pl, std::string &src, std::string &err);
+int search3_launch(nsfrb_plan *pl, cudaStream_t st, std::string &err); // compiles on first use; fills pl->d_partials
+void search3_free(nsfrb_plan *p);
 
 // ---- real-time path (nsfrb_stream.cu)
 void stream_free(nsfrb_plan *p);

@@ -44,7 +44,7 @@ assert CAND_DTYPE.itemsize == ctypes.sizeof(nsfrb_cand) == 20
 EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stream_reset", "nsfrb_search_host",
            "nsfrb_stream_push_host", "nsfrb_plan_destroy", "nsfrb_plan_get_delays", "nsfrb_plan_get_info",
            "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
-           "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time")
+           "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel")
 
 _lib = None
 
@@ -88,6 +88,10 @@ def lib() -> ctypes.CDLL:
         L.nsfrb_jit_stream_kernel.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, f64p, ctypes.c_double,
                                               f64p, ctypes.c_int, i32p, ctypes.c_int, ctypes.c_int, ctypes.c_char_p,
                                               ctypes.c_int, vp, ctypes.c_size_t, ctypes.POINTER(ctypes.c_size_t)]
+        L.nsfrb_jit_search_kernel.restype = ctypes.c_int
+        L.nsfrb_jit_search_kernel.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, f64p, ctypes.c_double,
+                                              f64p, ctypes.c_int, i32p, ctypes.c_int, ctypes.c_int, vp, ctypes.c_size_t,
+                                              ctypes.POINTER(ctypes.c_size_t)]
         L.nsfrb_bin_time.restype = ctypes.c_int
         L.nsfrb_bin_time.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_int, vp, vp]
         L.nsfrb_last_error.restype = ctypes.c_char_p
@@ -136,6 +140,21 @@ def jit_stream_kernel(nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, width_list
     _check(lib().nsfrb_jit_stream_kernel(*args, None, 0, ctypes.byref(need)))
     buf = ctypes.create_string_buffer(need.value)
     _check(lib().nsfrb_jit_stream_kernel(*args, buf, need.value, ctypes.byref(need)))
+    return buf.raw[: need.value]
+
+
+def jit_search_kernel(nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, width_list, cubin=False) -> bytes:
+    """nsfrb_jit_search_kernel: CUDA source (or sm_100a cubin) of the plan-specialised offline kernel.  Needs no GPU."""
+    f = np.ascontiguousarray(freqs_GHz, dtype=np.float64)
+    dm = np.ascontiguousarray(dm_list, dtype=np.float64)
+    w = np.ascontiguousarray(width_list, dtype=np.int32)
+    f64p, i32p = ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)
+    args = (int(nx), int(ny), int(nchan), int(nt), f.ctypes.data_as(f64p), float(tsamp_s), dm.ctypes.data_as(f64p), dm.size,
+            w.ctypes.data_as(i32p), w.size, int(bool(cubin)))
+    need = ctypes.c_size_t(0)
+    _check(lib().nsfrb_jit_search_kernel(*args, None, 0, ctypes.byref(need)))
+    buf = ctypes.create_string_buffer(need.value)
+    _check(lib().nsfrb_jit_search_kernel(*args, buf, need.value, ctypes.byref(need)))
     return buf.raw[: need.value]
 
 
