@@ -410,3 +410,20 @@ def test_two_plans_with_different_shared_memory_needs_coexist():
         r = p1.search(cube)
         torch.cuda.synchronize()
         assert np.isfinite(r.snr_map.cpu().numpy()).all()
+
+
+def test_more_than_32_widths_use_the_generic_kernel():
+    """Plans with more than 32 usable widths run the generic k_search (two width batches); everything else runs
+    the plan-specialised k_search3 -- both against the oracle, and against each other on the same cube."""
+    from dataclasses import replace
+    nsfrb = _nsfrb()
+    wl40 = replace(W.config("c1"), nx=6, ny=5, nt=700, width_list=np.arange(1, 41, dtype=np.int32) * 3 - 2, name="w40")
+    d = oracle.delays(wl40.freqs_GHz, wl40.tsamp_s, wl40.dm_list)
+    g = torch.Generator(device="cuda").manual_seed(41)
+    cube = torch.randn((wl40.nchan, wl40.nt, wl40.npix), device="cuda", generator=g)
+    st, cs, snr40, arg40 = _offline(wl40, cube, label="w40 generic")
+    # the first 32 of those widths through k_search3, then the maxima restricted to them must agree where they win
+    wl32 = replace(wl40, width_list=wl40.width_list[:32], name="w32")
+    st, cs, snr32, arg32 = _offline(wl32, cube, label="w32 specialised")
+    same = arg40[:, 1] < 32
+    assert same.any() and np.all(np.abs(snr40[same] - snr32[same]) <= PU.tol(snr40[same]))
