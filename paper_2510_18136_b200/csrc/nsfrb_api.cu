@@ -124,7 +124,7 @@ void build_dd_tables(nsfrb_plan *pl)
 int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offset, cudaStream_t st, float *snr_map,
                int32_t *argmax, nsfrb_cand *cands, uint32_t cap, uint32_t *ncands, int *launches)
 {
-    const int slices = (pl->nw_used > 0) ? pl->n_groups * pl->n_wb : 0;
+    int slices = (pl->nw_used > 0) ? pl->n_groups * pl->n_wb : 0;
     if (slices > 0) {
         SearchParams sp;
         sp.W = pl->d_W; sp.delays_u = pl->d_delays_u; sp.dmax_u = pl->d_dmax_u; sp.k_of_u = pl->d_k_of_u;
@@ -136,6 +136,7 @@ int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offse
         if (search3_usable(pl)) { // plan-specialised kernel (same algorithm, compiled per plan)
             std::string err;
             if (int rc = search3_launch(pl, st, err)) return fail(rc, err);
+            slices = search3_slices(pl);
         } else {
             CU(launch_search(sp, pl->smem_search, st), "k_search launch");
         }
@@ -355,7 +356,7 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const
     if (e == cudaSuccess) e = upload(&pl->d_widths, pl->widths_used, &acc);
     if (e == cudaSuccess) e = upload(&pl->d_j_of_used, pl->j_of_used, &acc);
     if (e == cudaSuccess) {
-        const size_t pb = (size_t)pl->npix * pl->n_groups * pl->n_wb * sizeof(Partial);
+        const size_t pb = (size_t)pl->npix * std::max(pl->n_groups * pl->n_wb, (pl->nuniq + 7) / 8) * sizeof(Partial);
         e = cudaMalloc(reinterpret_cast<void **>(&pl->d_partials), pb);
         acc += pb;
     }

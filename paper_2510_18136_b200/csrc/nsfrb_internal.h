@@ -133,6 +133,7 @@ bool search3_usable(const nsfrb_plan *pl);
 int search3_source(const nsfrb_plan *pl, std::string &src, std::string &err);
 int search3_launch(nsfrb_plan *pl, cudaStream_t st, std::string &err); // compiles on first use; fills pl->d_partials
 void search3_free(nsfrb_plan *p);
+int search3_slices(const nsfrb_plan *pl); // partial records per pixel written by the last search3_launch
 
 // ---- real-time path (nsfrb_stream.cu)
 void stream_free(nsfrb_plan *p);

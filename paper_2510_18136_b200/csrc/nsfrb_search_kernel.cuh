@@ -1,12 +1,13 @@
 // k_search3: the offline search kernel (steps a1..a6 of DESIGN.md), specialised per plan.
 //
 // Compiled at the first nsfrb_search of a plan (NVRTC, sm_100a) behind a generated prologue, like k_stream:
-//   NCHAN NU NW RS H PITCH NT WMID          integers (RS raw-tile row stride, H prefix ring length, PITCH workspace row)
+//   NCHAN NU NW RS H PITCH NT WMID TRIALS MINB   integers (RS raw-tile row stride, H prefix ring length, PITCH workspace row)
 //   D_TAB[NU][NCHAN]  delays of the unique trials (dmax ascending)   DMAX_TAB[NU]   K_OF_U[NU]
 //   W_TAB[NW]         the usable widths, caller's order (NW <= 32)    J_OF_W[NW]     original width index
 // Same algorithm as the generic k_search (nsfrb_search.cu: one CTA = one pixel x 16 trials, 256-sample blocks,
 // cp.async raw prefetch, differential dedispersion, warp = trial, prefix ring in shared memory, exact bound-based
 // pruning of wide boxcars), with what the plan fixes folded into the instruction stream:
+// One CTA = one pixel x TRIALS trials (a prologue constant: 8 trials = 256 threads lets 2-3 CTAs share an SM).
 //   phase 1  every dedispersion operand is rt[immediate]; no change lists in shared memory, no address arithmetic
 //   phase 2  the set of widths is static: widths <= 16 from the register window without per-width tests, widths
 //            17..WMID from the ring with aligned 128-bit loads (their block bound never prunes: DESIGN.md 5.1),
@@ -31,7 +32,7 @@ namespace s3 {
 
 #define S3_INF __int_as_float(0x7f800000)
 constexpr unsigned kFull = 0xffffffffu;
-constexpr int NWARP = 16;  // trials per CTA
+constexpr int NWARP = TRIALS; // trials (= warps) per CTA: 8 or 16
 constexpr int LB = 256;    // samples per block
 constexpr int SS = 288;    // staging stride per trial: t + 4*(t>>5)
 constexpr int NR = H / 32; // ring rows
@@ -349,8 +350,12 @@ template <int G> __device__ __forceinline__ void run_group(const Search3Params &
             const int tl = tid & (LB - 1);
             const float *rt = raw + tl;
             float *so = stage + tl + 4 * (tl >> 5);
-            if (tid < LB) dedisperse8<G, 0>(rt, so);
-            else dedisperse8<G, 1>(rt, so + 8 * SS);
+            if constexpr (NWARP == 8) {
+                dedisperse8<G, 0>(rt, so);
+            } else {
+                if (tid < LB) dedisperse8<G, 0>(rt, so);
+                else dedisperse8<G, 1>(rt, so + 8 * SS);
+            }
         }
         __syncthreads(); // stage(b) complete; the raw tile is free again
         if (t0 + LB < T_g) issue_raw(Wp, raw, t0 + LB, rows4, warp, lane);
@@ -437,7 +442,7 @@ template <int G0, int N> __device__ __forceinline__ void dispatch(int g, const S
 
 } // namespace s3
 
-extern "C" __global__ void __launch_bounds__(512, 1) k_search3(const Search3Params P)
+extern "C" __global__ void __launch_bounds__(s3::NWARP * 32, MINB) k_search3(const Search3Params P)
 {
     extern __shared__ __align__(16) float smem[];
     const int p = blockIdx.x / s3::NGRP;
