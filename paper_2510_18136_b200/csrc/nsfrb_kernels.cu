@@ -39,22 +39,36 @@ __device__ __forceinline__ bool better(float s, int k, int j, float bs, int bk, 
 __global__ void __launch_bounds__(256) k_transpose(const float *__restrict__ cube, float *__restrict__ W,
                                                    int npix, int nchan, int nt, int pitch)
 {
-    __shared__ float tile[32][33];
+    // 64 pixels x 64 samples per CTA: 256-byte runs on both the read (pixel-contiguous) and the write
+    // (time-contiguous) side; 65-float rows keep both shared-memory phases conflict-free or 2-way
+    __shared__ float tile[64][65];
     const int c = blockIdx.z;
-    const int p0 = blockIdx.x * 32, t0 = blockIdx.y * 32;
+    const int p0 = blockIdx.x * 64, t0 = blockIdx.y * 64;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const size_t chan0 = (size_t)c * nt * (size_t)npix;
     {
-        const int p = p0 + threadIdx.x;
-        const float b = (p < npix) ? __ldg(cube + chan0 + p) : 0.f;
-        for (int r = threadIdx.y; r < 32; r += 8) {
+        const int pa = p0 + lane, pb = p0 + 32 + lane;
+        const float ba = (pa < npix) ? __ldg(cube + chan0 + pa) : 0.f;
+        const float bb = (pb < npix) ? __ldg(cube + chan0 + pb) : 0.f;
+#pragma unroll 4
+        for (int r = warp; r < 64; r += 8) {
             const int t = t0 + r;
-            if (t < nt && p < npix) tile[r][threadIdx.x] = __ldg(cube + chan0 + (size_t)t * npix + p) - b;
+            if (t < nt) {
+                const float *row = cube + chan0 + (size_t)t * npix;
+                if (pa < npix) tile[r][lane] = __ldcs(row + pa) - ba;
+                if (pb < npix) tile[r][32 + lane] = __ldcs(row + pb) - bb;
+            }
         }
     }
     __syncthreads();
-    for (int r = threadIdx.y; r < 32; r += 8) {
-        const int p = p0 + r, t = t0 + threadIdx.x;
-        if (t < nt && p < npix) W[((size_t)p * nchan + c) * (size_t)pitch + t] = tile[threadIdx.x][r];
+#pragma unroll 4
+    for (int r = warp; r < 64; r += 8) {
+        const int p = p0 + r;
+        if (p < npix) {
+            float *dst = W + ((size_t)p * nchan + c) * (size_t)pitch + t0;
+            if (t0 + lane < nt) dst[lane] = tile[lane][r];
+            if (t0 + 32 + lane < nt) dst[32 + lane] = tile[32 + lane][r];
+        }
     }
 }
 
@@ -240,7 +254,7 @@ size_t final_smem_bytes(int nt) { return ((size_t)nt + 2) * sizeof(float); }
 
 cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, int nt, int pitch, cudaStream_t st)
 {
-    dim3 grid((npix + 31) / 32, (nt + 31) / 32, nchan), block(32, 8);
+    dim3 grid((npix + 63) / 64, (nt + 63) / 64, nchan), block(256);
     k_transpose<<<grid, block, 0, st>>>(cube, W, npix, nchan, nt, pitch);
     return cudaGetLastError();
 }
