@@ -125,6 +125,7 @@ int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offse
                int32_t *argmax, nsfrb_cand *cands, uint32_t cap, uint32_t *ncands, int *launches)
 {
     int slices = (pl->nw_used > 0) ? pl->n_groups * pl->n_wb : 0;
+    bool finalized = false;
     if (slices > 0) {
         SearchParams sp;
         sp.W = pl->d_W; sp.delays_u = pl->d_delays_u; sp.dmax_u = pl->d_dmax_u; sp.k_of_u = pl->d_k_of_u;
@@ -135,7 +136,7 @@ int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offse
         sp.H = pl->H; sp.RS = pl->RS; sp.wmax = pl->wmax_used; sp.tab_cap = pl->tab_cap;
         if (search3_usable(pl)) { // plan-specialised kernel (same algorithm, compiled per plan)
             std::string err;
-            if (int rc = search3_launch(pl, st, err)) return fail(rc, err);
+            if (int rc = search3_launch(pl, st, snr_map, argmax, &finalized, err)) return fail(rc, err);
             slices = search3_slices(pl);
         } else {
             CU(launch_search(sp, pl->smem_search, st), "k_search launch");
@@ -149,8 +150,10 @@ int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offse
     fp.npix = pl->npix; fp.nchan = pl->nchan; fp.pitch = pl->pitch; fp.ring_L = pl->nt;
     fp.origin = origin; fp.len = len; fp.raw_end_min = raw_end_min; fp.slices = slices; fp.t_offset = t_offset;
     fp.j_of_used = pl->d_j_of_used;
-    CU(launch_finalize(fp, pl->smem_final, st), "k_finalize launch");
-    ++*launches;
+    if (!finalized) {
+        CU(launch_finalize(fp, pl->smem_final, st), "k_finalize launch");
+        ++*launches;
+    }
     mark(pl, 3, st);
     CU(cudaMemsetAsync(ncands, 0, sizeof(uint32_t), st), "memset ncands");
     CU(launch_compact(snr_map, argmax, pl->npix, pl->threshold, cands, cap, ncands, st), "k_compact launch");

@@ -131,7 +131,8 @@ void free_plan(nsfrb_plan *p);
 // True if the plan can use k_search3 (at most 32 usable widths; NSFRB_SEARCH_JIT=0 forces the generic k_search).
 bool search3_usable(const nsfrb_plan *pl);
 int search3_source(const nsfrb_plan *pl, std::string &src, std::string &err);
-int search3_launch(nsfrb_plan *pl, cudaStream_t st, std::string &err); // compiles on first use; fills pl->d_partials
+// compiles on first use; fills pl->d_partials; *finalized = the kernel also wrote snr_map/argmax (fused a6)
+int search3_launch(nsfrb_plan *pl, cudaStream_t st, float *snr_map, int32_t *argmax, bool *finalized, std::string &err);
 void search3_free(nsfrb_plan *p);
 int search3_slices(const nsfrb_plan *pl); // partial records per pixel written by the last search3_launch
 

@@ -4,6 +4,7 @@
 //   NCHAN NU NW RS H PITCH NT WMID TRIALS MINB   integers (RS raw-tile row stride, H prefix ring length, PITCH workspace row)
 //   D_TAB[NU][NCHAN]  delays of the unique trials (dmax ascending)   DMAX_TAB[NU]   K_OF_U[NU]
 //   W_TAB[NW]         the usable widths, caller's order (NW <= 32)    J_OF_W[NW]     original width index
+//   FUSED             1: the kernel also does the per-pixel reduction and arg-max time (a6), no k_finalize launch
 // Same algorithm as the generic k_search (nsfrb_search.cu: one CTA = one pixel x 16 trials, 256-sample blocks,
 // cp.async raw prefetch, differential dedispersion, warp = trial, prefix ring in shared memory, exact bound-based
 // pruning of wide boxcars), with what the plan fixes folded into the instruction stream:
@@ -26,6 +27,10 @@ struct Search3Params {
     const float *W; // [npix][NCHAN][PITCH] time-contiguous workspace, baseline removed
     Partial3 *partials; // [npix][NGRP]
     int npix;
+    // FUSED: the last CTA of a pixel to finish reduces the pixel's partials and finds the arg-max time
+    int *counter;   // [npix], zero between launches (the last CTA resets it)
+    float *snr_map; // [npix]
+    int *argmax;    // [3][npix]
 };
 
 namespace s3 {
@@ -301,6 +306,105 @@ __device__ __forceinline__ void search_block(Trial &T, const float *stage_row, f
     __syncwarp();
 }
 
+// ---- a6, last step, fused: best group of the pixel, then the arg-max time by recomputing the winning series
+// (L2-hot: the pixel's CTAs have just read it) over the starts that can hold it, with the mean/sigma the search found.
+__device__ __forceinline__ void finalize_pixel(const Search3Params &P, float *fs, int p)
+{
+    constexpr int NTHR = NWARP * 32, PER = NTHR / 32;
+    float *sc_f = fs + NT + 2;                        // [NTHR]
+    int *sc_i = reinterpret_cast<int *>(sc_f + NTHR); // [NTHR]
+    __shared__ Partial3 best;
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        Partial3 b;
+        b.snr = -S3_INF; b.k = -1; b.j = -1; b.blk = -1; b.mu = 0.f; b.sigma = 0.f; b.u = -1; b.pad = 0;
+        const int4 *pp = reinterpret_cast<const int4 *>(P.partials + (size_t)p * NGRP);
+        for (int g = 0; g < NGRP; ++g) {
+            const int4 lo = __ldcg(pp + 2 * g), hi = __ldcg(pp + 2 * g + 1); // written by other CTAs: bypass L1
+            const float snr = __int_as_float(lo.x);
+            if (better(snr, lo.y, lo.z, b.snr, b.k, b.j)) {
+                b.snr = snr; b.k = lo.y; b.j = lo.z; b.blk = lo.w;
+                b.mu = __int_as_float(hi.x); b.sigma = __int_as_float(hi.y); b.u = hi.z; b.pad = hi.w;
+            }
+        }
+        best = b;
+    }
+    __syncthreads();
+    const Partial3 b = best;
+    if (b.k < 0) {
+        if (tid == 0) {
+            P.snr_map[p] = -S3_INF;
+            P.argmax[p] = -1; P.argmax[(size_t)P.npix + p] = -1; P.argmax[2 * (size_t)P.npix + p] = -1;
+        }
+        return;
+    }
+    const int w = W_TAB[b.j];
+    const int T = NT - DMAX_TAB[b.u];
+    const int n = T; // samples [0, T): every start 0..T-w is a candidate
+    const float *Wp = P.W + (size_t)p * NCHAN * (size_t)PITCH;
+    for (int i = tid; i < n; i += NTHR) {
+        float s0 = 0.f, s1 = 0.f;
+        sfor<0, NCHAN>([&](auto c) {
+            const float v = __ldg(Wp + (size_t)V(c) * PITCH + i + D_TAB[b.u][V(c)]);
+            if constexpr ((V(c) & 1) == 0) s0 += v; else s1 += v;
+        });
+        fs[i + 1] = (s0 + s1) - b.mu;
+    }
+    if (tid == 0) fs[0] = 0.f;
+    __syncthreads();
+    // block-wide inclusive scan of fs[1..n]: odd-length chunk per thread (conflict-free)
+    const int ch = ((n + NTHR - 1) / NTHR) | 1;
+    const int a0 = 1 + tid * ch, a1 = (a0 + ch < n + 1) ? a0 + ch : n + 1;
+    float tot = 0.f;
+    for (int i = a0; i < a1; ++i) tot += fs[i];
+    sc_f[tid] = tot;
+    __syncthreads();
+    if (tid < 32) { // scan of the NTHR chunk totals by one warp, PER per lane
+        float v[PER], run = 0.f;
+#pragma unroll
+        for (int i = 0; i < PER; ++i) { v[i] = sc_f[tid * PER + i]; run += v[i]; }
+        float incl = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const float y = __shfl_up_sync(kFull, incl, o);
+            if (tid >= o) incl += y;
+        }
+        float ex = incl - run;
+#pragma unroll
+        for (int i = 0; i < PER; ++i) { sc_f[tid * PER + i] = ex; ex += v[i]; }
+    }
+    __syncthreads();
+    {
+        float run = sc_f[tid];
+        for (int i = a0; i < a1; ++i) { run += fs[i]; fs[i] = run; }
+    }
+    __syncthreads();
+    // arg-max over starts i in [0, n-w]: B = P[i+w] - P[i], smallest i on ties
+    float bv = -S3_INF;
+    int bi = 0x7fffffff;
+    for (int i = tid; i <= n - w; i += NTHR) {
+        const float B = fs[i + w] - fs[i];
+        if (B > bv) { bv = B; bi = i; }
+    }
+    sc_f[tid] = bv; sc_i[tid] = bi;
+    __syncthreads();
+    for (int o = NTHR / 2; o > 0; o >>= 1) {
+        if (tid < o) {
+            const float ov = sc_f[tid + o]; const int oi = sc_i[tid + o];
+            if (ov > sc_f[tid] || (ov == sc_f[tid] && oi < sc_i[tid])) { sc_f[tid] = ov; sc_i[tid] = oi; }
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        const float B = sc_f[0];
+        const float S = b.sigma > 0.f ? B / (b.sigma * sqrtf((float)w)) : 0.f;
+        P.snr_map[p] = S;
+        P.argmax[p] = b.k;
+        P.argmax[(size_t)P.npix + p] = J_OF_W[b.j];
+        P.argmax[2 * (size_t)P.npix + p] = sc_i[0];
+    }
+}
+
 constexpr int kSmemFloats = NCHAN * RS + 4 + NWARP * SS + NWARP * H + NWARP * NR + NWARP * 8;
 
 template <int G> __device__ __forceinline__ void run_group(const Search3Params &P, float *smem, int p)
@@ -428,6 +532,20 @@ template <int G> __device__ __forceinline__ void run_group(const Search3Params &
         }
         P.partials[(size_t)p * NGRP + G] = out;
     }
+#if FUSED
+    __shared__ int is_last;
+    if (tid == 0) {
+        __threadfence(); // the partial is visible before the ticket is taken
+        const int prev = atomicAdd(P.counter + p, 1);
+        is_last = (prev == NGRP - 1);
+        if (is_last) P.counter[p] = 0; // ready for the next launch
+    }
+    __syncthreads();
+    if (is_last) {
+        __threadfence();
+        finalize_pixel(P, smem, p);
+    }
+#endif
 }
 
 template <int G0, int N> __device__ __forceinline__ void dispatch(int g, const Search3Params &P, float *smem, int p)
