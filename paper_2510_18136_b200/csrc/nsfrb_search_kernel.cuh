@@ -1,7 +1,7 @@
 // k_search3: the offline search kernel (steps a1..a6 of DESIGN.md), specialised per plan.
 //
 // Compiled at the first nsfrb_search of a plan (NVRTC, sm_100a) behind a generated prologue, like k_stream:
-//   NCHAN NU NW RS H PITCH NT WMID TRIALS MINB   integers (RS raw-tile row stride, H prefix ring length, PITCH workspace row)
+//   NCHAN NU NW RS H PITCH NT WMID TRIALS MINB CHAIN16 FUSED   integers (RS raw-tile row stride, H prefix ring length, PITCH workspace row)
 //   D_TAB[NU][NCHAN]  delays of the unique trials (dmax ascending)   DMAX_TAB[NU]   K_OF_U[NU]
 //   W_TAB[NW]         the usable widths, caller's order (NW <= 32)    J_OF_W[NW]     original width index
 //   FUSED             1: the kernel also does the per-pixel reduction and arg-max time (a6), no k_finalize launch
@@ -108,13 +108,15 @@ __device__ __forceinline__ bool better(float s, int k, int j, float bs, int bk, 
     return j < bj;
 }
 
-// ---- phase 1: differential dedispersion of one block for the 8 trials of half HALF of group G.
-// Thread tl (0..255) owns sample tl of the block; rt = raw + tl; so = stage + (HALF*8)*SS + tl + 4*(tl>>5).
-template <int G, int HALF> __device__ __forceinline__ void dedisperse8(const float *rt, float *so)
+// ---- phase 1: differential dedispersion of one block for LEN consecutive trials of group G, starting at trial
+// FIRST of the group.  Thread tl (0..255) owns sample tl of the block; rt = raw + tl; so = stage + FIRST*SS + tl + 4*(tl>>5).
+// LEN = 8: two chains per 16-trial group run side by side (all 512 threads busy); LEN = 16 (CHAIN16, many channels):
+// one chain by half the threads -- the full channel sum of a chain's first trial is paid once instead of twice.
+template <int G, int FIRST, int LEN> __device__ __forceinline__ void dedisperse(const float *rt, float *so)
 {
     float acc = 0.f;
-    sfor<0, 8>([&](auto s) {
-        constexpr int u = G * NWARP + HALF * 8 + V(s);
+    sfor<0, LEN>([&](auto s) {
+        constexpr int u = G * NWARP + FIRST + V(s);
         if constexpr (u < NU) {
             if constexpr (V(s) == 0) {
                 float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
@@ -455,10 +457,12 @@ template <int G> __device__ __forceinline__ void run_group(const Search3Params &
             const float *rt = raw + tl;
             float *so = stage + tl + 4 * (tl >> 5);
             if constexpr (NWARP == 8) {
-                dedisperse8<G, 0>(rt, so);
+                dedisperse<G, 0, 8>(rt, so);
+            } else if constexpr (CHAIN16) {
+                if (tid < LB) dedisperse<G, 0, 16>(rt, so);
             } else {
-                if (tid < LB) dedisperse8<G, 0>(rt, so);
-                else dedisperse8<G, 1>(rt, so + 8 * SS);
+                if (tid < LB) dedisperse<G, 0, 8>(rt, so);
+                else dedisperse<G, 8, 8>(rt, so + 8 * SS);
             }
         }
         __syncthreads(); // stage(b) complete; the raw tile is free again
