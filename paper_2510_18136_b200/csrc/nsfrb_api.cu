@@ -316,6 +316,12 @@ int nsfrb::plan_host_init(nsfrb_plan **out, int nx, int ny, int nchan, int nt, c
     pl->n_groups = (pl->nuniq + kSearchWarps - 1) / kSearchWarps;
     pl->n_wb = std::max(1, (pl->nw_used + kWidthBatch - 1) / kWidthBatch);
     pl->H = round_up(std::max(pl->wmax_used, 1) + kBlockLen + 32, 32);
+    {   // a power-of-two ring makes every wrap one AND (k_search3); take it when the shared memory allows
+        int h2 = 32;
+        while (h2 < pl->H) h2 <<= 1;
+        const int RS0 = round_up(kBlockLen + pl->dmax_all, 4);
+        if (search_smem_bytes(nchan, RS0, h2, 4096) + 4096 <= kMaxSmem) pl->H = h2;
+    }
     pl->RS = round_up(kBlockLen + pl->dmax_all, 4);
     pl->pitch = round_up(nt, 4);
     build_dd_tables(pl);

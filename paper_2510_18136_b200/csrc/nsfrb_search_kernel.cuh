@@ -43,6 +43,24 @@ constexpr int SS = 288;    // staging stride per trial: t + 4*(t>>5)
 constexpr int NR = H / 32; // ring rows
 constexpr int NGRP = (NU + NWARP - 1) / NWARP;
 
+// ring arithmetic: H (and NR = H/32) a power of two turns every wrap into one AND
+constexpr bool HP2 = (H & (H - 1)) == 0;
+__device__ __forceinline__ int wrapUp(int x) // x in [0, 2H)
+{
+    if constexpr (HP2) return x & (H - 1);
+    else return x >= H ? x - H : x;
+}
+__device__ __forceinline__ int wrapDn(int x) // x in (-H, H)
+{
+    if constexpr (HP2) return x & (H - 1);
+    else return x < 0 ? x + H : x;
+}
+__device__ __forceinline__ int wrapR(int r) // r in [0, 2NR)
+{
+    if constexpr (HP2) return r & (NR - 1);
+    else return r >= NR ? r - NR : r;
+}
+
 template <int I> struct IC { static constexpr int v = I; };
 #define V(x) (decltype(x)::v)
 template <int I, int N, class F> __device__ __forceinline__ void sfor(F &&f)
@@ -195,7 +213,7 @@ __device__ __forceinline__ void search_block(Trial &T, const float *stage_row, f
     T.carry = __shfl_sync(kFull, p8[7], 31);
 
     int sb = T.tpos + 8 * lane; // ring slot of sample tb (8 | H: the 8 slots never straddle the wrap)
-    if (sb >= H) sb -= H;
+    sb = wrapUp(sb);
     {
         float4 *rp = reinterpret_cast<float4 *>(ring + sb);
         rp[0] = make_float4(p8[0], p8[1], p8[2], p8[3]);
@@ -220,8 +238,8 @@ __device__ __forceinline__ void search_block(Trial &T, const float *stage_row, f
 #pragma unroll
         for (int i = 0; i < 8; ++i) Wn[16 + i] = p8[i];
         int s2b = sb - 16, s1b = sb - 8;
-        if (s2b < 0) s2b += H;
-        if (s1b < 0) s1b += H;
+        s2b = wrapDn(s2b);
+        s1b = wrapDn(s1b);
         const float4 *w2 = reinterpret_cast<const float4 *>(ring + s2b);
         const float4 *w1 = reinterpret_cast<const float4 *>(ring + s1b);
         const float4 a = w2[0], b = w2[1], c = w1[0], d = w1[1];
@@ -242,10 +260,10 @@ __device__ __forceinline__ void search_block(Trial &T, const float *stage_row, f
             constexpr int w = W_TAB[mid_idx(V(q))];
             constexpr int r = (4 - (w & 3)) & 3; // (sb - w) mod 4, sb being a multiple of 8
             int a0 = sb - w - r;                 // aligned slot of the first float4
-            if (a0 < 0) a0 += H;
+            a0 = wrapDn(a0);
             int a1 = a0 + 4, a2 = a0 + 8;
-            if (a1 >= H) a1 -= H;
-            if (a2 >= H) a2 -= H;
+            a1 = wrapUp(a1);
+            a2 = wrapUp(a2);
             const float4 x0 = *reinterpret_cast<const float4 *>(ring + a0);
             const float4 x1 = *reinterpret_cast<const float4 *>(ring + a1);
             float v[12] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w, 0.f, 0.f, 0.f, 0.f};
@@ -265,7 +283,7 @@ __device__ __forceinline__ void search_block(Trial &T, const float *stage_row, f
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             int pos = T.tpos + lane + 32 * i;
-            if (pos >= H) pos -= H;
+            pos = wrapUp(pos);
             const float v = (INSIDE || t0 + lane + 32 * i + 1 <= T_k) ? ring[pos] : -S3_INF;
             Pe[i] = v;
             emx = fmaxf(emx, v);
@@ -278,7 +296,7 @@ __device__ __forceinline__ void search_block(Trial &T, const float *stage_row, f
 #pragma unroll
             for (int q = 0; q < 9; ++q) {
                 mn = fminf(mn, rmin[r]);
-                if (++r == NR) r = 0;
+                r = wrapR(r + 1);
             }
             surv = (Emax - mn) > T.M;
         }
@@ -287,7 +305,7 @@ __device__ __forceinline__ void search_block(Trial &T, const float *stage_row, f
             const int j = __ffs(mask) - 1;
             mask &= mask - 1;
             int q = T.tpos - W_TAB[j]; // ring slot of the start that belongs to end slot tpos
-            if (q < 0) q += H;
+            q = wrapDn(q);
             float v = -S3_INF;
             if (q + LB <= H) {
                 const float *b = ring + q + lane;
@@ -297,7 +315,7 @@ __device__ __forceinline__ void search_block(Trial &T, const float *stage_row, f
 #pragma unroll
                 for (int i = 0; i < 8; ++i) {
                     int a = q + lane + 32 * i;
-                    if (a >= H) a -= H;
+                    a = wrapUp(a);
                     v = fmaxf(v, Pe[i] - ring[a]);
                 }
             }
@@ -473,9 +491,9 @@ template <int G> __device__ __forceinline__ void run_group(const Search3Params &
             else search_block<false>(T, stage + warp * SS, ring, rmin, lane, t0, T_k, wl, is_large);
         }
         T.tpos += LB;
-        if (T.tpos >= H) T.tpos -= H;
+        T.tpos = wrapUp(T.tpos);
         T.rr += LB / 32;
-        if (T.rr >= NR) T.rr -= NR;
+        T.rr = wrapR(T.rr);
     }
 
     // ---- a6 (per trial): exact mean / variance, normalise, best width
