@@ -427,3 +427,13 @@ def test_more_than_32_widths_use_the_generic_kernel():
     st, cs, snr32, arg32 = _offline(wl32, cube, label="w32 specialised")
     same = arg40[:, 1] < 32
     assert same.any() and np.all(np.abs(snr40[same] - snr32[same]) <= PU.tol(snr40[same]))
+
+
+def test_stream_64_channels():
+    """Real-time path on a 64-channel plan (config-5 band and DM spacing, 24 trials): the kernel is compiled with
+    one time step per tile; pushes compared with the oracle while the ring fills and after it wraps."""
+    wl = W.config("c5")
+    from dataclasses import replace
+    wl = replace(wl, nx=8, ny=5, nt=400, dm_list=np.linspace(0.0, 5000.0, 256)[:24], streaming=True, chunk_nt=25,
+                 width_list=np.asarray([1, 2, 3, 5, 8, 13, 21, 55, 144, 300], np.int32), name="c5-stream")
+    _stream_case(wl, 20, eval_at={0, 1, 5, 15, 16, 17, 19})
