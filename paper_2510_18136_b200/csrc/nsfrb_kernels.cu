@@ -179,6 +179,91 @@ __global__ void __launch_bounds__(256) k_finalize(const FinalParams F)
     }
 }
 
+// The same for short series (nt <= 2048): one WARP per pixel, 8 pixels per CTA, no block-wide barrier -- the
+// block-per-pixel version spends its time in __syncthreads when a series is only a few hundred samples (C4).
+__global__ void __launch_bounds__(256) k_finalize_warp(const FinalParams F)
+{
+    extern __shared__ __align__(16) float fsw[]; // [8][pitchw]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int p = blockIdx.x * 8 + warp;
+    if (p >= F.npix) return;
+    const int pitchw = F.len + 3;
+    float *fs = fsw + (size_t)warp * pitchw;
+    // best slice of the pixel (lane 0), broadcast
+    Partial b;
+    b.snr = -CUDART_INF_F; b.k = -1; b.j = -1; b.blk = -1; b.mu = 0.f; b.sigma = 0.f; b.u = -1; b.pad = 0;
+    if (lane == 0) {
+        const Partial *pp = F.partials + (size_t)p * F.slices;
+        for (int s = 0; s < F.slices; ++s) {
+            const Partial c = pp[s];
+            if (better(c.snr, c.k, c.j, b.snr, b.k, b.j)) b = c;
+        }
+    }
+    b.k = __shfl_sync(kFull, b.k, 0); b.j = __shfl_sync(kFull, b.j, 0); b.u = __shfl_sync(kFull, b.u, 0);
+    b.mu = __shfl_sync(kFull, b.mu, 0); b.sigma = __shfl_sync(kFull, b.sigma, 0);
+    if (b.k < 0) {
+        if (lane == 0) {
+            F.snr_map[p] = -CUDART_INF_F;
+            F.argmax[p] = -1; F.argmax[(size_t)F.npix + p] = -1; F.argmax[2 * (size_t)F.npix + p] = -1;
+        }
+        return;
+    }
+    const int w = __ldg(F.widths + b.j);
+    const int dmax = __ldg(F.dmax_u + b.u);
+    const int T = F.len - dmax;
+    const int emin = F.raw_end_min - dmax + 1;
+    const int ta = max(w, emin) - w; // first start
+    const int n = T - ta;            // samples [ta, T)
+    const int32_t *dk = F.delays_u + (size_t)b.u * F.nchan;
+    const float *Wp = F.W + (size_t)p * F.nchan * (size_t)F.pitch;
+    for (int i = lane; i < n; i += 32) {
+        float s = 0.f;
+        for (int c = 0; c < F.nchan; ++c) {
+            int slot = F.origin + ta + i + __ldg(dk + c);
+            if (slot >= F.ring_L) slot -= F.ring_L;
+            s += __ldg(Wp + (size_t)c * F.pitch + slot);
+        }
+        fs[i + 1] = s - b.mu;
+    }
+    if (lane == 0) fs[0] = 0.f;
+    __syncwarp();
+    // inclusive scan of fs[1..n]: odd-length chunk per lane (conflict-free), one warp scan of the chunk totals
+    const int ch = ((n + 31) / 32) | 1;
+    const int a0 = 1 + lane * ch, a1 = min(a0 + ch, n + 1);
+    float tot = 0.f;
+    for (int i = a0; i < a1; ++i) tot += fs[i];
+    float incl = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const float y = __shfl_up_sync(kFull, incl, o);
+        if (lane >= o) incl += y;
+    }
+    {
+        float run = incl - tot;
+        for (int i = a0; i < a1; ++i) { run += fs[i]; fs[i] = run; }
+    }
+    __syncwarp();
+    float bv = -CUDART_INF_F;
+    int bi = 0x7fffffff;
+    for (int i = lane; i <= n - w; i += 32) {
+        const float B = fs[i + w] - fs[i];
+        if (B > bv) { bv = B; bi = i; }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float ov = __shfl_xor_sync(kFull, bv, o);
+        const int oi = __shfl_xor_sync(kFull, bi, o);
+        if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    }
+    if (lane == 0) {
+        const float S = b.sigma > 0.f ? bv / (b.sigma * sqrtf((float)w)) : 0.f;
+        F.snr_map[p] = S;
+        F.argmax[p] = b.k;
+        F.argmax[(size_t)F.npix + p] = __ldg(F.j_of_used + b.j);
+        F.argmax[2 * (size_t)F.npix + p] = (int32_t)(((uint32_t)F.t_offset + (uint32_t)(ta + bi)) & 0x7fffffffu);
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // a7: snr > threshold -> candidate list, one atomicAdd per warp.
 // ------------------------------------------------------------------------------------------
@@ -261,10 +346,20 @@ cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, i
 
 cudaError_t launch_finalize(const FinalParams &p, size_t smem_bytes, cudaStream_t st)
 {
-    static size_t granted[64] = {0}; // per-device function attribute shared by all plans: only ever raise it
+    static size_t granted[64] = {0}, granted_w[64] = {0}; // per-device function attributes shared by all plans: only ever raise them
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
+    if (p.len <= 2048) { // short series: one warp per pixel
+        const size_t smw = 8 * ((size_t)p.len + 3) * sizeof(float);
+        if (dev >= 0 && dev < 64 && smw > granted_w[dev]) {
+            e = cudaFuncSetAttribute(k_finalize_warp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smw);
+            if (e != cudaSuccess) return e;
+            granted_w[dev] = smw;
+        }
+        k_finalize_warp<<<(p.npix + 7) / 8, 256, smw, st>>>(p);
+        return cudaGetLastError();
+    }
     if (dev >= 0 && dev < 64 && smem_bytes > granted[dev]) {
         e = cudaFuncSetAttribute(k_finalize, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
         if (e != cudaSuccess) return e;
