@@ -122,11 +122,15 @@ def barrier(world):
 class StreamBench:
     """C2: ring filled to steady state, then timed pushes."""
 
-    def __init__(self, wl, plan_mod):
+    def __init__(self, wl, plan_mod, cubes=False):
         self.wl = wl
         self.plan = plan_mod.Plan.for_workload(wl, cand_capacity=4096)
         self.delays = self.plan.delays()
         self.info = self.plan.info()
+        if cubes:  # NEXT 3: also write the per-(dm, width, pixel) S/N and TOA cubes every push
+            shape = (len(wl.dm_list), len(wl.width_list), wl.npix)
+            self.cubes = (torch.empty(shape, device="cuda"), torch.empty(shape, dtype=torch.int32, device="cuda"))
+            self.plan.stream_set_cubes(*self.cubes)
         n_fill = -(-wl.nt // wl.chunk_nt) + 1
         self.src = W.ChunkSource(wl, self.delays, n_fill + 600, "cuda")
         self.out = self.plan.alloc_outputs()
@@ -232,7 +236,7 @@ def run_cuda_arm(args, rank, world, local):
     torch.cuda.set_device(local)
     hbm_peak, peak_src, peaks = measured_peaks()
     wl = W.config(args.workload)
-    bench = StreamBench(wl, nsfrb) if wl.streaming else OfflineBench(wl, nsfrb)
+    bench = StreamBench(wl, nsfrb, cubes=args.cubes) if wl.streaming else OfflineBench(wl, nsfrb)
 
     flusher = None
     if bench.algorithmic_bytes() < (256 << 20):
@@ -336,7 +340,7 @@ def run_cuda_arm(args, rank, world, local):
                    "ndm": len(wl.dm_list), "ndm_unique": info["ndm_unique"], "nwidth": len(wl.width_list),
                    "cells_per_step": bench.cells_per_step,
                    "l2": "inputs larger than L2 (ring 6.4 GB + rotating chunks)" if flusher is None else "L2 flushed between steps",
-                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+                   "parallelism": "replicas only" if world > 1 else "1 GPU", "cubes": bool(args.cubes and wl.streaming)},
         "e2e": e2e, "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
         "clocks": clocks,
         "roofline": roof,
@@ -465,6 +469,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cubes", action="store_true", help="c2: also write the S/N and TOA cubes every push (NEXT 3)")
     ap.add_argument("--op", default="search", choices=["search", "bin"], help="bin: time the binning kernel (NEXT 2)")
     ap.add_argument("--bin-factor", type=int, default=5)
     args = ap.parse_args()

@@ -121,6 +121,18 @@ int nsfrb_stream_push(nsfrb_plan *plan, const float *chunk, int chunk_nt, void *
                       float *snr_map, int32_t *argmax,
                       nsfrb_cand *cands, uint32_t cand_capacity, uint32_t *ncands);
 
+/*
+ * Optional cube outputs of the real-time path ("the S/N and TOA for all pixels, widths and DMs" are
+ * kept for post-processing).  After this call every nsfrb_stream_push also writes, on its stream,
+ *   snr_cube  device, [ndm][nwidth][npix] float32: max over this push's windows of S(k, j, t); -INFINITY where the
+ *             (dm, width) has no window yet (or never: width longer than the ring)
+ *   toa_cube  device, same shape, int32: the window start attaining it (smallest on ties), absolute like argmax's t;
+ *             -1 where no window exists
+ * in the caller's dm_list / width_list order (pixel-contiguous, like the input).  Trials whose delay vector repeats an
+ * earlier one repeat its planes.  Pass two NULLs to switch the outputs off.  The caller owns both buffers.
+ */
+int nsfrb_stream_set_cubes(nsfrb_plan *plan, float *snr_cube, int32_t *toa_cube);
+
 /* Forget all pushed samples; the plan can be used for nsfrb_search again. */
 int nsfrb_stream_reset(nsfrb_plan *plan);
 

@@ -434,6 +434,14 @@ int nsfrb_stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, void *st
     return NSFRB_OK;
 }
 
+int nsfrb_stream_set_cubes(nsfrb_plan *pl, float *snr_cube, int32_t *toa_cube)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    std::string err;
+    if (int rc = stream_set_cubes(pl, snr_cube, toa_cube, err)) return fail(rc, err);
+    return NSFRB_OK;
+}
+
 int nsfrb_stream_reset(nsfrb_plan *pl)
 {
     if (!pl) return fail(NSFRB_EINVAL, "plan is null");

@@ -117,6 +117,8 @@ struct nsfrb_plan {
     bool ev_valid = false;
     // real-time path (nsfrb_stream.cu): ring, provisional means, plan-specialised kernel
     nsfrb::StreamState *stream = nullptr;
+    float *cube_snr = nullptr;   // caller's optional cube outputs of the real-time path (nsfrb_stream_set_cubes)
+    int32_t *cube_toa = nullptr;
     // offline path: plan-specialised k_search3 (nsfrb_search_kernel.cuh), compiled at the first nsfrb_search
     nsfrb::Search3State *search3 = nullptr;
 };
@@ -139,6 +141,7 @@ int search3_slices(const nsfrb_plan *pl); // partial records per pixel written b
 // ---- real-time path (nsfrb_stream.cu)
 void stream_free(nsfrb_plan *p);
 void stream_reset(nsfrb_plan *p);
+int stream_set_cubes(nsfrb_plan *pl, float *snr_cube, int32_t *toa_cube, std::string &err);
 size_t stream_bytes(const nsfrb_plan *p); // device bytes the real-time path holds (0 before the first push)
 // a8 + k_stream passes + reduction over slices; outputs as nsfrb_stream_push.  Returns an NSFRB_* code and
 // leaves the message in `err`.

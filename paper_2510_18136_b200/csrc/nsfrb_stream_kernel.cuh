@@ -8,7 +8,7 @@
 // ahead of time with the BASELINE config-2 prologue as a build check.
 //
 // Prologue (see nsfrb_jit.cu: make_stream_prologue):
-//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD   integers
+//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD NW_ALL   integers (NW_ALL: length of the caller's width list)
 //   D_TAB[NU][NCHAN]   integer delays d[u][c] of the unique trials, DM ascending
 //   DMAX_TAB[NU]       dmax_u                 K_OF_U[NU]  lowest original dm index of the trial
 //   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index   RSQ_W[NW]  1/sqrt(width)
@@ -59,6 +59,10 @@ struct StreamParams {
     int *aws;           // their end indices, same shape
     float *sws;         // segment totals S1, S2  [pixel block][supergroup][2][GPC*KK][SEG][32]
     int bound[9];       // segment q < SEG marches steps (bound[q], bound[q+1]], multiples of TT (SEG <= 8)
+    // optional per-(trial, width) outputs (S/N and TOA kept for all pixels x widths x DMs), or null:
+    float *snr_cube;    // [NDM_ALL][NW_ALL][NPIX] peak S/N of every (dm, width) over this push's windows
+    int *toa_cube;      // same shape: its window start (absolute, t_offset added); -1 where no window exists
+    int t_offset;
 };
 
 namespace sk {
@@ -456,6 +460,13 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                                     const int ii = P.i0 + w.ag[(V(kk) * NW + j) * 32];
                                     const int t = Tk - ii - wj;
                                     if (better(S, K_OF_U[u], J_OF_W[j], t, bs, bk, bj, bt)) { bs = S; bk = K_OF_U[u]; bj = J_OF_W[j]; bt = t; }
+                                    if (P.snr_cube && live) { // cube entry: max over the passes of a push, ties to the smaller t
+                                        const long long ci = ((long long)K_OF_U[u] * NW_ALL + J_OF_W[j]) * NPIX + pix;
+                                        if (P.slice0 == 0 || S >= P.snr_cube[ci]) {
+                                            P.snr_cube[ci] = S;
+                                            P.toa_cube[ci] = (int)(((unsigned)P.t_offset + (unsigned)t) & 0x7fffffffu);
+                                        }
+                                    }
                                 }
                             }
                     });

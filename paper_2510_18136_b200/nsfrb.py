@@ -44,7 +44,7 @@ assert CAND_DTYPE.itemsize == ctypes.sizeof(nsfrb_cand) == 20
 EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stream_reset", "nsfrb_search_host",
            "nsfrb_stream_push_host", "nsfrb_plan_destroy", "nsfrb_plan_get_delays", "nsfrb_plan_get_info",
            "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
-           "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel")
+           "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes")
 
 _lib = None
 
@@ -70,6 +70,8 @@ def lib() -> ctypes.CDLL:
         L.nsfrb_search_host.argtypes = [vp, vp, vp] + out
         L.nsfrb_stream_push_host.restype = ctypes.c_int
         L.nsfrb_stream_push_host.argtypes = [vp, vp, ctypes.c_int, vp] + out
+        L.nsfrb_stream_set_cubes.restype = ctypes.c_int
+        L.nsfrb_stream_set_cubes.argtypes = [vp, vp, vp]
         L.nsfrb_stream_reset.restype = ctypes.c_int
         L.nsfrb_stream_reset.argtypes = [vp]
         L.nsfrb_plan_destroy.restype = ctypes.c_int
@@ -252,6 +254,20 @@ class Plan:
                                        out.snr_map.data_ptr(), out.argmax.data_ptr(), out.cands.data_ptr(),
                                        self.cand_capacity, out.ncands.data_ptr()))
         return out
+
+    def stream_set_cubes(self, snr_cube: torch.Tensor | None, toa_cube: torch.Tensor | None):
+        """nsfrb_stream_set_cubes: per-(dm, width, pixel) peak S/N [ndm][nwidth][npix] float32 and window start (int32)
+        written by every later push; None, None switches them off.  The tensors must stay alive."""
+        if snr_cube is None and toa_cube is None:
+            _check(lib().nsfrb_stream_set_cubes(self._h, None, None))
+            self._cubes = None
+            return
+        shape = (self.ndm, self.nwidth, self.npix)
+        for t, dt in ((snr_cube, torch.float32), (toa_cube, torch.int32)):
+            if t is None or not t.is_cuda or t.dtype != dt or not t.is_contiguous() or tuple(t.shape) != shape:
+                raise ValueError(f"cubes must be contiguous CUDA tensors of shape {shape} (float32 / int32)")
+        _check(lib().nsfrb_stream_set_cubes(self._h, snr_cube.data_ptr(), toa_cube.data_ptr()))
+        self._cubes = (snr_cube, toa_cube)
 
     def stream_reset(self):
         _check(lib().nsfrb_stream_reset(self._h))

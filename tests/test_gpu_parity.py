@@ -437,3 +437,53 @@ def test_stream_64_channels():
     wl = replace(wl, nx=8, ny=5, nt=400, dm_list=np.linspace(0.0, 5000.0, 256)[:24], streaming=True, chunk_nt=25,
                  width_list=np.asarray([1, 2, 3, 5, 8, 13, 21, 55, 144, 300], np.int32), name="c5-stream")
     _stream_case(wl, 20, eval_at={0, 1, 5, 15, 16, 17, 19})
+
+
+# ----------------------------------------------------------------------------- NEXT 3: S/N and TOA cubes (L94)
+def test_stream_cubes_match_oracle():
+    """nsfrb_stream_set_cubes: per-(dm, width, pixel) peak S/N and window start of every push against the oracle's
+    per-(k, j) maxima (details=True), incl. duplicate DMs (planes repeated), a width longer than the ring (-inf, -1),
+    the filling ring (widths without a window yet) and chunks longer than the first one (several passes)."""
+    from dataclasses import replace
+    nsfrb = _nsfrb()
+    dms = np.asarray([0.0, 300.0, 300.0, 900.0, 1400.0, 0.0], dtype=np.float64)
+    wl = replace(W.config("c1"), nx=8, ny=5, nt=160, dm_list=dms, streaming=True, threshold=5.0,
+                 width_list=np.asarray([2, 1, 500, 9, 40], np.int32), name="cubes")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    g = torch.Generator(device="cuda").manual_seed(51)
+    so = oracle.StreamOracle(wl.nchan, wl.npix, wl.nt, d, wl.width_list)
+    snr_cube = torch.zeros((len(dms), len(wl.width_list), wl.npix), device="cuda")
+    toa_cube = torch.zeros((len(dms), len(wl.width_list), wl.npix), dtype=torch.int32, device="cuda")
+    with nsfrb.Plan.for_workload(wl, cand_capacity=64) as plan:
+        plan.stream_set_cubes(snr_cube, toa_cube)
+        out = plan.alloc_outputs()
+        for i, c in enumerate([10, 3, 25, 60, 160, 7, 12]):
+            chunk = torch.randn((wl.nchan, c, wl.npix), device="cuda", generator=g)
+            plan.stream_push(chunk, out)
+            torch.cuda.synchronize()
+            n_prev = so.n
+            so.n += c
+            so.hist = np.concatenate([so.hist, chunk.cpu().numpy()], axis=1)[:, -so.L:, :]
+            lo = max(0, so.n - so.L)
+            r = oracle.search(so.hist, d, wl.width_list, raw_end_min=n_prev - lo, t_offset=lo, details=True)
+            S = snr_cube.cpu().numpy().transpose(2, 0, 1)      # [npix][ndm][nw]
+            Tm = toa_cube.cpu().numpy().transpose(2, 0, 1)
+            undefined = np.isneginf(r.best)
+            assert np.array_equal(np.isneginf(S), undefined), f"push {i}: defined sets differ"
+            assert np.all(Tm[undefined] == -1)
+            ok = ~undefined
+            assert np.all(np.abs(S[ok] - r.best[ok]) <= PU.tol(r.best[ok])), f"push {i}"
+            assert np.all(S[:, :, 2] == -np.inf)               # width 500 never fits the 160-sample ring
+            assert np.array_equal(S[:, 2], S[:, 1]) and np.array_equal(Tm[:, 2], Tm[:, 1])   # duplicate DM planes
+            assert np.array_equal(S[:, 5], S[:, 0])
+            # window starts: identical, or the oracle rates the GPU's window within tolerance of the maximum
+            diff = np.argwhere(ok & (Tm != r.best_t))
+            assert len(diff) <= 0.1 * ok.sum()
+            for p, k, j in diff:
+                s_at = oracle.snr_at(so.hist, d, wl.width_list, p, k, j, int(Tm[p, k, j]), raw_end_min=n_prev - lo, t_offset=lo)
+                assert s_at >= r.best[p, k, j] - 2 * PU.tol(r.best[p, k, j]), (i, p, k, j)
+            # the maps are the maxima of the cubes
+            assert np.allclose(out.snr_map.cpu().numpy(), S.reshape(wl.npix, -1).max(axis=1), rtol=0, atol=0)
+        plan.stream_set_cubes(None, None)
+        plan.stream_push(torch.randn((wl.nchan, 5, wl.npix), device="cuda", generator=g), out)
+        torch.cuda.synchronize()

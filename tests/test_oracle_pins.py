@@ -435,3 +435,24 @@ def test_binned_search_reuses_the_delay_table():
     assert tuple(r.argmax[0]) == (k, 2, t0)
     Tk = nt // 5 - d5[k].max()
     assert abs(r.snr[0] - np.sqrt(Tk - w)) < 1e-9      # noise-free closed form, as in the unbinned pin
+
+
+def test_per_trial_width_maxima_are_consistent():
+    """The oracle's [ndm][nw] cubes (details=True; PAPER.md:L94 keeps S/N and TOA for all widths and DMs): their maximum
+    is the map, the arg of the maximum is the arg-max, and the prefix and brute-force routines agree on them."""
+    rng = np.random.default_rng(94)
+    cube = rng.standard_normal((4, 90, 6)).astype(np.float32)
+    d = np.asarray([[0, 0, 0, 0], [3, 2, 1, 0], [7, 5, 2, 0]], dtype=np.int32)
+    w = [1, 4, 13, 200]
+    a = oracle.search(cube, d, w, details=True)
+    b = oracle.search(cube, d, w, details=True, brute=True)
+    assert np.allclose(a.best[:, :, :3], b.best[:, :, :3], rtol=0, atol=1e-12) and np.array_equal(a.best_t, b.best_t)
+    assert np.all(np.isneginf(a.best[:, :, 3])) and np.all(a.best_t[:, :, 3] == -1)      # width 200 > 90 samples
+    flat = a.best.reshape(6, -1)
+    assert np.array_equal(flat.max(axis=1), a.snr)
+    k, j = np.unravel_index(flat.argmax(axis=1), (3, 4))
+    assert np.array_equal(np.stack([k, j, a.best_t[np.arange(6), k, j]], axis=1), a.argmax)
+    # a width-1 maximum is the largest normalised sample of the dedispersed series (DM 0 row)
+    D0 = cube.astype(np.float64).sum(axis=0)
+    z = (D0 - D0.mean(axis=0)) / D0.std(axis=0)
+    assert np.allclose(a.best[:, 0, 0], z.max(axis=0), rtol=0, atol=1e-12) and np.array_equal(a.best_t[:, 0, 0], z.argmax(axis=0))
