@@ -101,17 +101,29 @@ __device__ __forceinline__ void cp_async16(float *dst, const float *src, int src
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// raw[c][i] = W[p][c][t0+i] for i < rows4 (PITCH is a multiple of 4: aligned 16-byte copies), zero beyond NT
-__device__ __forceinline__ void issue_raw(const float *Wp, float *raw, int t0, int rows4, int warp, int lane)
+// raw[c][i] = W[p][c][t0+i] for i < ROWS4 (PITCH is a multiple of 4: aligned 16-byte copies), zero beyond NT.
+// Blocks whose rows all lie inside the series take the unchecked path: one pointer pair per channel, static trip count.
+template <int ROWS4> __device__ __forceinline__ void issue_raw(const float *Wp, float *raw, int t0, int warp, int lane)
 {
-    for (int c = warp; c < NCHAN; c += NWARP) {
-        const float *src = Wp + (size_t)c * PITCH;
-        float *dst = raw + c * RS;
-        for (int i = lane * 4; i < rows4; i += 128) {
-            const int r = t0 + i;
-            int nvalid = NT - r;
-            nvalid = nvalid < 0 ? 0 : (nvalid > 4 ? 4 : nvalid);
-            cp_async16(dst + i, src + (nvalid ? r : 0), nvalid * 4);
+    constexpr int ITER = (ROWS4 + 127) / 128;
+    if (t0 + ROWS4 <= NT) {
+        for (int c = warp; c < NCHAN; c += NWARP) {
+            const float *src = Wp + (size_t)c * PITCH + t0 + lane * 4;
+            float *dst = raw + c * RS + lane * 4;
+#pragma unroll
+            for (int k = 0; k < ITER; ++k)
+                if (lane * 4 + 128 * k < ROWS4) cp_async16(dst + 128 * k, src + 128 * k, 16);
+        }
+    } else {
+        for (int c = warp; c < NCHAN; c += NWARP) {
+            const float *src = Wp + (size_t)c * PITCH;
+            float *dst = raw + c * RS;
+            for (int i = lane * 4; i < ROWS4; i += 128) {
+                const int r = t0 + i;
+                int nvalid = NT - r;
+                nvalid = nvalid < 0 ? 0 : (nvalid > 4 ? 4 : nvalid);
+                cp_async16(dst + i, src + (nvalid ? r : 0), nvalid * 4);
+            }
         }
     }
     cp_async_commit();
@@ -464,7 +476,7 @@ template <int G> __device__ __forceinline__ void run_group(const Search3Params &
     if (T.rr >= NR || T.rr < 0) T.rr = 0;
 
     const float *Wp = P.W + (size_t)p * NCHAN * (size_t)PITCH;
-    if (T_g > 0) issue_raw(Wp, raw, 0, rows4, warp, lane);
+    if (T_g > 0) issue_raw<rows4>(Wp, raw, 0, warp, lane);
     __syncthreads();
 
     for (int t0 = 0; t0 < T_g; t0 += LB) {
@@ -484,7 +496,7 @@ template <int G> __device__ __forceinline__ void run_group(const Search3Params &
             }
         }
         __syncthreads(); // stage(b) complete; the raw tile is free again
-        if (t0 + LB < T_g) issue_raw(Wp, raw, t0 + LB, rows4, warp, lane);
+        if (t0 + LB < T_g) issue_raw<rows4>(Wp, raw, t0 + LB, warp, lane);
 
         if (has && t0 < T_k) {
             if (t0 + LB <= T_k) search_block<true>(T, stage + warp * SS, ring, rmin, lane, t0, T_k, wl, is_large);
