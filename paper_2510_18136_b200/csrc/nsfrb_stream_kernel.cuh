@@ -8,7 +8,7 @@
 // ahead of time with the BASELINE config-2 prologue as a build check.
 //
 // Prologue (see nsfrb_jit.cu: make_stream_prologue):
-//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD NW_ALL   integers (NW_ALL: length of the caller's width list)
+//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD NW_ALL CUBES   integers (NW_ALL: length of the caller's width list; CUBES = 1 compiles the cube outputs in)
 //   D_TAB[NU][NCHAN]   integer delays d[u][c] of the unique trials, DM ascending
 //   DMAX_TAB[NU]       dmax_u                 K_OF_U[NU]  lowest original dm index of the trial
 //   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index   RSQ_W[NW]  1/sqrt(width)
@@ -460,6 +460,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                                     const int ii = P.i0 + w.ag[(V(kk) * NW + j) * 32];
                                     const int t = Tk - ii - wj;
                                     if (better(S, K_OF_U[u], J_OF_W[j], t, bs, bk, bj, bt)) { bs = S; bk = K_OF_U[u]; bj = J_OF_W[j]; bt = t; }
+#if CUBES
                                     if (P.snr_cube && live) { // cube entry: max over the passes of a push, ties to the smaller t
                                         const long long ci = ((long long)K_OF_U[u] * NW_ALL + J_OF_W[j]) * NPIX + pix;
                                         if (P.slice0 == 0 || S >= P.snr_cube[ci]) {
@@ -467,6 +468,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                                             P.toa_cube[ci] = (int)(((unsigned)P.t_offset + (unsigned)t) & 0x7fffffffu);
                                         }
                                     }
+#endif
                                 }
                             }
                     });
