@@ -114,7 +114,7 @@ int nsfrb_search(nsfrb_plan *plan, const float *cube, void *stream,
  * 1 <= chunk_nt <= nt.  Outputs as nsfrb_search.
  * The first push of a plan compiles the plan-specialised kernel with NVRTC (seconds to a minute, growing with
  * ndm*nchan) and allocates the ring (2*(nt + guard)*nchan*npix*4 B); a compile failure returns NSFRB_ECUDA with
- * the compiler log.  Compiled kernels are cached on disk (NSFRB_JIT_CACHE=<dir>, default /tmp/nsfrb_jit_cache;
+ * the compiler log.  Compiled kernels are cached on disk (NSFRB_JIT_CACHE=<dir>, default /tmp/nsfrb_jit_cache_<uid>, private to the user;
  * NSFRB_JIT_CACHE=0 disables).  Chunks longer than the plan's first chunk are searched in several passes.
  */
 int nsfrb_stream_push(nsfrb_plan *plan, const float *chunk, int chunk_nt, void *stream,
@@ -129,7 +129,8 @@ int nsfrb_stream_push(nsfrb_plan *plan, const float *chunk, int chunk_nt, void *
  *   toa_cube  device, same shape, int32: the window start attaining it (smallest on ties), absolute like argmax's t;
  *             -1 where no window exists
  * in the caller's dm_list / width_list order (pixel-contiguous, like the input).  Trials whose delay vector repeats an
- * earlier one repeat its planes.  Pass two NULLs to switch the outputs off.  The caller owns both buffers.
+ * earlier one repeat its planes.  Pass two NULLs to switch the outputs off.  The caller owns both buffers.  The first
+ * push after switching the outputs on compiles a second variant of the plan's kernel (seconds, cached).
  */
 int nsfrb_stream_set_cubes(nsfrb_plan *plan, float *snr_cube, int32_t *toa_cube);
 
