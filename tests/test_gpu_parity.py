@@ -117,7 +117,7 @@ def _check_recovery(wl, d, pulses, snr, frac=0.7):
 
 
 # ----------------------------------------------------------------------------- streaming (C2)
-def _stream_case(wl, n_push, eval_at, chunk_sizes=None, capacity=1024):
+def _stream_case(wl, n_push, eval_at, chunk_sizes=None, capacity=1024, cubes=False):
     nsfrb = _nsfrb()
     d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
     src = W.ChunkSource(wl, d, n_push, "cuda")
@@ -125,6 +125,10 @@ def _stream_case(wl, n_push, eval_at, chunk_sizes=None, capacity=1024):
     stats = []
     with nsfrb.Plan.for_workload(wl, cand_capacity=capacity) as plan:
         out = plan.alloc_outputs()
+        if cubes:
+            shape = (len(wl.dm_list), len(wl.width_list), wl.npix)
+            cs, ct = torch.zeros(shape, device="cuda"), torch.zeros(shape, dtype=torch.int32, device="cuda")
+            plan.stream_set_cubes(cs, ct)
         for i in range(n_push):
             if chunk_sizes is None:
                 chunk = src.next()
@@ -145,6 +149,12 @@ def _stream_case(wl, n_push, eval_at, chunk_sizes=None, capacity=1024):
                               t_offset=lo, label=f"{wl.name} push {i}")
                 PU.check_candidates(st["oracle"], np.arange(wl.npix), out.candidates(), out.n_found(), wl.threshold,
                                     capacity)
+                if cubes:  # the maps are the maxima of the cubes, bit for bit, and the arg-max entry holds the map's t
+                    S = cs.cpu().numpy().reshape(-1, wl.npix)
+                    assert np.array_equal(S.max(axis=0), snr)
+                    has = arg[:, 0] >= 0
+                    pp = np.nonzero(has)[0]
+                    assert np.array_equal(ct.cpu().numpy()[arg[pp, 0], arg[pp, 1], pp], arg[pp, 2])
                 stats.append(st)
         # offline search is refused while the plan holds streamed samples
         cube = torch.zeros((wl.nchan, wl.nt, wl.npix), device="cuda")
@@ -436,7 +446,7 @@ def test_stream_64_channels():
     from dataclasses import replace
     wl = replace(wl, nx=8, ny=5, nt=400, dm_list=np.linspace(0.0, 5000.0, 256)[:24], streaming=True, chunk_nt=25,
                  width_list=np.asarray([1, 2, 3, 5, 8, 13, 21, 55, 144, 300], np.int32), name="c5-stream")
-    _stream_case(wl, 20, eval_at={0, 1, 5, 15, 16, 17, 19})
+    _stream_case(wl, 20, eval_at={0, 1, 5, 15, 16, 17, 19}, cubes=True)   # 24 trials: two supergroups of CTAs
 
 
 # ----------------------------------------------------------------------------- NEXT 3: S/N and TOA cubes (L94)
