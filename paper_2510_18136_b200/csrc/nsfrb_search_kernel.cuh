@@ -460,8 +460,12 @@ template <int G> __device__ __forceinline__ void run_group(const Search3Params &
     constexpr int T_g = NT - DMAX_TAB[G * NWARP]; // longest series of the group
     constexpr int rows4 = (LB + dmax_g + 3) & ~3;
 
-    for (int i = lane; i < H; i += 32) ring[i] = (i == H - 1) ? 0.f : S3_INF; // P[0] = 0 at slot -1
-    for (int i = lane; i < NR; i += 32) rmin[i] = (i == NR - 1) ? 0.f : S3_INF;
+    // "before time 0": only the slots a start can reach from the first blocks need the +inf marker -- the last
+    // INIT slots of the ring (widest width + the 32-slot rows the bound looks at); the rest is written before it is read
+    constexpr int WMAXS = []() { int m = 1; for (int j = 0; j < NW; ++j) m = (W_TAB[j] > m && W_TAB[j] < H) ? W_TAB[j] : m; return m; }();
+    constexpr int INIT = ((WMAXS + 95) / 32) * 32 < H ? ((WMAXS + 95) / 32) * 32 : H;
+    for (int i = H - INIT + lane; i < H; i += 32) ring[i] = (i == H - 1) ? 0.f : S3_INF; // P[0] = 0 at slot -1
+    for (int i = NR - INIT / 32 + lane; i < NR; i += 32) rmin[i] = (i == NR - 1) ? 0.f : S3_INF;
 
     const int wl = lane < NW ? W_TAB[lane] : 0;
     const bool is_large = wl > WMID;
