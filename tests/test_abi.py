@@ -100,3 +100,37 @@ def test_product_path_does_not_import_oracle():
         if fn.endswith((".py", ".c")):
             src = open(os.path.join(ROOT, "oracle", fn)).read()
             assert "paper_2510_18136_b200" not in src and "libnsfrb.so" not in src, fn
+
+
+def test_header_is_valid_c99_and_a_c_caller_links(tmp_path):
+    """include/nsfrb.h must be usable from plain C: compile a C99 caller of the four main entry points against the
+    header and link it with the library (no GPU needed to link; the program is not run here)."""
+    import shutil
+    import subprocess
+    nsfrb = _lib()
+    gcc = shutil.which("gcc")
+    if gcc is None:
+        pytest.skip("gcc not available")
+    src = tmp_path / "caller.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include "nsfrb.h"
+int main(void)
+{
+    nsfrb_plan *plan = NULL;
+    const double f[2] = {1.3, 1.5}, dm[1] = {0.0};
+    const int32_t w[1] = {1};
+    int rc = nsfrb_plan_create(&plan, 4, 4, 2, 64, f, 0.1342, dm, 1, w, 1, 6.0f);
+    if (rc != NSFRB_OK) { printf("%s\n", nsfrb_last_error()); return 1; }
+    rc = nsfrb_search(plan, NULL, NULL, NULL, NULL, NULL, 0, NULL);          /* EINVAL: null cube */
+    rc = nsfrb_stream_push(plan, NULL, 25, NULL, NULL, NULL, NULL, 0, NULL); /* EINVAL: null chunk */
+    (void)sizeof(nsfrb_cand);
+    return nsfrb_plan_destroy(plan);
+}
+''')
+    inc = os.path.join(ROOT, "include")
+    libdir = os.path.dirname(nsfrb.LIB_PATH)
+    exe = tmp_path / "caller"
+    subprocess.check_call([gcc, "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", inc, str(src), "-o", str(exe),
+                           "-L", libdir, "-l:libnsfrb.so", f"-Wl,-rpath,{libdir}"])
+    assert exe.exists()
