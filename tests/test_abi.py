@@ -134,3 +134,6 @@ int main(void)
     subprocess.check_call([gcc, "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", inc, str(src), "-o", str(exe),
                            "-L", libdir, "-l:libnsfrb.so", f"-Wl,-rpath,{libdir}"])
     assert exe.exists()
+    import torch
+    if torch.cuda.is_available():   # on the GPU box also run it: create, two rejected calls, destroy -> exit code 0
+        assert subprocess.run([str(exe)]).returncode == 0
