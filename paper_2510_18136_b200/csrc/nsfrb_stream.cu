@@ -89,6 +89,26 @@ bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamC
     gpc = std::max(1, std::min(gpc, ngroups));
     seg = std::max(1, std::min(seg, 8));
     tt = std::max(1, std::min(tt, 8));
+    if (!(variant && *variant)) {
+        // register estimate of the default shape: raw rows (nchan*TT) + carried halo (sum over channels of the delay
+        // spread within a group of kk trials) + accumulators and state; above the 3-CTAs-per-SM budget use 2 CTAs
+        int carry = 0;
+        for (int g0 = 0; g0 < pl->nuniq; g0 += kk) {
+            int s = 0;
+            const int g1 = std::min(g0 + kk, pl->nuniq) - 1;
+            for (int ch = 0; ch < pl->nchan; ++ch) {
+                int lo = 1 << 30, hi = -(1 << 30);
+                for (int u = g0; u <= g1; ++u) {
+                    const int e = pl->dmax_u[g1] - pl->delays_u[(size_t)u * pl->nchan + ch];
+                    lo = std::min(lo, e);
+                    hi = std::max(hi, e);
+                }
+                s += hi - lo;
+            }
+            carry = std::max(carry, s);
+        }
+        if (pl->nchan * tt + carry + kk * (tt + 4) + 36 > 165) minb = std::min(minb, 2);
+    }
     c.KK = kk; c.GPC = gpc; c.SEG = seg; c.TT = tt; c.PFD = std::max(0, std::min(pfd, 24 / tt)); // the ring's guard rows cover 24 rows of look-ahead
     c.NSUPER = (ngroups + gpc - 1) / gpc;
     // ends per pass: the whole first chunk if it fits one CTA's shared memory, else as many as fit (more passes)

@@ -94,6 +94,12 @@ def config(name: str) -> Workload:
         return Workload("c5", 128, 128, 64, 8192, subband_centres(64), np.linspace(0.0, 5000.0, 256),
                         log_widths(32), 6.0, seed=5, n_pulses=100, s0_range=(6.0, 100.0),
                         note="DM/width stress; RFI-like spikes in channels 13 and 41")
+    if name == "paper":
+        # the grid the paper itself runs in real time: 301x301 px, 16 sub-bands, 16 DM trials
+        # 171-4000 pc/cm^3, log2 widths 1-16 samples, 25-sample chunks, 8.5 sigma; the ring length is ours (as C2)
+        return Workload("paper", 301, 301, 16, 1536, subband_centres(16), np.linspace(171.0, 4000.0, 16),
+                        np.asarray([1, 2, 4, 8, 16], dtype=np.int32), 8.5, seed=12, streaming=True, chunk_nt=25,
+                        s0_range=(8.0, 40.0), note="the paper's own real-time grid: 16 DM x 5 log2 widths, 301x301 px")
     raise ValueError(f"unknown config {name!r}")
 
 
