@@ -381,12 +381,12 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
         w.load_new(cur, r_begin);
         int rb = r_begin;
         int plain_until = r_begin; // exclusive
-        while (rb < r_end) {
+        // classify the tile at rb: does it store ends or meet a start range?  (also keeps the Qe barrier protocol)
+        auto classify = [&]() -> bool {
             if (seg == 0 && !synced && rb >= qe_end) { // every Qe of this pass is written
                 bar_named(1, kThreads);
                 synced = true;
             }
-            const bool masked = rb < 0 || rb + TT > r_fast_end;
             bool cells = rb >= plain_until; // tiles below plain_until are known to hold no end and no start
             if (cells) {
                 cells = rb < qe_end;
@@ -407,8 +407,25 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     synced = true;
                 }
             }
-            if (masked) w.template tile<true>(cur, rb, rb + TT < r_end, pf, true);
-            else w.template tile<false>(cur, rb, rb + TT < r_end, pf, cells);
+            return cells;
+        };
+        // three loops, so that the hot one holds a single tile body: masked lead-in (rb < 0), unmasked run, masked tail
+        while (rb < r_end && rb < 0) {
+            classify();
+            w.template tile<true>(cur, rb, rb + TT < r_end, pf, true);
+            rb += TT;
+        }
+        {
+            const int fast_stop = r_end < r_fast_end - TT + 1 ? r_end : r_fast_end - TT + 1; // rb < fast_stop <=> tile fully valid
+            while (rb < fast_stop) {
+                const bool cells = classify();
+                w.template tile<false>(cur, rb, rb + TT < r_end, pf, cells);
+                rb += TT;
+            }
+        }
+        while (rb < r_end) {
+            classify();
+            w.template tile<true>(cur, rb, rb + TT < r_end, pf, true);
             rb += TT;
         }
     }
