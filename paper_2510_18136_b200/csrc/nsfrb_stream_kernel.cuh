@@ -250,13 +250,10 @@ template <int G> struct Worker {
             }
         });
         // carry the halo: next tile's element m is this tile's element m + TT
-        {
-            float nc[T::CARRY];
-            sfor<0, NCHAN>([&](auto c) {
-                sfor<0, T::span(V(c))>([&](auto m) { nc[T::coff(V(c)) + V(m)] = Wn(c, IC<V(m) + TT>{}); });
-            });
-            sfor<0, T::CARRY>([&](auto i) { carry[V(i)] = nc[V(i)]; });
-        }
+        // (in place, ascending m: element m + TT is read before it is overwritten)
+        sfor<0, NCHAN>([&](auto c) {
+            sfor<0, T::span(V(c))>([&](auto m) { carry[T::coff(V(c)) + V(m)] = Wn(c, IC<V(m) + TT>{}); });
+        });
         if (more) load_new(cur, rb + TT); // rows of the next tile; their latency overlaps what follows
         if (PFD > 0 && pf) prefetch_l2(rb + PFD * TT);
         // a1, a3, a4: centred sample, suffix sum (left in Dv), sum of squares
