@@ -272,3 +272,52 @@ class ChunkSource:
                     out[c, a - a0:b - a0, pu.pixel] += pu.amp
         self.n = a1
         return out
+
+
+# ---- inputs of the post-search candidate selection (nsfrb_psf_mask / nsfrb_cluster) -------------------
+
+def synthetic_psf(size: int = 301, seed: int = 0, n_ant: int = 24) -> np.ndarray:
+    """A simulated dirty beam [size][size] float32, peak 1 at [size//2][size//2] (stands in for the paper's
+    "simulated PSF", L94; the DSA-110 one is not public).  Antennas on a mostly east-west line with a few
+    north-south outriggers (L46: the array is east-west dominated), one frequency: the beam is the mean over
+    baselines of cos(2 pi (u x + v y)), so it has a narrow main lobe, a north-south elongation and sidelobes."""
+    rng = np.random.default_rng(1000 + seed)
+    ew = np.sort(rng.uniform(-1.0, 1.0, n_ant))
+    ns = np.where(rng.random(n_ant) < 0.25, rng.uniform(-0.5, 0.5, n_ant), rng.normal(0.0, 0.01, n_ant))
+    i, j = np.triu_indices(n_ant, 1)
+    u = (ew[i] - ew[j]) * 0.12                     # cycles per pixel at the longest baseline ~ 0.24
+    v = (ns[i] - ns[j]) * 0.12
+    r = np.arange(size) - size // 2
+    px = np.exp(2j * np.pi * np.outer(u, r))       # [nbl][size]
+    py = np.exp(2j * np.pi * np.outer(v, r))
+    beam = np.real(np.einsum("by,bx->yx", py, px)) / u.size
+    return np.ascontiguousarray(beam, dtype=np.float32)
+
+
+def synthetic_snr_map(nx: int, ny: int, psf: np.ndarray, seed: int = 0, *, peak: float = 25.0, n_side: int = 6,
+                      n_spurious: int = 3, background: float = 4.5):
+    """A per-pixel peak-S/N map [ny][nx] float32 shaped like one with a bright source: noise-only pixels around
+    `background` (the maximum of many trials), one source of S/N `peak`, `n_side` copies at the strongest PSF
+    sidelobe offsets scaled by the PSF there, and `n_spurious` unrelated threshold crossings.  Returns
+    (map, (x0, y0))."""
+    rng = np.random.default_rng(2000 + seed)
+    m = (background + 0.45 * rng.gumbel(size=(ny, nx))).astype(np.float32)
+    x0, y0 = int(rng.integers(nx // 4, 3 * nx // 4)), int(rng.integers(ny // 4, 3 * ny // 4))
+    mh, mw = psf.shape
+    side = psf.astype(np.float64).copy()
+    cy, cx = mh // 2, mw // 2
+    side[max(0, cy - 3):cy + 4, max(0, cx - 3):cx + 4] = -np.inf      # not the main lobe itself
+    placed = 0
+    for flat in np.argsort(-side, axis=None):
+        if placed == n_side:
+            break
+        dy, dx = int(flat // mw) - cy, int(flat % mw) - cx
+        x, y = x0 + dx, y0 + dy
+        if 0 <= x < nx and 0 <= y < ny:
+            m[y, x] = np.float32(peak * float(psf[cy + dy, cx + dx]) + rng.normal(0.0, 0.5))
+            side[max(0, cy + dy - 2):cy + dy + 3, max(0, cx + dx - 2):cx + dx + 3] = -np.inf
+            placed += 1
+    m[y0, x0] = np.float32(peak)
+    for _ in range(n_spurious):
+        m[int(rng.integers(ny)), int(rng.integers(nx))] = np.float32(rng.uniform(7.0, 12.0))
+    return m, (x0, y0)
