@@ -460,6 +460,47 @@ def run_bin_arm(args):
                                    "kernel": "k_bin", "algorithmic_bytes": nbytes}}))
 
 
+def run_cluster_arm(args):
+    """--op cluster: NEXT 3's candidate selection (top-10 + PSF-mask clustering, one launch of k_cluster) on a
+    map of the workload's image size.  Algorithmic bytes = the S/N map read once (the ten selection rounds re-read
+    each CTA's 8 KB slice from L1/L2); at these sizes the launch is latency-bound, which the fraction shows."""
+    from paper_2510_18136_b200 import nsfrb
+    torch.cuda.set_device(0)
+    hbm_peak, peak_src, _ = measured_peaks()
+    wl = W.config(args.workload)
+    psf = W.synthetic_psf(301, 0)
+    m, _ = W.synthetic_snr_map(wl.nx, wl.ny, psf, 0)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    with nsfrb.Plan(wl.nx, wl.ny, 2, 64, [1.3, 1.5], W.TSAMP_S, [0.0], [1], wl.threshold) as plan:
+        dm = torch.from_numpy(m.ravel().copy()).cuda()
+        arg = torch.zeros((3, wl.npix), dtype=torch.int32, device="cuda")
+        dpsf = torch.from_numpy(psf).cuda()
+        dmask, _ = nsfrb.psf_mask(dpsf, 90.0)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for i in range(args.warmup + args.steps):
+            flush.zero_()                                  # L2 flush between iterations
+            j = i - args.warmup
+            if j >= 0:
+                ev[j][0].record()
+            res = plan.cluster(dm, arg, dpsf, dmask, 10)
+            if j >= 0:
+                ev[j][1].record()
+        torch.cuda.synchronize()
+        ms = float(np.mean([a.elapsed_time(b) for a, b in ev]))
+        got = res.to_host()
+    nbytes = wl.npix * 4
+    print(json.dumps({"metric": "maps/s (top-10 + PSF clustering, NEXT 3)", "value": 1e3 / ms, "unit": "maps/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+                      "dtype": "f32 keys, f64 means", "data": "synthetic",
+                      "config": {"workload": f"{wl.nx}x{wl.ny} S/N map, 301x301 PSF, top 10", "l2": "flushed between steps",
+                                 "n_found": len(got["pixels"]), "best_pixel": got["pixels"][got["best"]] if got["pixels"] else -1},
+                      "gpu_launches": args.steps,
+                      "roofline": {"bound": "hbm", "achieved": nbytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                                   "frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": None, "peak_source": peak_src,
+                                   "kernel": "k_cluster", "algorithmic_bytes": nbytes,
+                                   "note": "latency-bound: one launch, three dependent phases"}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -470,7 +511,8 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cubes", action="store_true", help="c2: also write the S/N and TOA cubes every push (NEXT 3)")
-    ap.add_argument("--op", default="search", choices=["search", "bin"], help="bin: time the binning kernel (NEXT 2)")
+    ap.add_argument("--op", default="search", choices=["search", "bin", "cluster"],
+                    help="bin: time the binning kernel (NEXT 2); cluster: top-10 + PSF clustering (NEXT 3)")
     ap.add_argument("--bin-factor", type=int, default=5)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
@@ -478,6 +520,9 @@ def main():
     if args.op == "bin" and args.impl == "cuda":
         if rank == 0:
             run_bin_arm(args)
+    elif args.op == "cluster" and args.impl == "cuda":
+        if rank == 0:
+            run_cluster_arm(args)
     elif args.impl == "reference":
         run_reference_arm(args, rank, world)
     else:

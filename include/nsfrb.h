@@ -181,6 +181,44 @@ int nsfrb_plan_get_kernel_ms(nsfrb_plan *plan, float out[4]);
 int nsfrb_bin_time(const float *cube, int nchan, int nt, int64_t npix, int factor, float *out, void *stream);
 
 /*
+ * Post-search candidate selection (readings R25-R28 in DESIGN.md).
+ *
+ * nsfrb_psf_mask: "the PSF is thresholded at the 90th percentile to make a binary mask".  The percentile value is
+ * v[lo] + (r - lo)*(v[lo+1] - v[lo]) with v = the PSF elements in ascending order, r = percentile/100*(mh*mw - 1),
+ * lo = floor(r), evaluated in float64; mask[i] = 1 where (double)psf[i] > value, else 0.
+ *   psf    device, [mh][mw] float32, finite values, read only
+ *   mask   device, [mh][mw] uint8, written
+ *   value  device, one float64, written (may be NULL)
+ * Asynchronous on `stream`; one launch.  NSFRB_EINVAL for null pointers, non-positive sizes, a percentile outside
+ * [0, 100] or more than 2^31-1 elements.
+ *
+ * nsfrb_cluster: "Standard post-processing is limited to the 10 highest S/N candidates ... [the mask] is centered
+ * on each candidate in turn.  This candidate is treated as the central PSF lobe, and any other candidates within the
+ * binary mask are identified as possible sidelobes.  The weighted mean S/N is computed over the central and sidelobe
+ * candidate S/Ns.  After repeating with each candidate, the maximum S/N is identified and its central lobe
+ * candidate's width, DM, position, and TOA are taken as the final, most-likely candidate."
+ *   Candidates: the pixels with snr_map > the plan's threshold (strict); the `topn` highest, equal S/N -> smaller
+ *   pixel index; n_found <= topn of them exist.  For centre i (rank order, best first) a candidate j at offset
+ *   (dx, dy) = (x_j - x_i, y_j - y_i) is a member if j == i, or if (mh/2 + dy, mw/2 + dx) lies inside the PSF array
+ *   and the mask is set there; its weight is the PSF value there (psf[mh/2][mw/2] for the centre).
+ *   wsnr[i] = sum_j w_j*snr_j / sum_j w_j over the members in rank order, float64, each operation rounded once.
+ *   best = the i with the largest wsnr (equal -> smaller i), -1 if n_found == 0.
+ *   snr_map  device, [ny][nx] float32, and  argmax  device, [3][npix] int32: outputs of nsfrb_search /
+ *            nsfrb_stream_push of this plan (or anything of that layout); read only
+ *   psf, mask  device, [mh][mw] float32 / uint8 (as written by nsfrb_psf_mask); psf[mh/2][mw/2] must be > 0
+ *   topn     1..32
+ *   top      device, [topn] nsfrb_cand: the candidates in rank order; entries >= n_found are (-1,-1,-1,-1,0)
+ *   wsnr     device, [topn] float64;  members  device, [topn] int32 (member counts; 0 beyond n_found)
+ *   result   device, [2] int32: n_found, best
+ * Asynchronous on `stream`; one launch; the first call allocates a small workspace in the plan.  Calls on one plan
+ * must be stream-ordered (as for nsfrb_search).  NSFRB_EINVAL for null arguments or sizes out of range.
+ */
+int nsfrb_psf_mask(const float *psf, int mh, int mw, double percentile, uint8_t *mask, double *value, void *stream);
+int nsfrb_cluster(nsfrb_plan *plan, const float *snr_map, const int32_t *argmax, const float *psf,
+                  const uint8_t *mask, int mh, int mw, int topn, nsfrb_cand *top, double *wsnr, int32_t *members,
+                  int32_t *result, void *stream);
+
+/*
  * Harness access to the plan-specialised real-time kernel: for the plan the first ten
  * arguments describe (as nsfrb_plan_create) and a first chunk of chunk_nt samples, writes either the CUDA
  * source the library compiles at the first nsfrb_stream_push (want_cubin = 0) or its sm_100a cubin

@@ -8,7 +8,9 @@ weighted mean S/N is computed over the central and sidelobe candidate S/Ns.  Aft
 the maximum S/N is identified and its central lobe candidate's width, DM, position, and TOA are taken as the final,
 most-likely candidate."
 
-Plain numpy / Python loops in float64, written in the order of that passage.  Readings (R25..R28):
+Plain numpy / Python loops in float64, written in the order of that passage.  The weights of the weighted mean
+are a reading (R28): PARITY UNPINNED to the paper for them (no worked example is printed); everything else is pinned
+in tests/test_cluster_pins.py.  Readings (R25..R28):
   R25  percentile = linear interpolation between order statistics at rank q/100*(n-1); mask = psf > that value.
   R26  candidates = per-pixel peaks with snr > threshold (O7, strict); the N highest, equal S/N -> smaller pixel.
   R27  the mask is centred by putting PSF element [mh//2][mw//2] on the central candidate; a candidate outside the

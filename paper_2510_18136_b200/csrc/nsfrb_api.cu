@@ -48,6 +48,7 @@ void nsfrb::free_plan(nsfrb_plan *p)
     cudaFree(p->d_dd_tab); cudaFree(p->d_dd_off);
     cudaFree(p->d_widths); cudaFree(p->d_j_of_used); cudaFree(p->d_partials); cudaFree(p->d_in); cudaFree(p->d_snr);
     cudaFree(p->d_arg); cudaFree(p->d_cands); cudaFree(p->d_ncands);
+    cudaFree(p->d_cluster_ws);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     stream_free(p);
     search3_free(p);
@@ -565,6 +566,46 @@ int nsfrb_bin_time(const float *cube, int nchan, int nt, int64_t npix, int facto
     if (nchan > 65535) return fail(NSFRB_EINVAL, "too many channels");
     if (cube == out) return fail(NSFRB_EINVAL, "in-place binning is not supported");
     CU(launch_bin(cube, out, nchan, nt, (long long)npix, factor, static_cast<cudaStream_t>(stream)), "k_bin launch");
+    return NSFRB_OK;
+}
+
+int nsfrb_psf_mask(const float *psf, int mh, int mw, double percentile, uint8_t *mask, double *value, void *stream)
+{
+    if (!psf || !mask) return fail(NSFRB_EINVAL, "null pointer");
+    if (mh < 1 || mw < 1) return fail(NSFRB_EINVAL, "non-positive PSF size");
+    if (!(percentile >= 0.0 && percentile <= 100.0)) return fail(NSFRB_EINVAL, "percentile outside [0, 100]");
+    const long long n = (long long)mh * mw;
+    if (n > 0x7fffffffLL) return fail(NSFRB_EINVAL, "PSF too large");
+    // reading R25: rank q/100*(n-1), linear interpolation between the neighbouring order statistics
+    const double r = percentile / 100.0 * (double)(n - 1);
+    long long lo = (long long)std::floor(r);
+    lo = std::min(std::max(lo, 0LL), n - 1);
+    CU(launch_psf_mask(psf, n, lo, r - (double)lo, mask, value, static_cast<cudaStream_t>(stream)), "k_psf_mask launch");
+    return NSFRB_OK;
+}
+
+int nsfrb_cluster(nsfrb_plan *pl, const float *snr_map, const int32_t *argmax, const float *psf, const uint8_t *mask,
+                  int mh, int mw, int topn, nsfrb_cand *top, double *wsnr, int32_t *members, int32_t *result,
+                  void *stream)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (!snr_map || !argmax || !psf || !mask || !top || !wsnr || !members || !result)
+        return fail(NSFRB_EINVAL, "null pointer");
+    if (mh < 1 || mw < 1) return fail(NSFRB_EINVAL, "non-positive PSF size");
+    if (topn < 1 || topn > cluster_max_top()) return fail(NSFRB_EINVAL, "topn outside 1..32");
+    CU(cudaSetDevice(pl->device), "set device");
+    if (!pl->d_cluster_ws) {
+        const size_t bytes = 256 + (size_t)cluster_grid(pl->npix) * cluster_max_top() * sizeof(unsigned long long);
+        CU(cudaMalloc(&pl->d_cluster_ws, bytes), "cluster workspace");
+        CU(cudaMemset(pl->d_cluster_ws, 0, 256), "cluster workspace");
+        pl->workspace_bytes += bytes;
+    }
+    char *ws = static_cast<char *>(pl->d_cluster_ws);
+    CU(launch_cluster(snr_map, argmax, pl->npix, pl->nx, pl->threshold, psf, mask, mh, mw, topn, ws + 256,
+                      reinterpret_cast<unsigned int *>(ws), top, wsnr, members, result,
+                      static_cast<cudaStream_t>(stream)),
+       "k_cluster launch");
+    pl->last_launches = 1;
     return NSFRB_OK;
 }
 

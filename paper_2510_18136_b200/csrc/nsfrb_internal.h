@@ -121,6 +121,8 @@ struct nsfrb_plan {
     int32_t *cube_toa = nullptr;
     // offline path: plan-specialised k_search3 (nsfrb_search_kernel.cuh), compiled at the first nsfrb_search
     nsfrb::Search3State *search3 = nullptr;
+    // candidate selection (nsfrb_cluster.cu): per-CTA key lists + ticket, allocated at the first nsfrb_cluster
+    void *d_cluster_ws = nullptr;
 };
 
 namespace nsfrb {
@@ -160,6 +162,15 @@ cudaError_t launch_finalize(const FinalParams &p, size_t smem_bytes, cudaStream_
 cudaError_t launch_compact(const float *snr_map, const int32_t *argmax, int npix, float threshold,
                            nsfrb_cand *cands, uint32_t cap, uint32_t *ncands, cudaStream_t st);
 cudaError_t launch_bin(const float *in, float *out, int nchan, int nt, long long npix, int factor, cudaStream_t st);
+cudaError_t launch_psf_mask(const float *psf, long long n, long long lo, double frac, uint8_t *mask, double *value,
+                            cudaStream_t st);
+int cluster_max_top();
+int cluster_grid(int npix);
+// ws: cluster_grid(npix) * topn 64-bit keys; ticket: one zero-initialised counter (the kernel leaves it at zero)
+cudaError_t launch_cluster(const float *snr_map, const int32_t *argmax, int npix, int nx, float threshold,
+                           const float *psf, const uint8_t *mask, int mh, int mw, int topn, void *ws,
+                           unsigned int *ticket, nsfrb_cand *top, double *wsnr, int32_t *members, int32_t *result,
+                           cudaStream_t st);
 size_t search_smem_bytes(int nchan, int RS, int H, int tab_cap);
 size_t final_smem_bytes(int nt);
 

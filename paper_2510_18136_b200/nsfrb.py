@@ -44,7 +44,8 @@ assert CAND_DTYPE.itemsize == ctypes.sizeof(nsfrb_cand) == 20
 EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stream_reset", "nsfrb_search_host",
            "nsfrb_stream_push_host", "nsfrb_plan_destroy", "nsfrb_plan_get_delays", "nsfrb_plan_get_info",
            "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
-           "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes")
+           "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes",
+           "nsfrb_psf_mask", "nsfrb_cluster")
 
 _lib = None
 
@@ -96,6 +97,10 @@ def lib() -> ctypes.CDLL:
                                               ctypes.POINTER(ctypes.c_size_t)]
         L.nsfrb_bin_time.restype = ctypes.c_int
         L.nsfrb_bin_time.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_int, vp, vp]
+        L.nsfrb_psf_mask.restype = ctypes.c_int
+        L.nsfrb_psf_mask.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, vp, vp, vp]
+        L.nsfrb_cluster.restype = ctypes.c_int
+        L.nsfrb_cluster.argtypes = [vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp]
         L.nsfrb_last_error.restype = ctypes.c_char_p
         L.nsfrb_version.restype = ctypes.c_char_p
         _lib = L
@@ -172,6 +177,33 @@ def bin_time(cube: torch.Tensor, factor: int, out: torch.Tensor | None = None, s
     s = torch.cuda.current_stream() if stream is None else stream
     _check(lib().nsfrb_bin_time(cube.data_ptr(), nchan, nt, npix, int(factor), out.data_ptr(), int(s.cuda_stream)))
     return out
+
+
+def psf_mask(psf: torch.Tensor, percentile: float = 90.0, stream=None):
+    """nsfrb_psf_mask on a device PSF [mh][mw] float32 -> (mask uint8 [mh][mw], value float64 [1]) (asynchronous)."""
+    if not psf.is_cuda or psf.dtype != torch.float32 or not psf.is_contiguous() or psf.dim() != 2:
+        raise ValueError("expected a contiguous float32 CUDA tensor [mh][mw]")
+    mask = torch.empty(psf.shape, dtype=torch.uint8, device=psf.device)
+    value = torch.empty(1, dtype=torch.float64, device=psf.device)
+    s = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().nsfrb_psf_mask(psf.data_ptr(), psf.shape[0], psf.shape[1], float(percentile), mask.data_ptr(),
+                                value.data_ptr(), int(s.cuda_stream)))
+    return mask, value
+
+
+@dataclass
+class ClusterResult:
+    top: torch.Tensor       # [topn*20] uint8 (raw nsfrb_cand records, rank order)
+    wsnr: torch.Tensor      # [topn] float64
+    members: torch.Tensor   # [topn] int32
+    result: torch.Tensor    # [2] int32: n_found, best
+
+    def to_host(self) -> dict:
+        """Synchronises; the found candidates only."""
+        n, best = (int(v) for v in self.result.cpu())
+        cands = self.top.cpu().numpy().view(CAND_DTYPE)[:n].copy()
+        return dict(cands=cands, pixels=[int(p) for p in cands["pixel"]], wsnr=self.wsnr.cpu().numpy()[:n].tolist(),
+                    members=self.members.cpu().numpy()[:n].tolist(), best=best)
 
 
 class Plan:
@@ -271,6 +303,29 @@ class Plan:
 
     def stream_reset(self):
         _check(lib().nsfrb_stream_reset(self._h))
+
+    def cluster(self, snr_map: torch.Tensor, argmax: torch.Tensor, psf: torch.Tensor, mask: torch.Tensor, topn: int = 10,
+                stream=None) -> ClusterResult:
+        """nsfrb_cluster: the topn best candidates of (snr_map, argmax) and their PSF-mask weighted mean S/N."""
+        if not (snr_map.is_cuda and snr_map.dtype == torch.float32 and snr_map.is_contiguous()
+                and snr_map.numel() == self.npix):
+            raise ValueError("snr_map must be a contiguous float32 CUDA tensor of npix elements")
+        if not (argmax.is_cuda and argmax.dtype == torch.int32 and argmax.is_contiguous()
+                and tuple(argmax.shape) == (3, self.npix)):
+            raise ValueError("argmax must be a contiguous int32 CUDA tensor [3][npix]")
+        if not (psf.is_cuda and psf.dtype == torch.float32 and psf.is_contiguous() and psf.dim() == 2
+                and mask.is_cuda and mask.dtype == torch.uint8 and mask.is_contiguous() and mask.shape == psf.shape):
+            raise ValueError("psf / mask must be contiguous CUDA tensors [mh][mw] (float32 / uint8)")
+        n = max(int(topn), 1)
+        dev = self.device
+        res = ClusterResult(torch.empty(n * CAND_DTYPE.itemsize, dtype=torch.uint8, device=dev),
+                            torch.empty(n, dtype=torch.float64, device=dev),
+                            torch.empty(n, dtype=torch.int32, device=dev), torch.empty(2, dtype=torch.int32, device=dev))
+        s = torch.cuda.current_stream() if stream is None else stream
+        _check(lib().nsfrb_cluster(self._h, snr_map.data_ptr(), argmax.data_ptr(), psf.data_ptr(), mask.data_ptr(),
+                                   psf.shape[0], psf.shape[1], int(topn), res.top.data_ptr(), res.wsnr.data_ptr(),
+                                   res.members.data_ptr(), res.result.data_ptr(), int(s.cuda_stream)))
+        return res
 
     # -- host-buffer variants (H2D, search, D2H, synchronise) used for the end-to-end number
     def _host_out(self):

@@ -76,6 +76,14 @@ def test_null_arguments_and_destroy_null():
     assert L.nsfrb_stream_push(None, None, 1, None, None, None, None, 0, None) == nsfrb.NSFRB_EINVAL
     assert L.nsfrb_plan_get_delays(None, None) == nsfrb.NSFRB_EINVAL
     assert L.nsfrb_plan_last_launches(None) == 0
+    assert L.nsfrb_psf_mask(None, 3, 3, 90.0, None, None, None) == nsfrb.NSFRB_EINVAL
+    assert L.nsfrb_cluster(None, None, None, None, None, 3, 3, 10, None, None, None, None, None) == nsfrb.NSFRB_EINVAL
+    buf = (ctypes.c_float * 9)()
+    m = (ctypes.c_uint8 * 9)()      # host memory: the argument checks come before any launch
+    addr = ctypes.addressof
+    assert L.nsfrb_psf_mask(addr(buf), 0, 3, 90.0, addr(m), None, None) == nsfrb.NSFRB_EINVAL
+    assert L.nsfrb_psf_mask(addr(buf), 3, 3, 101.0, addr(m), None, None) == nsfrb.NSFRB_EINVAL
+    assert L.nsfrb_psf_mask(addr(buf), 3, 3, float("nan"), addr(m), None, None) == nsfrb.NSFRB_EINVAL
 
 
 def test_no_cpu_fallback_without_gpu():
