@@ -161,6 +161,20 @@ def bin_time(cube, factor: int) -> np.ndarray:
     return out
 
 
+def median_subtract(cube):
+    """NEXT 1 (first part) / reading R29: "Data is first median subtracted in each pixel".  For every
+    (channel, pixel) series of the nt samples: median = the middle element of the sorted series (the mean of the two
+    middle ones for even nt, in float64, rounded once to float32); out = cube - median in float32.
+    Returns (out [nchan][nt][npix] float32, median [nchan][npix] float32)."""
+    a = np.ascontiguousarray(cube, dtype=np.float32)
+    nchan, nt, npix = a.shape
+    if nt < 1:
+        raise ValueError("nt must be >= 1")
+    s = np.sort(a.astype(np.float64), axis=1)
+    med = (0.5 * (s[:, (nt - 1) // 2, :] + s[:, nt // 2, :])).astype(np.float32)
+    return a - med[:, None, :], med
+
+
 class StreamOracle:
     """S1..S6: the streaming definition, by re-running the offline definition on the
     chronological ring contents after every push (no incremental state)."""

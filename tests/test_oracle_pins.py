@@ -456,3 +456,56 @@ def test_per_trial_width_maxima_are_consistent():
     D0 = cube.astype(np.float64).sum(axis=0)
     z = (D0 - D0.mean(axis=0)) / D0.std(axis=0)
     assert np.allclose(a.best[:, 0, 0], z.max(axis=0), rtol=0, atol=1e-12) and np.array_equal(a.best_t[:, 0, 0], z.argmax(axis=0))
+
+
+# ---- NEXT 1 (first part): per-(channel, pixel) median subtraction (reading R29) ------------------------
+
+@pytest.mark.parametrize("nt", [1, 2, 3, 24, 25, 64, 101])
+def test_median_matches_numpy_routine_and_rank_definition(nt):
+    rng = np.random.default_rng(nt)
+    a = rng.normal(size=(3, nt, 7)).astype(np.float32)
+    a[0, :, 0] = np.round(a[0, :, 0])                    # ties
+    out, med = oracle.median_subtract(a)
+    assert np.array_equal(med, np.median(a.astype(np.float64), axis=1).astype(np.float32))
+    assert np.array_equal(out, a - med[:, None, :]) and out.dtype == np.float32
+    # the definition by counting: at least half of the samples are <= m and at least half are >= m
+    for c in range(3):
+        for p in range(7):
+            x, m = a[c, :, p].astype(np.float64), float(med[c, p])
+            lo, hi = np.sort(x)[(nt - 1) // 2], np.sort(x)[nt // 2]
+            assert lo <= m <= hi or np.isclose(m, 0.5 * (lo + hi), rtol=1e-7, atol=0)
+            assert 2 * np.sum(x <= hi) >= nt and 2 * np.sum(x >= lo) >= nt
+
+
+def test_median_closed_forms_and_invariances():
+    t = np.arange(25, dtype=np.float32)
+    a = np.stack([t, t[::-1], np.full(25, 3.5, np.float32)])[:, :, None]          # [3][25][1]
+    out, med = oracle.median_subtract(a)
+    assert med.ravel().tolist() == [12.0, 12.0, 3.5] and np.array_equal(out[0, :, 0], t - 12) and not out[2].any()
+    out, med = oracle.median_subtract(np.asarray([1.0, 4.0], np.float32).reshape(1, 2, 1))
+    assert med.ravel().tolist() == [2.5] and out.ravel().tolist() == [-1.5, 1.5]
+    out, med = oracle.median_subtract(np.asarray([7.0], np.float32).reshape(1, 1, 1))
+    assert med.ravel().tolist() == [7.0] and out.ravel().tolist() == [0.0]
+    # one outlier does not move it (the reason the paper uses a median, L75 / L130)
+    x = np.asarray([0, 1, 2, 3, 1e6], np.float32).reshape(1, 5, 1)
+    assert oracle.median_subtract(x)[1].ravel().tolist() == [2.0]
+    # permutation of the samples: same median; integer shift: exact equivariance; already subtracted: median 0
+    rng = np.random.default_rng(0)
+    a = rng.integers(-50, 50, size=(2, 40, 5)).astype(np.float32)
+    _, m0 = oracle.median_subtract(a)
+    _, m1 = oracle.median_subtract(a[:, rng.permutation(40), :])
+    o2, m2 = oracle.median_subtract(a + 17.0)
+    assert np.array_equal(m0, m1) and np.array_equal(m2, m0 + 17.0)
+    assert not oracle.median_subtract(o2)[1].any()
+
+
+def test_median_subtraction_cancels_in_the_search():
+    """Reading R6/R29: the per-(pixel, DM) mean of O3 removes any per-channel constant, so subtracting the
+    channel medians first changes no S/N beyond rounding -- which is why the median is NEXT 1 and not on the path."""
+    wl = W.config("c1")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    cube = W.make_cube(wl).numpy()[:, :, :40]
+    r0 = oracle.search(cube, d, wl.width_list)
+    r1 = oracle.search(oracle.median_subtract(cube)[0], d, wl.width_list)
+    assert np.allclose(r0.snr, r1.snr, rtol=0, atol=2e-5)
+    assert (r0.argmax == r1.argmax).all(axis=1).mean() > 0.95
