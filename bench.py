@@ -460,6 +460,45 @@ def run_bin_arm(args):
                                    "kernel": "k_bin", "algorithmic_bytes": nbytes}}))
 
 
+def run_median_arm(args):
+    """--op median: NEXT 1's per-(channel, pixel) median subtraction.  HBM-bound by contract: algorithmic bytes =
+    cube read once + written once (+ the medians).  Default: 40 chunk-shaped cubes of C2 (16 x 25 x 65 536, the
+    paper's 3.35 s chunk) back to back so the inputs exceed L2; --workload c3: the 2048-sample offline cube."""
+    from paper_2510_18136_b200 import nsfrb
+    torch.cuda.set_device(0)
+    hbm_peak, peak_src, _ = measured_peaks()
+    wl = W.config(args.workload)
+    g = torch.Generator(device="cuda").manual_seed(wl.seed)
+    if wl.name == "c2":
+        nt, ncubes = wl.chunk_nt, 40
+    else:
+        nt, ncubes = wl.nt, 1
+    cubes = [torch.randn((wl.nchan, nt, wl.npix), device="cuda", generator=g) for _ in range(ncubes)]
+    outs = [torch.empty_like(c) for c in cubes[:2]]
+    meds = torch.empty((wl.nchan, wl.npix), device="cuda")
+    L = nsfrb.lib()
+    s = int(torch.cuda.current_stream().cuda_stream)
+
+    def step():
+        for i, c in enumerate(cubes):
+            rc = L.nsfrb_median_subtract(c.data_ptr(), wl.nchan, nt, wl.npix, outs[i & 1].data_ptr(), meds.data_ptr(), s)
+            assert rc == 0, nsfrb.last_error()
+
+    per_step = time_steps(step, args.steps, args.warmup)
+    ms = float(np.mean(per_step)) / ncubes
+    nbytes = cubes[0].numel() * 8 + meds.numel() * 4
+    kern = "k_median_reg<32>" if nt <= 32 else "k_median_tile"
+    print(json.dumps({"metric": "GB/s (median subtraction, NEXT 1)", "value": nbytes / (ms * 1e-3) / 1e9, "unit": "GB/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+                      "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": f"{wl.name}: {wl.nchan} ch x {nt} samples x {wl.npix} pixels", "cubes_per_step": ncubes,
+                                 "l2": "inputs larger than L2"},
+                      "gpu_launches": args.steps * ncubes,
+                      "roofline": {"bound": "hbm", "achieved": nbytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                                   "frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": None, "peak_source": peak_src,
+                                   "kernel": kern, "algorithmic_bytes": nbytes}}))
+
+
 def run_cluster_arm(args):
     """--op cluster: NEXT 3's candidate selection (top-10 + PSF-mask clustering, one launch of k_cluster) on a
     map of the workload's image size.  Algorithmic bytes = the S/N map read once (the ten selection rounds re-read
@@ -511,8 +550,9 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cubes", action="store_true", help="c2: also write the S/N and TOA cubes every push (NEXT 3)")
-    ap.add_argument("--op", default="search", choices=["search", "bin", "cluster"],
-                    help="bin: time the binning kernel (NEXT 2); cluster: top-10 + PSF clustering (NEXT 3)")
+    ap.add_argument("--op", default="search", choices=["search", "bin", "cluster", "median"],
+                    help="bin: time the binning kernel (NEXT 2); cluster: top-10 + PSF clustering (NEXT 3); "
+                         "median: per-pixel median subtraction (NEXT 1)")
     ap.add_argument("--bin-factor", type=int, default=5)
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
@@ -520,6 +560,9 @@ def main():
     if args.op == "bin" and args.impl == "cuda":
         if rank == 0:
             run_bin_arm(args)
+    elif args.op == "median" and args.impl == "cuda":
+        if rank == 0:
+            run_median_arm(args)
     elif args.op == "cluster" and args.impl == "cuda":
         if rank == 0:
             run_cluster_arm(args)

@@ -181,6 +181,21 @@ int nsfrb_plan_get_kernel_ms(nsfrb_plan *plan, float out[4]);
 int nsfrb_bin_time(const float *cube, int nchan, int nt, int64_t npix, int factor, float *out, void *stream);
 
 /*
+ * Per-pixel median subtraction ("Data is first median subtracted in each pixel"; SURVEY.md 8(f) NEXT 1,
+ * first part; reading R29).  For every (channel c, pixel p): m = the median of cube[c][0..nt-1][p] -- the middle
+ * element of the sorted series, for even nt the mean of the two middle elements computed in float64 and rounded once
+ * to float32 -- and out[c][t][p] = cube[c][t][p] - m (float32).  Inputs must be finite (no NaN).  Under the path's
+ * per-(pixel, DM) mean subtraction (O3) this step changes no S/N beyond rounding; it is provided as the first stage
+ * of the paper's robust-baseline variant.
+ *   cube    device, [nchan][nt][npix] float32, read only unless out == cube
+ *   out     device, same shape; may be the same pointer as cube (in place), must not overlap it otherwise
+ *   median  device, [nchan][npix] float32, written (may be NULL)
+ * Asynchronous on `stream`; one launch.  NSFRB_EINVAL for null pointers, non-positive sizes, nchan > 65535 or
+ * nt > 43007 (the series of a tile must fit in shared memory).
+ */
+int nsfrb_median_subtract(const float *cube, int nchan, int nt, int64_t npix, float *out, float *median, void *stream);
+
+/*
  * Post-search candidate selection (readings R25-R28 in DESIGN.md).
  *
  * nsfrb_psf_mask: "the PSF is thresholded at the 90th percentile to make a binary mask".  The percentile value is

@@ -569,6 +569,18 @@ int nsfrb_bin_time(const float *cube, int nchan, int nt, int64_t npix, int facto
     return NSFRB_OK;
 }
 
+int nsfrb_median_subtract(const float *cube, int nchan, int nt, int64_t npix, float *out, float *median, void *stream)
+{
+    if (!cube || !out) return fail(NSFRB_EINVAL, "null pointer");
+    if (nchan < 1 || nt < 1 || npix < 1) return fail(NSFRB_EINVAL, "non-positive size");
+    if (nchan > 65535) return fail(NSFRB_EINVAL, "too many channels");
+    if (nt > median_max_nt()) return fail(NSFRB_EINVAL, "nt too large for the shared-memory tile (max 43007)");
+    if ((long long)nchan * npix > 0x7fffffffLL * 256) return fail(NSFRB_EINVAL, "too many series");
+    CU(launch_median(cube, out, median, nchan, nt, (long long)npix, static_cast<cudaStream_t>(stream)),
+       "k_median launch");
+    return NSFRB_OK;
+}
+
 int nsfrb_psf_mask(const float *psf, int mh, int mw, double percentile, uint8_t *mask, double *value, void *stream)
 {
     if (!psf || !mask) return fail(NSFRB_EINVAL, "null pointer");

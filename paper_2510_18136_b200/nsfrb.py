@@ -45,7 +45,7 @@ EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stre
            "nsfrb_stream_push_host", "nsfrb_plan_destroy", "nsfrb_plan_get_delays", "nsfrb_plan_get_info",
            "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
            "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes",
-           "nsfrb_psf_mask", "nsfrb_cluster")
+           "nsfrb_psf_mask", "nsfrb_cluster", "nsfrb_median_subtract")
 
 _lib = None
 
@@ -97,6 +97,8 @@ def lib() -> ctypes.CDLL:
                                               ctypes.POINTER(ctypes.c_size_t)]
         L.nsfrb_bin_time.restype = ctypes.c_int
         L.nsfrb_bin_time.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_int, vp, vp]
+        L.nsfrb_median_subtract.restype = ctypes.c_int
+        L.nsfrb_median_subtract.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, vp, vp, vp]
         L.nsfrb_psf_mask.restype = ctypes.c_int
         L.nsfrb_psf_mask.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, vp, vp, vp]
         L.nsfrb_cluster.restype = ctypes.c_int
@@ -177,6 +179,23 @@ def bin_time(cube: torch.Tensor, factor: int, out: torch.Tensor | None = None, s
     s = torch.cuda.current_stream() if stream is None else stream
     _check(lib().nsfrb_bin_time(cube.data_ptr(), nchan, nt, npix, int(factor), out.data_ptr(), int(s.cuda_stream)))
     return out
+
+
+def median_subtract(cube: torch.Tensor, out: torch.Tensor | None = None, want_median: bool = True, stream=None):
+    """nsfrb_median_subtract on a device cube [nchan][nt][npix] float32 -> (out, median [nchan][npix] or None);
+    out=cube works in place (asynchronous)."""
+    if not cube.is_cuda or cube.dtype != torch.float32 or not cube.is_contiguous() or cube.dim() != 3:
+        raise ValueError("expected a contiguous float32 CUDA tensor [nchan][nt][npix]")
+    nchan, nt, npix = cube.shape
+    if out is None:
+        out = torch.empty_like(cube)
+    elif out.shape != cube.shape or out.dtype != cube.dtype or not out.is_contiguous() or out.device != cube.device:
+        raise ValueError("out must match the cube")
+    med = torch.empty((nchan, npix), dtype=torch.float32, device=cube.device) if want_median else None
+    s = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().nsfrb_median_subtract(cube.data_ptr(), nchan, nt, npix, out.data_ptr(),
+                                       med.data_ptr() if med is not None else None, int(s.cuda_stream)))
+    return out, med
 
 
 def psf_mask(psf: torch.Tensor, percentile: float = 90.0, stream=None):

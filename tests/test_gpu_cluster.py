@@ -157,3 +157,63 @@ def test_cluster_after_stream_push():
         top2 = sorted(want["wsnr"])[-2:]
         if top2[1] - top2[0] > 2e-3:
             assert got["best"] == want["best"]
+
+
+# ---- NEXT 1 (first part): nsfrb_median_subtract vs oracle.median_subtract, exact ------------------------------------
+
+@pytest.mark.parametrize("nchan,nt,npix", [
+    (1, 1, 1), (2, 2, 33), (3, 3, 77), (2, 5, 300), (2, 8, 64), (1, 16, 1000), (2, 17, 129), (16, 25, 1024),
+    (2, 31, 95), (2, 32, 257), (2, 33, 257), (3, 64, 100), (2, 100, 77), (1, 257, 65), (2, 1000, 90), (2, 2048, 75),
+    (1, 2304, 40), (1, 4097, 21), (1, 16384, 7), (1, 30000, 3), (1, 43007, 2)])
+def test_median_subtract_matches_oracle(nchan, nt, npix):
+    nsfrb = _nsfrb()
+    rng = np.random.default_rng(nt * 131 + npix)
+    a = rng.normal(size=(nchan, nt, npix)).astype(np.float32)
+    a[0, :, 0] = np.round(3 * a[0, :, 0])                 # exact ties, zeros
+    if nt > 3:
+        a[0, 1, 0], a[0, 2, 0] = 0.0, -0.0
+    a[-1, :, -1] = -np.abs(a[-1, :, -1]) * 1e30            # large negative values: the key order of negative floats
+    want, wmed = oracle.median_subtract(a)
+    d = torch.from_numpy(a).cuda()
+    out, med = nsfrb.median_subtract(d)
+    assert np.array_equal(med.cpu().numpy(), wmed)
+    assert np.array_equal(out.cpu().numpy(), want)
+    assert np.array_equal(d.cpu().numpy(), a)              # the input is untouched
+    out2, none = nsfrb.median_subtract(d, out=d, want_median=False)      # in place, no median output
+    assert none is None and out2 is d and np.array_equal(d.cpu().numpy(), want)
+
+
+def test_median_subtract_every_register_length():
+    """nt = 1..32 each has its own compile-time comparator network: all of them, with ties."""
+    nsfrb = _nsfrb()
+    for nt in range(1, 33):
+        rng = np.random.default_rng(nt)
+        a = rng.normal(size=(2, nt, 300)).astype(np.float32)
+        a[1] = np.round(2 * a[1])
+        want, wmed = oracle.median_subtract(a)
+        out, med = nsfrb.median_subtract(torch.from_numpy(a).cuda())
+        assert np.array_equal(med.cpu().numpy(), wmed), nt
+        assert np.array_equal(out.cpu().numpy(), want), nt
+
+
+def test_median_subtract_rejects_bad_arguments():
+    nsfrb = _nsfrb()
+    L = nsfrb.lib()
+    d = torch.zeros((1, 4, 4), device="cuda")
+    assert L.nsfrb_median_subtract(d.data_ptr(), 1, 0, 4, d.data_ptr(), None, None) == nsfrb.NSFRB_EINVAL
+    assert L.nsfrb_median_subtract(d.data_ptr(), 1, 43008, 4, d.data_ptr(), None, None) == nsfrb.NSFRB_EINVAL
+    assert L.nsfrb_median_subtract(None, 1, 4, 4, d.data_ptr(), None, None) == nsfrb.NSFRB_EINVAL
+
+
+def test_median_then_search_is_the_same_search():
+    """R6/R29: the search of the median-subtracted cube equals the search of the cube within the parity tolerance."""
+    nsfrb = _nsfrb()
+    wl = W.config("c1")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    cube = W.make_cube(wl, "cuda")
+    W.inject(cube, W.injection_table(wl, d), d, extra_delays=oracle.delays(wl.freqs_GHz, wl.tsamp_s, [500.0])[0])
+    sub, _ = nsfrb.median_subtract(cube)
+    with nsfrb.Plan.for_workload(wl) as plan:
+        s1 = plan.search(sub).snr_map.cpu().numpy()
+    r = oracle.search(oracle.median_subtract(cube.cpu().numpy())[0], d, wl.width_list, nthreads=8)
+    assert np.all(np.abs(s1 - r.snr) <= 1e-4 + 1e-4 * np.abs(r.snr))
