@@ -9,6 +9,8 @@
 //                     element by one more pass (warp per series), subtraction on the way out.
 #include "nsfrb_internal.h"
 
+#include <cstdlib>
+
 namespace nsfrb {
 namespace {
 
@@ -132,9 +134,18 @@ __global__ void __launch_bounds__(kTileThreads) k_median_tile(const float *in, f
     const int np = (int)min((long long)P, npix - p0);
     const float *src = in + c * nt * npix + p0;
     const int total = nt * P;
-    for (int idx = tid; idx < total; idx += kTileThreads) {
-        const int t = idx / P, p = idx % P;
-        if (p < np) keys[p * stride + t] = ord_key(src[(long long)t * npix + p]);
+    // asynchronous 4-byte copies straight into the transposed tile: no register dependence, so a thread keeps all of
+    // its loads in flight (rows of P pixels are neither 16-byte aligned nor a multiple of 16 bytes in general)
+    {
+        const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(keys);
+        for (int idx = tid; idx < total; idx += kTileThreads) {
+            const int t = idx / P, p = idx % P;
+            if (p < np)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sbase + 4u * (uint32_t)(p * stride + t)),
+                             "l"(src + (long long)t * npix + p)
+                             : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
     }
     for (int i = tid; i < kHistWords; i += kTileThreads) hist[i] = 0;
     const int k1 = (nt - 1) >> 1, k2 = nt >> 1;
@@ -142,17 +153,31 @@ __global__ void __launch_bounds__(kTileThreads) k_median_tile(const float *in, f
         s_prefix[tid] = 0;
         s_k[tid] = k1;
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
     // ---- exact order statistic k1 of every series: 4 passes of 8 bits, all warps over all series
-    const int rows32 = (nt + 31) >> 5, items = np * rows32;
     for (int pass = 0; pass < 4; ++pass) {
         const int shift = 24 - 8 * pass;
-        for (int item = warp; item < items; item += NW) {
-            const int p = item / rows32, t = (item - p * rows32) * 32 + lane;
-            if (t < nt) {
-                const uint32_t key = keys[p * stride + t];
-                const bool match = pass == 0 || ((key ^ s_prefix[p]) >> (shift + 8)) == 0u;
-                if (match) atomicAdd(&hist[((p * S + (lane & (S - 1))) << 8) + ((key >> shift) & 255u)], 1u);
+        // P >= 16 (short series): a warp per series; P <= 8 (long series): the whole CTA walks one series at a time.
+        // Pass 0 also turns the float bits the copies delivered into order-preserving keys, in place.
+        const int pstep = P >= 16 ? NW : 1, tstep = P >= 16 ? 32 : kTileThreads;
+        for (int p = P >= 16 ? warp : 0; p < np; p += pstep) {
+            uint32_t *row = keys + p * stride;
+            uint32_t *hp = hist + ((p * S + (lane & (S - 1))) << 8);
+            const uint32_t prefix = s_prefix[p];
+            if (pass == 0) {
+#pragma unroll 4
+                for (int t = P >= 16 ? lane : tid; t < nt; t += tstep) {
+                    const uint32_t key = ord_key(__uint_as_float(row[t]));
+                    row[t] = key;
+                    atomicAdd(hp + (key >> 24), 1u);
+                }
+            } else {
+#pragma unroll 4
+                for (int t = P >= 16 ? lane : tid; t < nt; t += tstep) {
+                    const uint32_t key = row[t];
+                    if (((key ^ prefix) >> (shift + 8)) == 0u) atomicAdd(hp + ((key >> shift) & 255u), 1u);
+                }
             }
         }
         __syncthreads();
@@ -263,6 +288,7 @@ int median_tile_pixels(int nt)
 {
     const int stride = nt | 1;
     int p = 32;
+    if (const char *e = getenv("NSFRB_MEDIAN_P")) return atoi(e);
     while (p > 8 && (size_t)p * stride * 4 > (72 - 32) * 1024) p >>= 1;   // three CTAs per SM while rows stay >= 32 bytes
     while (p > 1 && (size_t)p * stride * 4 > (200 - 32) * 1024) p >>= 1;  // (32 KB of every CTA are the histograms)
     return p;
