@@ -149,6 +149,24 @@ int nsfrb_stream_push_host(nsfrb_plan *plan, const float *chunk_host, int chunk_
                            float *snr_map_host, int32_t *argmax_host,
                            nsfrb_cand *cands_host, uint32_t cand_capacity, uint32_t *ncands_host);
 
+/*
+ * Pipelined variant of nsfrb_stream_push_host for back-to-back chunks: the call enqueues the host->device copy of
+ * the chunk on a copy stream owned by the plan, the push (nsfrb_stream_push) on a compute stream owned by the plan
+ * once the copy has landed, and the device->host copies of snr_map / argmax / ncands and of all cand_capacity
+ * candidate records into the caller's buffers -- and returns without waiting.  The copy of chunk i+1 overlaps the
+ * search of chunk i.  Two pushes may be in flight (two staging slots): a third call first waits for the oldest.
+ *   chunk_host and the four output buffers must stay valid and untouched until nsfrb_stream_wait (or the second
+ *   following call) returns; use page-locked memory, otherwise the copies are staged by the driver and do not overlap.
+ *   Different pushes in flight need different output buffers.
+ * nsfrb_stream_wait blocks until every push in flight has delivered its outputs.  Do not mix with
+ * nsfrb_stream_push / nsfrb_stream_push_host / nsfrb_stream_reset on the same plan without an nsfrb_stream_wait (and,
+ * for the device-pointer variant, a synchronisation of the caller's stream) in between.
+ */
+int nsfrb_stream_push_host_async(nsfrb_plan *plan, const float *chunk_host, int chunk_nt, float *snr_map_host,
+                                 int32_t *argmax_host, nsfrb_cand *cands_host, uint32_t cand_capacity,
+                                 uint32_t *ncands_host);
+int nsfrb_stream_wait(nsfrb_plan *plan);
+
 /* Release everything the plan owns.  NULL is a no-op returning 0. */
 int nsfrb_plan_destroy(nsfrb_plan *plan);
 

@@ -204,6 +204,54 @@ int copy_back(nsfrb_plan *pl, cudaStream_t st, float *snr_h, int32_t *arg_h, nsf
     return NSFRB_OK;
 }
 
+void pipe_free(nsfrb_plan *pl)
+{
+    auto *pp = pl->pipe;
+    if (!pp) return;
+    for (int b = 0; b < 2; ++b) {
+        if (pp->done[b]) cudaEventSynchronize(pp->done[b]);
+        cudaFree(pp->d_in[b]); cudaFree(pp->d_snr[b]); cudaFree(pp->d_arg[b]); cudaFree(pp->d_cands[b]);
+        cudaFree(pp->d_ncands[b]);
+        if (pp->copied[b]) cudaEventDestroy(pp->copied[b]);
+        if (pp->done[b]) cudaEventDestroy(pp->done[b]);
+    }
+    if (pp->s_copy) cudaStreamDestroy(pp->s_copy);
+    if (pp->s_comp) cudaStreamDestroy(pp->s_comp);
+    delete pp;
+    pl->pipe = nullptr;
+}
+
+int pipe_slot(nsfrb_plan *pl, int b, size_t in_bytes, uint32_t cap)
+{
+    if (!pl->pipe) {
+        pl->pipe = new (std::nothrow) nsfrb_plan::HostPipe();
+        if (!pl->pipe) return fail(NSFRB_ENOMEM, "out of host memory");
+        CU(cudaStreamCreateWithFlags(&pl->pipe->s_copy, cudaStreamNonBlocking), "copy stream");
+        CU(cudaStreamCreateWithFlags(&pl->pipe->s_comp, cudaStreamNonBlocking), "compute stream");
+    }
+    auto *pp = pl->pipe;
+    if (!pp->copied[b]) CU(cudaEventCreateWithFlags(&pp->copied[b], cudaEventDisableTiming), "event");
+    if (!pp->done[b]) CU(cudaEventCreateWithFlags(&pp->done[b], cudaEventDisableTiming), "event");
+    if (pp->busy[b]) {   // the push that used this slot two calls ago: its staging and host outputs must be complete
+        CU(cudaEventSynchronize(pp->done[b]), "wait for the slot");
+        pp->busy[b] = false;
+    }
+    if (pp->in_bytes[b] < in_bytes) {
+        cudaFree(pp->d_in[b]); pp->d_in[b] = nullptr; pp->in_bytes[b] = 0;
+        CU(cudaMalloc(reinterpret_cast<void **>(&pp->d_in[b]), in_bytes), "staging input alloc");
+        pp->in_bytes[b] = in_bytes;
+    }
+    if (!pp->d_snr[b]) CU(cudaMalloc(reinterpret_cast<void **>(&pp->d_snr[b]), (size_t)pl->npix * sizeof(float)), "staging alloc");
+    if (!pp->d_arg[b]) CU(cudaMalloc(reinterpret_cast<void **>(&pp->d_arg[b]), 3 * (size_t)pl->npix * sizeof(int32_t)), "staging alloc");
+    if (!pp->d_ncands[b]) CU(cudaMalloc(reinterpret_cast<void **>(&pp->d_ncands[b]), sizeof(uint32_t)), "staging alloc");
+    if (cap > pp->cands_cap[b]) {
+        cudaFree(pp->d_cands[b]); pp->d_cands[b] = nullptr; pp->cands_cap[b] = 0;
+        CU(cudaMalloc(reinterpret_cast<void **>(&pp->d_cands[b]), (size_t)cap * sizeof(nsfrb_cand)), "staging alloc");
+        pp->cands_cap[b] = cap;
+    }
+    return NSFRB_OK;
+}
+
 } // namespace
 
 #pragma GCC visibility push(default)
@@ -446,6 +494,12 @@ int nsfrb_stream_set_cubes(nsfrb_plan *pl, float *snr_cube, int32_t *toa_cube)
 int nsfrb_stream_reset(nsfrb_plan *pl)
 {
     if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (pl->pipe)   // pipelined pushes still in flight read and write the ring
+        for (int b = 0; b < 2; ++b)
+            if (pl->pipe->busy[b]) {
+                CU(cudaEventSynchronize(pl->pipe->done[b]), "wait");
+                pl->pipe->busy[b] = false;
+            }
     pl->n_received = 0;
     stream_reset(pl);
     return NSFRB_OK;
@@ -482,10 +536,54 @@ int nsfrb_stream_push_host(nsfrb_plan *pl, const float *chunk_host, int chunk_nt
     return copy_back(pl, st, snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host);
 }
 
+int nsfrb_stream_push_host_async(nsfrb_plan *pl, const float *chunk_host, int chunk_nt, float *snr_map_host,
+                                 int32_t *argmax_host, nsfrb_cand *cands_host, uint32_t cand_capacity,
+                                 uint32_t *ncands_host)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (!chunk_host) return fail(NSFRB_EINVAL, "chunk is null");
+    if (chunk_nt < 1 || chunk_nt > pl->nt) return fail(NSFRB_EINVAL, "chunk_nt must be in [1, nt]");
+    if (int rc = check_outputs(snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host)) return rc;
+    CU(cudaSetDevice(pl->device), "set device");
+    const size_t bytes = (size_t)pl->nchan * chunk_nt * (size_t)pl->npix * sizeof(float);
+    const int b = pl->pipe ? (int)(pl->pipe->count & 1) : 0;
+    if (int rc = pipe_slot(pl, b, bytes, cand_capacity)) return rc;
+    auto *pp = pl->pipe;
+    // copy stream: chunk i+1 travels while the compute stream still works on chunk i
+    CU(cudaMemcpyAsync(pp->d_in[b], chunk_host, bytes, cudaMemcpyHostToDevice, pp->s_copy), "H2D chunk");
+    CU(cudaEventRecord(pp->copied[b], pp->s_copy), "event record");
+    CU(cudaStreamWaitEvent(pp->s_comp, pp->copied[b], 0), "stream wait");
+    if (int rc = nsfrb_stream_push(pl, pp->d_in[b], chunk_nt, pp->s_comp, pp->d_snr[b], pp->d_arg[b], pp->d_cands[b],
+                                   cand_capacity, pp->d_ncands[b]))
+        return rc;
+    CU(cudaMemcpyAsync(snr_map_host, pp->d_snr[b], (size_t)pl->npix * sizeof(float), cudaMemcpyDeviceToHost, pp->s_comp), "D2H snr");
+    CU(cudaMemcpyAsync(argmax_host, pp->d_arg[b], 3 * (size_t)pl->npix * sizeof(int32_t), cudaMemcpyDeviceToHost, pp->s_comp), "D2H argmax");
+    CU(cudaMemcpyAsync(ncands_host, pp->d_ncands[b], sizeof(uint32_t), cudaMemcpyDeviceToHost, pp->s_comp), "D2H ncands");
+    if (cand_capacity > 0)   // the count is not known on the host yet: all cand_capacity records travel
+        CU(cudaMemcpyAsync(cands_host, pp->d_cands[b], (size_t)cand_capacity * sizeof(nsfrb_cand), cudaMemcpyDeviceToHost, pp->s_comp), "D2H cands");
+    CU(cudaEventRecord(pp->done[b], pp->s_comp), "event record");
+    pp->busy[b] = true;
+    ++pp->count;
+    return NSFRB_OK;
+}
+
+int nsfrb_stream_wait(nsfrb_plan *pl)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    if (!pl->pipe) return NSFRB_OK;
+    for (int b = 0; b < 2; ++b)
+        if (pl->pipe->busy[b]) {
+            CU(cudaEventSynchronize(pl->pipe->done[b]), "wait");
+            pl->pipe->busy[b] = false;
+        }
+    return NSFRB_OK;
+}
+
 int nsfrb_plan_destroy(nsfrb_plan *pl)
 {
     if (!pl) return NSFRB_OK;
     cudaDeviceSynchronize();
+    pipe_free(pl);
     free_plan(pl);
     return NSFRB_OK;
 }

@@ -121,6 +121,20 @@ struct nsfrb_plan {
     int32_t *cube_toa = nullptr;
     // offline path: plan-specialised k_search3 (nsfrb_search_kernel.cuh), compiled at the first nsfrb_search
     nsfrb::Search3State *search3 = nullptr;
+    // pipelined host-buffer pushes (nsfrb_stream_push_host_async): two staging slots, a copy and a compute stream
+    struct HostPipe {
+        cudaStream_t s_copy = nullptr, s_comp = nullptr;
+        cudaEvent_t copied[2] = {nullptr, nullptr}, done[2] = {nullptr, nullptr};
+        bool busy[2] = {false, false};
+        float *d_in[2] = {nullptr, nullptr};
+        size_t in_bytes[2] = {0, 0};
+        float *d_snr[2] = {nullptr, nullptr};
+        int32_t *d_arg[2] = {nullptr, nullptr};
+        nsfrb_cand *d_cands[2] = {nullptr, nullptr};
+        uint32_t cands_cap[2] = {0, 0};
+        uint32_t *d_ncands[2] = {nullptr, nullptr};
+        uint64_t count = 0;
+    } *pipe = nullptr;
     // candidate selection (nsfrb_cluster.cu): per-CTA key lists + ticket, allocated at the first nsfrb_cluster
     void *d_cluster_ws = nullptr;
 };

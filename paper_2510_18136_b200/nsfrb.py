@@ -45,7 +45,8 @@ EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stre
            "nsfrb_stream_push_host", "nsfrb_plan_destroy", "nsfrb_plan_get_delays", "nsfrb_plan_get_info",
            "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
            "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes",
-           "nsfrb_psf_mask", "nsfrb_cluster", "nsfrb_median_subtract")
+           "nsfrb_psf_mask", "nsfrb_cluster", "nsfrb_median_subtract",
+           "nsfrb_stream_push_host_async", "nsfrb_stream_wait")
 
 _lib = None
 
@@ -97,6 +98,10 @@ def lib() -> ctypes.CDLL:
                                               ctypes.POINTER(ctypes.c_size_t)]
         L.nsfrb_bin_time.restype = ctypes.c_int
         L.nsfrb_bin_time.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_int, vp, vp]
+        L.nsfrb_stream_push_host_async.restype = ctypes.c_int
+        L.nsfrb_stream_push_host_async.argtypes = [vp, vp, ctypes.c_int, vp, vp, vp, ctypes.c_uint32, vp]
+        L.nsfrb_stream_wait.restype = ctypes.c_int
+        L.nsfrb_stream_wait.argtypes = [vp]
         L.nsfrb_median_subtract.restype = ctypes.c_int
         L.nsfrb_median_subtract.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, vp, vp, vp]
         L.nsfrb_psf_mask.restype = ctypes.c_int
@@ -368,6 +373,18 @@ class Plan:
                                             self._stream_handle(stream), out[0].data_ptr(), out[1].data_ptr(),
                                             out[2].data_ptr(), self.cand_capacity, out[3].data_ptr()))
         return out
+
+    def stream_push_host_async(self, chunk_host: torch.Tensor, out):
+        """nsfrb_stream_push_host_async: returns at once; `out` (from _host_out(), pinned) is valid after stream_wait()
+        or after the second following call.  Keep chunk_host and out alive and untouched until then."""
+        self._check_host(chunk_host, (self.nchan, chunk_host.shape[1], self.npix))
+        _check(lib().nsfrb_stream_push_host_async(self._h, chunk_host.data_ptr(), int(chunk_host.shape[1]),
+                                                  out[0].data_ptr(), out[1].data_ptr(), out[2].data_ptr(),
+                                                  self.cand_capacity, out[3].data_ptr()))
+        return out
+
+    def stream_wait(self):
+        _check(lib().nsfrb_stream_wait(self._h))
 
     # -- checks / lifetime
     def _check_dev(self, t, shape):

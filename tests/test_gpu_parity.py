@@ -497,3 +497,43 @@ def test_stream_cubes_match_oracle():
         plan.stream_set_cubes(None, None)
         plan.stream_push(torch.randn((wl.nchan, 5, wl.npix), device="cuda", generator=g), out)
         torch.cuda.synchronize()
+
+
+def test_pipelined_host_pushes_equal_device_pushes():
+    """nsfrb_stream_push_host_async (copy of chunk i+1 overlapping the search of chunk i, two pushes in flight) must
+    deliver, for every push, exactly what nsfrb_stream_push delivers for the same chunks on a second plan; the last
+    push is also checked against the oracle."""
+    nsfrb = _nsfrb()
+    wl = W.config("c1")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    n_push = 7
+    src = W.ChunkSource(wl, d, n_push, "cuda")
+    chunks = [src.next().clone() for _ in range(n_push)]
+    host = [c.cpu().pin_memory() for c in chunks]
+    so = oracle.StreamOracle(wl.nchan, wl.npix, wl.nt, d, wl.width_list)
+    with nsfrb.Plan.for_workload(wl, cand_capacity=64) as pa, nsfrb.Plan.for_workload(wl, cand_capacity=64) as pb:
+        outs = [pa._host_out() for _ in range(n_push)]
+        for i in range(n_push):                       # all enqueued back to back; the third call waits for the first
+            pa.stream_push_host_async(host[i], outs[i])
+        pa.stream_wait()
+        ref = pb.alloc_outputs()
+        for i in range(n_push):
+            pb.stream_push(chunks[i], ref)
+            torch.cuda.synchronize()
+            ores = so.push(chunks[i].cpu().numpy(), nthreads=8)
+            assert np.array_equal(outs[i][0].numpy(), ref.snr_map.cpu().numpy()), i
+            assert np.array_equal(outs[i][1].numpy(), ref.argmax.cpu().numpy()), i
+            n = int(outs[i][3].numpy().view(np.uint32)[0])
+            assert n == ref.n_found()
+            got = outs[i][2].numpy()[: n * nsfrb.CAND_DTYPE.itemsize].view(nsfrb.CAND_DTYPE)
+            assert sorted(map(tuple, got)) == sorted(map(tuple, ref.candidates()))
+        snr = outs[-1][0].numpy()
+        assert np.all(np.abs(snr - ores.snr) <= 1e-4 + 1e-4 * np.abs(ores.snr))
+        # the synchronous calls still work on the same plan after a wait, and reset waits for pushes in flight
+        pa.stream_push_host_async(host[0], outs[0])
+        pa.stream_reset()
+        o = pa.stream_push_host(host[0])
+        pb.stream_reset()
+        pb.stream_push(chunks[0], ref)
+        torch.cuda.synchronize()
+        assert np.array_equal(o[0].numpy(), ref.snr_map.cpu().numpy())
