@@ -87,10 +87,13 @@ typedef struct {
     int64_t raw_end_min;     /* S5 */
     int64_t t_offset;        /* S6 */
     int brute;               /* 1: O(w) direct boxcar sums, no prefix array */
+    const double *sigma_norm; /* NULL, or [n_sel][ndm]: the standard deviation S is normalised by (reading R30:
+                                 the "running standard deviation") instead of this call's own sigma_k */
 } oracle_problem;
 
 /* scratch: D[nt], P[nt+1] */
-static void oracle_one_pixel(const oracle_problem *q, int64_t p, double *D, double *P,
+static void oracle_one_pixel(const oracle_problem *q, int64_t p, const double *sigma_norm /* [ndm] or NULL */,
+                             double *D, double *P,
                              double *snr_out, int64_t *arg_out /* [3] */,
                              double *mu_out /* [ndm] or NULL */,
                              double *sigma_out /* [ndm] or NULL */,
@@ -142,7 +145,8 @@ static void oracle_one_pixel(const oracle_problem *q, int64_t p, double *D, doub
         for (int j = 0; j < q->nw; ++j) {
             const int w = q->widths[j];
             if (w > T) continue;
-            const double norm = sigma * sqrt((double)w);
+            const double snorm = sigma_norm ? sigma_norm[k] : sigma; /* O5: sigma_k, or the caller's running one */
+            const double norm = snorm * sqrt((double)w);
             double kj_best = -INFINITY;
             int64_t kj_t = -1;
             for (int t = 0; t <= T - w; ++t) {
@@ -154,7 +158,7 @@ static void oracle_one_pixel(const oracle_problem *q, int64_t p, double *D, doub
                 } else {
                     B = P[t + w] - P[t];
                 }
-                const double S = (sigma == 0.0) ? 0.0 : B / norm;
+                const double S = (snorm == 0.0) ? 0.0 : B / norm;
                 if (S > kj_best) { kj_best = S; kj_t = t; }
             }
             if (best_out) {
@@ -191,7 +195,8 @@ static void *oracle_worker(void *arg)
     const size_t kw = (size_t)q->ndm * (size_t)q->nw;
     for (int64_t i = jb->begin; i < jb->end; i += jb->stride) {
         const int64_t p = jb->pixels ? jb->pixels[i] : i;
-        oracle_one_pixel(q, p, D, P, &jb->snr[i], &jb->argmax[3 * i],
+        oracle_one_pixel(q, p, q->sigma_norm ? q->sigma_norm + (size_t)i * q->ndm : NULL, D, P,
+                         &jb->snr[i], &jb->argmax[3 * i],
                          jb->mu ? jb->mu + (size_t)i * q->ndm : NULL,
                          jb->sigma ? jb->sigma + (size_t)i * q->ndm : NULL,
                          jb->best ? jb->best + (size_t)i * kw : NULL,
@@ -210,12 +215,35 @@ static void *oracle_worker(void *arg)
  * nthreads >= 1: pixels are dealt round-robin to that many pthreads (each pixel is
  * still computed by one thread, start to finish).
  */
+int nsfrb_oracle_search_norm(const float *cube, int64_t npix, int nchan, int nt,
+                             const int32_t *delays, int ndm, const int32_t *widths, int nw,
+                             int64_t raw_end_min, int64_t t_offset, int brute,
+                             const int64_t *pixels, int64_t n_sel, int nthreads,
+                             double *snr, int64_t *argmax,
+                             double *mu, double *sigma, double *best, int64_t *best_t,
+                             const double *sigma_norm);
+
 int nsfrb_oracle_search(const float *cube, int64_t npix, int nchan, int nt,
                         const int32_t *delays, int ndm, const int32_t *widths, int nw,
                         int64_t raw_end_min, int64_t t_offset, int brute,
                         const int64_t *pixels, int64_t n_sel, int nthreads,
                         double *snr, int64_t *argmax,
                         double *mu, double *sigma, double *best, int64_t *best_t)
+{
+    return nsfrb_oracle_search_norm(cube, npix, nchan, nt, delays, ndm, widths, nw, raw_end_min, t_offset, brute,
+                                    pixels, n_sel, nthreads, snr, argmax, mu, sigma, best, best_t, NULL);
+}
+
+/* As nsfrb_oracle_search, but S(k,j,t) is normalised by sigma_norm[i][k] (i = position in the selection) when
+ * sigma_norm != NULL -- NEXT 1 / reading R30: the running standard deviation carried across pushes.  mu_k and the
+ * boxcar sums are this call's; the sigma output still reports this call's own sigma_k. */
+int nsfrb_oracle_search_norm(const float *cube, int64_t npix, int nchan, int nt,
+                             const int32_t *delays, int ndm, const int32_t *widths, int nw,
+                             int64_t raw_end_min, int64_t t_offset, int brute,
+                             const int64_t *pixels, int64_t n_sel, int nthreads,
+                             double *snr, int64_t *argmax,
+                             double *mu, double *sigma, double *best, int64_t *best_t,
+                             const double *sigma_norm)
 {
     if (!cube || !delays || !widths || !snr || !argmax) return -1;
     if (npix < 1 || nchan < 1 || nt < 1 || ndm < 1 || nw < 1 || n_sel < 0) return -1;
@@ -233,6 +261,7 @@ int nsfrb_oracle_search(const float *cube, int64_t npix, int nchan, int nt,
     q.cube = cube; q.npix = npix; q.nchan = nchan; q.nt = nt;
     q.delays = delays; q.ndm = ndm; q.widths = widths; q.nw = nw;
     q.raw_end_min = raw_end_min; q.t_offset = t_offset; q.brute = brute;
+    q.sigma_norm = sigma_norm;
 
     oracle_job jobs[256];
     pthread_t th[256];

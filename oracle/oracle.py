@@ -46,6 +46,8 @@ def _load():
             ctypes.c_int64, ctypes.c_int64, ctypes.c_int, i64p, ctypes.c_int64, ctypes.c_int,
             f64p, i64p, f64p, f64p, f64p, i64p,
         ]
+        lib.nsfrb_oracle_search_norm.restype = ctypes.c_int
+        lib.nsfrb_oracle_search_norm.argtypes = lib.nsfrb_oracle_search.argtypes + [f64p]
         lib.nsfrb_oracle_snr_at.restype = ctypes.c_double
         lib.nsfrb_oracle_snr_at.argtypes = [
             f32p, ctypes.c_int64, ctypes.c_int, ctypes.c_int, i32p, ctypes.c_int, i32p, ctypes.c_int,
@@ -93,8 +95,9 @@ class OracleResult:
 
 
 def search(cube, delay_table, widths, *, pixels=None, raw_end_min=0, t_offset=0,
-           brute=False, nthreads=1, details=False) -> OracleResult:
-    """O2..O6 (+S5/S6) for the selected pixels of cube[nchan][nt][npix] (float32)."""
+           brute=False, nthreads=1, details=False, sigma_norm=None) -> OracleResult:
+    """O2..O6 (+S5/S6) for the selected pixels of cube[nchan][nt][npix] (float32).
+    sigma_norm [n_sel][ndm] (float64), if given, replaces sigma_k in O5 (reading R30: running standard deviation)."""
     cube = np.ascontiguousarray(cube, dtype=np.float32)
     if cube.ndim != 3:
         raise ValueError("cube must be [nchan][nt][npix]")
@@ -120,11 +123,16 @@ def search(cube, delay_table, widths, *, pixels=None, raw_end_min=0, t_offset=0,
         sigma = np.empty((n_sel, ndm), dtype=np.float64)
         best = np.empty((n_sel, ndm, nw), dtype=np.float64)
         best_t = np.empty((n_sel, ndm, nw), dtype=np.int64)
-    rc = _load().nsfrb_oracle_search(
+    sn = None
+    if sigma_norm is not None:
+        sn = np.ascontiguousarray(sigma_norm, dtype=np.float64)
+        if sn.shape != (n_sel, ndm):
+            raise ValueError("sigma_norm must be [n_sel][ndm]")
+    rc = _load().nsfrb_oracle_search_norm(
         _p(cube, ctypes.c_float), npix, nchan, nt, _p(d, ctypes.c_int32), ndm, _p(w, ctypes.c_int32), nw,
         int(raw_end_min), int(t_offset), int(bool(brute)), _p(pix, ctypes.c_int64), n_sel, int(nthreads),
         _p(snr, ctypes.c_double), _p(arg, ctypes.c_int64), _p(mu, ctypes.c_double), _p(sigma, ctypes.c_double),
-        _p(best, ctypes.c_double), _p(best_t, ctypes.c_int64))
+        _p(best, ctypes.c_double), _p(best_t, ctypes.c_int64), _p(sn, ctypes.c_double))
     if rc != 0:
         raise ValueError(f"nsfrb_oracle_search failed: {rc}")
     return OracleResult(snr, arg, sel, mu, sigma, best, best_t)
@@ -194,3 +202,36 @@ class StreamOracle:
         self.hist = np.concatenate([self.hist, chunk], axis=1)[:, -self.L:, :]
         lo = max(0, self.n - self.L)                               # S1
         return search(self.hist, self.d, self.w, raw_end_min=n_prev - lo, t_offset=lo, **kw)  # S3..S6
+
+
+def running_variance(var_prev, sigma_now, alpha: float):
+    """Reading R30 ("normalized by the running standard deviation", L180 "the running standard deviation
+    accumulated during" the survey): per (pixel, DM trial) an exponentially weighted variance carried across pushes,
+        v_0 = sigma_0^2,   v_n = (1 - alpha) v_{n-1} + alpha sigma_n^2,
+    sigma_n = this push's own sigma_k (O3).  A trial with no valid sample yet (sigma NaN) keeps its previous state."""
+    s2 = np.asarray(sigma_now, dtype=np.float64) ** 2
+    if var_prev is None:
+        return s2.copy()
+    v = (1.0 - alpha) * var_prev + alpha * s2
+    v = np.where(np.isnan(var_prev), s2, v)        # first defined sigma starts the recursion
+    return np.where(np.isnan(s2), var_prev, v)
+
+
+class RunningStreamOracle(StreamOracle):
+    """S1..S6 with O5 normalised by the running standard deviation (reading R30): every push first evaluates the
+    offline definition for this push's own sigma_k, updates the running variance, then evaluates the definition again
+    with sigma_norm = sqrt(v_n).  No incremental shortcut."""
+
+    def __init__(self, nchan, npix, ring_len, delay_table, widths, alpha):
+        super().__init__(nchan, npix, ring_len, delay_table, widths)
+        self.alpha = float(alpha)
+        self.var = None            # [npix][ndm] float64
+
+    def push(self, chunk, **kw) -> OracleResult:
+        kw.pop("details", None)
+        inst = super().push(chunk, details=True, **kw)
+        self.var = running_variance(self.var, inst.sigma, self.alpha)
+        n_prev = self.n - np.asarray(chunk).shape[1]
+        lo = max(0, self.n - self.L)
+        return search(self.hist, self.d, self.w, raw_end_min=n_prev - lo, t_offset=lo, details=True,
+                      sigma_norm=np.sqrt(self.var), **kw)

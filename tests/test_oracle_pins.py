@@ -509,3 +509,66 @@ def test_median_subtraction_cancels_in_the_search():
     r1 = oracle.search(oracle.median_subtract(cube)[0], d, wl.width_list)
     assert np.allclose(r0.snr, r1.snr, rtol=0, atol=2e-5)
     assert (r0.argmax == r1.argmax).all(axis=1).mean() > 0.95
+
+
+# ---- NEXT 1 (second part): running standard deviation (reading R30) ----------------------------
+
+def test_sigma_norm_scales_every_snr_and_keeps_the_argmax():
+    wl = W.config("c1")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    cube = W.make_cube(wl).numpy()[:, :, :30]
+    r0 = oracle.search(cube, d, wl.width_list, details=True)
+    r1 = oracle.search(cube, d, wl.width_list, details=True, sigma_norm=r0.sigma)          # own sigma: identity
+    assert np.array_equal(r0.snr, r1.snr) and np.array_equal(r0.argmax, r1.argmax) and np.array_equal(r0.best, r1.best)
+    r2 = oracle.search(cube, d, wl.width_list, details=True, sigma_norm=4.0 * r0.sigma)    # power of two: exact
+    assert np.array_equal(r2.snr, r0.snr / 4.0) and np.array_equal(r2.argmax, r0.argmax)
+    assert np.array_equal(r2.sigma, r0.sigma)                                              # still this call's sigma
+    # a per-trial factor: each (pixel, k) row of the maxima scales by its own factor; the winner is the max of those
+    rng = np.random.default_rng(0)
+    f = rng.uniform(0.5, 2.0, size=r0.sigma.shape)
+    r3 = oracle.search(cube, d, wl.width_list, details=True, sigma_norm=f * r0.sigma)
+    want = r0.best / f[:, :, None]
+    assert np.allclose(r3.best, want, rtol=1e-12, atol=0)
+    assert np.allclose(r3.snr, want.reshape(want.shape[0], -1).max(axis=1), rtol=1e-12, atol=0)
+    assert np.array_equal(r3.best_t, r0.best_t)
+    # brute-force boxcar route agrees
+    r4 = oracle.search(cube[:, :, :6], d, wl.width_list, brute=True, sigma_norm=(f * r0.sigma)[:6])
+    assert np.allclose(r4.snr, r3.snr[:6], rtol=1e-9, atol=1e-12)
+    # sigma_norm = 0 -> S = 0 (the O5 convention), as for a flat series
+    z = oracle.search(cube[:, :, :3], d, wl.width_list, sigma_norm=np.zeros((3, len(wl.dm_list))))
+    assert not z.snr.any()
+
+
+def test_running_variance_recursion_closed_form():
+    a = 0.25
+    v = None
+    for _ in range(6):
+        v = oracle.running_variance(v, np.asarray([[2.0]]), a)
+    assert v[0, 0] == 4.0                                           # constant sigma: fixed point
+    v = np.asarray([[9.0]])
+    for n in range(1, 8):                                           # step from 9 to 1: v_n = 1 + 8 (1-a)^n
+        v = oracle.running_variance(v, np.asarray([[1.0]]), a)
+        assert v[0, 0] == pytest.approx(1.0 + 8.0 * (1 - a) ** n, rel=1e-14)
+    assert oracle.running_variance(np.asarray([[9.0]]), np.asarray([[3.0]]), 1.0)[0, 0] == 9.0    # alpha = 1: instantaneous
+    # undefined trials: NaN sigma keeps the state; a first defined sigma starts it
+    v = oracle.running_variance(np.asarray([[np.nan, 4.0]]), np.asarray([[3.0, np.nan]]), a)
+    assert v.tolist() == [[9.0, 4.0]]
+
+
+def test_running_sigma_stream_alpha_one_is_the_plain_stream_and_bias_is_removed():
+    wl = W.config("c1")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    rng = np.random.default_rng(4)
+    npix = 12
+    plain = oracle.StreamOracle(wl.nchan, npix, wl.nt, d, wl.width_list)
+    run1 = oracle.RunningStreamOracle(wl.nchan, npix, wl.nt, d, wl.width_list, alpha=1.0)
+    runs = oracle.RunningStreamOracle(wl.nchan, npix, wl.nt, d, wl.width_list, alpha=0.05)
+    for i in range(5):
+        chunk = rng.normal(size=(wl.nchan, wl.chunk_nt, npix)).astype(np.float32)
+        if i == 4:   # a bright, wide, undispersed pulse in pixel 3: it inflates this push's own sigma (L130)
+            chunk[:, 5:5 + 16, 3] += 3.0
+        a, b, c = plain.push(chunk), run1.push(chunk), runs.push(chunk)
+        assert np.array_equal(a.snr, b.snr) and np.array_equal(a.argmax, b.argmax)           # alpha = 1
+    assert c.snr[3] > 1.15 * a.snr[3]            # the slowly updated sigma is not contaminated by the pulse
+    others = np.arange(npix) != 3
+    assert np.allclose(c.snr[others], a.snr[others], rtol=0.35)   # 25..64-sample sigmas scatter by ~15 %
