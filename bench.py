@@ -122,7 +122,7 @@ def barrier(world):
 class StreamBench:
     """C2: ring filled to steady state, then timed pushes."""
 
-    def __init__(self, wl, plan_mod, cubes=False):
+    def __init__(self, wl, plan_mod, cubes=False, running=False):
         self.wl = wl
         self.plan = plan_mod.Plan.for_workload(wl, cand_capacity=4096)
         self.delays = self.plan.delays()
@@ -131,6 +131,9 @@ class StreamBench:
             shape = (len(wl.dm_list), len(wl.width_list), wl.npix)
             self.cubes = (torch.empty(shape, device="cuda"), torch.empty(shape, dtype=torch.int32, device="cuda"))
             self.plan.stream_set_cubes(*self.cubes)
+        if running:  # NEXT 1: also the maps normalised by the running standard deviation
+            self.run = (torch.empty(wl.npix, device="cuda"), torch.empty((3, wl.npix), dtype=torch.int32, device="cuda"))
+            self.plan.stream_set_running_sigma(0.05, *self.run)
         n_fill = -(-wl.nt // wl.chunk_nt) + 1
         self.src = W.ChunkSource(wl, self.delays, n_fill + 600, "cuda")
         self.out = self.plan.alloc_outputs()
@@ -245,7 +248,7 @@ def run_cuda_arm(args, rank, world, local):
     torch.cuda.set_device(local)
     hbm_peak, peak_src, peaks = measured_peaks()
     wl = W.config(args.workload)
-    bench = StreamBench(wl, nsfrb, cubes=args.cubes) if wl.streaming else OfflineBench(wl, nsfrb)
+    bench = StreamBench(wl, nsfrb, cubes=args.cubes, running=args.running) if wl.streaming else OfflineBench(wl, nsfrb)
 
     flusher = None
     if bench.algorithmic_bytes() < (256 << 20):
@@ -361,7 +364,8 @@ def run_cuda_arm(args, rank, world, local):
                    "ndm": len(wl.dm_list), "ndm_unique": info["ndm_unique"], "nwidth": len(wl.width_list),
                    "cells_per_step": bench.cells_per_step,
                    "l2": "inputs larger than L2 (ring 6.4 GB + rotating chunks)" if flusher is None else "L2 flushed between steps",
-                   "parallelism": "replicas only" if world > 1 else "1 GPU", "cubes": bool(args.cubes and wl.streaming)},
+                   "parallelism": "replicas only" if world > 1 else "1 GPU", "cubes": bool(args.cubes and wl.streaming),
+                   "running_sigma": bool(args.running and wl.streaming)},
         "e2e": e2e, "gpu_launches": launches * args.steps, "gpu_launches_per_step": launches,
         "clocks": clocks,
         "roofline": roof,
@@ -571,6 +575,7 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cubes", action="store_true", help="c2: also write the S/N and TOA cubes every push (NEXT 3)")
+    ap.add_argument("--running", action="store_true", help="c2: also the running-sigma maps every push (NEXT 1)")
     ap.add_argument("--op", default="search", choices=["search", "bin", "cluster", "median"],
                     help="bin: time the binning kernel (NEXT 2); cluster: top-10 + PSF clustering (NEXT 3); "
                          "median: per-pixel median subtraction (NEXT 1)")

@@ -134,6 +134,23 @@ int nsfrb_stream_push(nsfrb_plan *plan, const float *chunk, int chunk_nt, void *
  */
 int nsfrb_stream_set_cubes(nsfrb_plan *plan, float *snr_cube, int32_t *toa_cube);
 
+/*
+ * Running standard deviation ("normalized by the running standard deviation", L180; SURVEY.md 8(f) NEXT 1,
+ * second part; reading R30): besides snr_map/argmax (normalised by this push's own sigma_k, O5), every later push
+ * also writes the maps normalised by a standard deviation carried across pushes.  Per (pixel, DM trial):
+ *     v_0 = sigma_0^2,   v_n = (1 - alpha) v_{n-1} + alpha sigma_n^2      (sigma_n = this push's sigma_k; a trial
+ *     S_run(k,j,t) = (B_j(t) - w_j mu_k) / (sqrt(v_n) sqrt(w_j))           without a valid sample keeps its state)
+ * (S_run = 0 where v_n = 0), reduced over (k, j, t) exactly like O6.  A pulse inflates only a fraction alpha of the
+ * normalisation of its own push (the bias of L130).  alpha = 1 reproduces snr_map/argmax.
+ *   alpha        in (0, 1]
+ *   snr_map_run  device, [npix] float32;  argmax_run  device, [3][npix] int32 (layout and conventions of
+ *                snr_map/argmax); both NULL switch the mode off.  The caller owns both buffers.
+ * The running variance lives in the plan; it restarts with this call and with nsfrb_stream_reset.  The mode uses the
+ * per-(trial, width) maxima of nsfrb_stream_set_cubes (the library keeps its own cubes, 8*ndm*nwidth*npix bytes, if the
+ * caller registered none) and adds one small launch per push.
+ */
+int nsfrb_stream_set_running_sigma(nsfrb_plan *plan, double alpha, float *snr_map_run, int32_t *argmax_run);
+
 /* Forget all pushed samples; the plan can be used for nsfrb_search again. */
 int nsfrb_stream_reset(nsfrb_plan *plan);
 

@@ -491,6 +491,14 @@ int nsfrb_stream_set_cubes(nsfrb_plan *pl, float *snr_cube, int32_t *toa_cube)
     return NSFRB_OK;
 }
 
+int nsfrb_stream_set_running_sigma(nsfrb_plan *pl, double alpha, float *snr_map_run, int32_t *argmax_run)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    std::string err;
+    if (int rc = stream_set_running(pl, alpha, snr_map_run, argmax_run, err)) return fail(rc, err);
+    return NSFRB_OK;
+}
+
 int nsfrb_stream_reset(nsfrb_plan *pl)
 {
     if (!pl) return fail(NSFRB_EINVAL, "plan is null");

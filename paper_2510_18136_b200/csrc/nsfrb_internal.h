@@ -119,6 +119,9 @@ struct nsfrb_plan {
     nsfrb::StreamState *stream = nullptr;
     float *cube_snr = nullptr;   // caller's optional cube outputs of the real-time path (nsfrb_stream_set_cubes)
     int32_t *cube_toa = nullptr;
+    float run_alpha = 0.f;       // running-sigma mode (nsfrb_stream_set_running_sigma): caller's outputs, or null = off
+    float *run_snr = nullptr;
+    int32_t *run_arg = nullptr;
     // offline path: plan-specialised k_search3 (nsfrb_search_kernel.cuh), compiled at the first nsfrb_search
     nsfrb::Search3State *search3 = nullptr;
     // pipelined host-buffer pushes (nsfrb_stream_push_host_async): two staging slots, a copy and a compute stream
@@ -158,6 +161,7 @@ int search3_slices(const nsfrb_plan *pl); // partial records per pixel written b
 void stream_free(nsfrb_plan *p);
 void stream_reset(nsfrb_plan *p);
 int stream_set_cubes(nsfrb_plan *pl, float *snr_cube, int32_t *toa_cube, std::string &err);
+int stream_set_running(nsfrb_plan *pl, double alpha, float *snr_run, int32_t *arg_run, std::string &err);
 size_t stream_bytes(const nsfrb_plan *p); // device bytes the real-time path holds (0 before the first push)
 // a8 + k_stream passes + reduction over slices; outputs as nsfrb_stream_push.  Returns an NSFRB_* code and
 // leaves the message in `err`.

@@ -46,6 +46,7 @@ struct StreamParams {
     int32_t bound[9];
     float *snr_cube;
     int32_t *toa_cube;
+    float *sig_out;
     int32_t t_offset;
 };
 
@@ -276,6 +277,12 @@ struct StreamState {
     float *snr_cube = nullptr; // caller's optional [ndm][nwidth][npix] outputs (nsfrb_stream_set_cubes)
     int32_t *toa_cube = nullptr;
     int32_t *d_canon = nullptr; // [ndm] lowest dm index with the same delay vector
+    // running-sigma mode (nsfrb_stream_set_running_sigma): this push's sigma and the running variance of every
+    // (unique trial, pixel); cubes owned by the library when the caller registered none
+    float *sig = nullptr, *var = nullptr;
+    bool var_init = false;
+    float *own_cs = nullptr;
+    int32_t *own_ct = nullptr;
     int guard = 0, max_slices = 0;
     size_t bytes = 0;
 };
@@ -343,6 +350,51 @@ __global__ void __launch_bounds__(256) k_stream_finalize(const SPartial *__restr
         argmax[(size_t)npix + p] = b.j;
         argmax[2 * (size_t)npix + p] = (int32_t)(((uint32_t)t_offset + (uint32_t)b.t) & 0x7fffffffu);
     }
+}
+
+// Running standard deviation (reading R30): v_n = (1 - alpha) v_{n-1} + alpha sigma_n^2 per (unique trial, pixel),
+// S_run = S * sigma_n / sqrt(v_n) applied to the per-(trial, width) maxima of this push (a positive factor per trial, so
+// the maximising window of every (trial, width) is unchanged); then the O6 reduction over trials and widths.
+__global__ void __launch_bounds__(256) k_running(const float *__restrict__ snr_cube, const int32_t *__restrict__ toa_cube,
+                                                  const float *__restrict__ sig, float *__restrict__ var,
+                                                  const int32_t *__restrict__ k_of_u, int nuniq, int nw, int npix,
+                                                  float alpha, int first, float *__restrict__ snr_run,
+                                                  int32_t *__restrict__ arg_run)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= npix) return;
+    float bs = __int_as_float(0xff800000);
+    int bk = -1, bj = -1, bt = -1;
+    for (int u = 0; u < nuniq; ++u) {
+        const float s = sig[(size_t)u * npix + p];
+        float v = var[(size_t)u * npix + p];
+        if (s != s) continue;                      // no valid sample of this trial yet: state untouched, no window
+        const float s2 = s * s;
+        v = (first || v != v) ? s2 : (1.f - alpha) * v + alpha * s2;
+        var[(size_t)u * npix + p] = v;
+        const float sr = sqrtf(v);
+        const float a = sr > 0.f ? s / sr : 0.f;   // sigma_run = 0 => S = 0 (the O5 convention)
+        const int k = k_of_u[u];
+        for (int j = 0; j < nw; ++j) {
+            const size_t ci = ((size_t)k * nw + j) * npix + p;
+            const float S = snr_cube[ci];
+            if (S == __int_as_float(0xff800000)) continue;
+            const float Sr = S * a;
+            const int t = toa_cube[ci];
+            bool better = bk < 0;
+            if (!better) {
+                if (Sr != bs) better = Sr > bs;
+                else if (k != bk) better = k < bk;
+                else if (j != bj) better = j < bj;
+                else better = t < bt;
+            }
+            if (better) { bs = Sr; bk = k; bj = j; bt = t; }
+        }
+    }
+    snr_run[p] = bs;
+    arg_run[p] = bk;
+    arg_run[(size_t)npix + p] = bj;
+    arg_run[2 * (size_t)npix + p] = bt;
 }
 
 // cubes: every entry starts as "no window" (-inf, -1) ...
@@ -489,6 +541,7 @@ void stream_free(nsfrb_plan *p)
     if (!p || !p->stream) return;
     StreamState *ss = p->stream;
     cudaFree(ss->ring); cudaFree(ss->base); cudaFree(ss->mu0); cudaFree(ss->partials); cudaFree(ss->mws); cudaFree(ss->aws); cudaFree(ss->sws); cudaFree(ss->d_canon);
+    cudaFree(ss->sig); cudaFree(ss->var); cudaFree(ss->own_cs); cudaFree(ss->own_ct);
     for (auto &l : ss->lib) if (l) cudaLibraryUnload(l);
     cudaGetLastError();
     delete ss;
@@ -511,6 +564,19 @@ void stream_reset(nsfrb_plan *p)
 {
     if (!p || !p->stream) return;
     if (p->stream->mu0) cudaMemset(p->stream->mu0, 0, (size_t)p->nuniq * p->npix * sizeof(float));
+    p->stream->var_init = false;   // the running variance starts again with the next push
+}
+
+// Running-sigma outputs (nulls switch the mode off).  The running variance restarts.
+int stream_set_running(nsfrb_plan *pl, double alpha, float *snr_run, int32_t *arg_run, std::string &err)
+{
+    if ((snr_run == nullptr) != (arg_run == nullptr)) { err = "snr_map_run and argmax_run must both be given or both be null"; return NSFRB_EINVAL; }
+    if (snr_run && !(alpha > 0.0 && alpha <= 1.0)) { err = "alpha must be in (0, 1]"; return NSFRB_EINVAL; }
+    pl->run_alpha = (float)alpha;
+    pl->run_snr = snr_run;
+    pl->run_arg = arg_run;
+    if (pl->stream) pl->stream->var_init = false;
+    return NSFRB_OK;
 }
 
 int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t st, float *snr_map, int32_t *argmax,
@@ -523,7 +589,25 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         }
     }
     StreamState *ss = pl->stream;
-    const int variant = ss->snr_cube ? 1 : 0;
+    const bool running = pl->run_snr != nullptr;
+    if (running) {   // needs this push's sigma per (unique trial, pixel) and the per-(trial, width) maxima
+        const size_t nb = (size_t)pl->nuniq * pl->npix * sizeof(float);
+        if (!ss->sig) {
+            SCU(cudaMalloc(reinterpret_cast<void **>(&ss->sig), nb), "sigma alloc");
+            SCU(cudaMalloc(reinterpret_cast<void **>(&ss->var), nb), "running variance alloc");
+            ss->bytes += 2 * nb;
+            ss->var_init = false;
+        }
+        if (!ss->snr_cube && !ss->own_cs) {
+            const size_t cb = (size_t)pl->ndm * pl->nw * pl->npix * sizeof(float);
+            SCU(cudaMalloc(reinterpret_cast<void **>(&ss->own_cs), cb), "cube alloc");
+            SCU(cudaMalloc(reinterpret_cast<void **>(&ss->own_ct), cb), "cube alloc");
+            ss->bytes += 2 * cb;
+        }
+    }
+    float *const cs = ss->snr_cube ? ss->snr_cube : (running ? ss->own_cs : nullptr);
+    int32_t *const ct = ss->snr_cube ? ss->toa_cube : (running ? ss->own_ct : nullptr);
+    const int variant = cs ? 1 : 0;
     if (int rc = stream_kernel(pl, ss, variant, err)) return rc;
     const StreamCfg &c = ss->cfg;
     const int L = pl->nt;
@@ -562,12 +646,14 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
     }
     const int base_slot = (int)(lo % L);
     const size_t cube_plane = (size_t)pl->nw * pl->npix; // one trial's [nwidth][npix]
-    if (ss->snr_cube) {
+    if (cs) {
         const size_t ncube = cube_plane * pl->ndm;
-        k_cube_fill<<<(unsigned)((ncube + 255) / 256), 256, 0, st>>>(ss->snr_cube, ss->toa_cube, ncube);
+        k_cube_fill<<<(unsigned)((ncube + 255) / 256), 256, 0, st>>>(cs, ct, ncube);
         SCU(cudaGetLastError(), "k_cube_fill launch");
         ++*launches;
     }
+    if (running)   // NaN = "this trial has no valid sample yet"
+        SCU(cudaMemsetAsync(ss->sig, 0xff, (size_t)pl->nuniq * pl->npix * sizeof(float), st), "sigma preset");
     for (int b = 0; b < npass; ++b) {
         StreamParams sp;
         sp.ring = ss->ring; sp.mu0 = ss->mu0; sp.partials = ss->partials;
@@ -578,17 +664,25 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         sp.nslice = nslice;
         sp.slice0 = b * c.NSUPER;
         sp.mws = ss->mws; sp.aws = ss->aws; sp.sws = ss->sws;
-        sp.snr_cube = ss->snr_cube; sp.toa_cube = ss->toa_cube; sp.t_offset = (int32_t)(lo & 0x7fffffff);
+        sp.snr_cube = cs; sp.toa_cube = ct; sp.t_offset = (int32_t)(lo & 0x7fffffff);
+        sp.sig_out = running ? ss->sig : nullptr;
         segment_bounds(pl, c, len, sp.i0, sp.C, sp.bound);
         void *args[] = {&sp};
         dim3 grid((pl->npix + 31) / 32, c.NSUPER);
         SCU(cudaLaunchKernel((const void *)ss->fn[variant], grid, dim3(c.threads()), args, c.smem, st), "k_stream launch");
         ++*launches;
     }
-    if (ss->snr_cube && pl->nuniq < pl->ndm) {
+    if (ss->snr_cube && pl->nuniq < pl->ndm) {   // (the library's own cubes are read for canonical trials only)
         dim3 grid((unsigned)((cube_plane + 255) / 256), pl->ndm);
         k_cube_dups<<<grid, 256, 0, st>>>(ss->snr_cube, ss->toa_cube, ss->d_canon, cube_plane);
         SCU(cudaGetLastError(), "k_cube_dups launch");
+        ++*launches;
+    }
+    if (running) {
+        k_running<<<(pl->npix + 255) / 256, 256, 0, st>>>(cs, ct, ss->sig, ss->var, pl->d_k_of_u, pl->nuniq, pl->nw, pl->npix,
+                                                          pl->run_alpha, ss->var_init ? 0 : 1, pl->run_snr, pl->run_arg);
+        SCU(cudaGetLastError(), "k_running launch");
+        ss->var_init = true;
         ++*launches;
     }
     if (pl->profiling && pl->ev[2]) cudaEventRecord(pl->ev[2], st);

@@ -62,6 +62,7 @@ struct StreamParams {
     // optional per-(trial, width) outputs (S/N and TOA kept for all pixels x widths x DMs), or null:
     float *snr_cube;    // [NDM_ALL][NW_ALL][NPIX] peak S/N of every (dm, width) over this push's windows
     int *toa_cube;      // same shape: its window start (absolute, t_offset added); -1 where no window exists
+    float *sig_out;     // [NU][NPIX] this push's sigma of every unique trial (running-sigma mode), or null
     int t_offset;
 };
 
@@ -462,6 +463,9 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     const float sigma = sqrtf(var);
                     const float rsig = sigma > 0.f ? 1.f / sigma : 0.f; // sigma = 0 => S = 0 (definition)
                     if (P.slice0 == 0 && live) P.mu0[(long long)u * NPIX + pix] = w.mu[V(kk)] + delta;
+#if CUBES
+                    if (P.sig_out && P.slice0 == 0 && live) P.sig_out[(long long)u * NPIX + pix] = sigma;
+#endif
                     sfor<0, SEG>([&](auto q) {
                         const int j0 = rng[(gl * SEG + V(q)) * 2 + 0], j1 = rng[(gl * SEG + V(q)) * 2 + 1];
                         if (j0 >= 0)

@@ -46,7 +46,7 @@ EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stre
            "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
            "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes",
            "nsfrb_psf_mask", "nsfrb_cluster", "nsfrb_median_subtract",
-           "nsfrb_stream_push_host_async", "nsfrb_stream_wait")
+           "nsfrb_stream_push_host_async", "nsfrb_stream_wait", "nsfrb_stream_set_running_sigma")
 
 _lib = None
 
@@ -100,6 +100,8 @@ def lib() -> ctypes.CDLL:
         L.nsfrb_bin_time.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int64, ctypes.c_int, vp, vp]
         L.nsfrb_stream_push_host_async.restype = ctypes.c_int
         L.nsfrb_stream_push_host_async.argtypes = [vp, vp, ctypes.c_int, vp, vp, vp, ctypes.c_uint32, vp]
+        L.nsfrb_stream_set_running_sigma.restype = ctypes.c_int
+        L.nsfrb_stream_set_running_sigma.argtypes = [vp, ctypes.c_double, vp, vp]
         L.nsfrb_stream_wait.restype = ctypes.c_int
         L.nsfrb_stream_wait.argtypes = [vp]
         L.nsfrb_median_subtract.restype = ctypes.c_int
@@ -327,6 +329,22 @@ class Plan:
 
     def stream_reset(self):
         _check(lib().nsfrb_stream_reset(self._h))
+
+    def stream_set_running_sigma(self, alpha: float, snr_map_run: torch.Tensor | None, argmax_run: torch.Tensor | None):
+        """nsfrb_stream_set_running_sigma: every later push also writes the maps normalised by the running standard
+        deviation (float32 [npix], int32 [3][npix]); None, None switches the mode off.  The tensors must stay alive."""
+        if snr_map_run is None and argmax_run is None:
+            _check(lib().nsfrb_stream_set_running_sigma(self._h, float(alpha), None, None))
+            self._running = None
+            return
+        ok = (snr_map_run is not None and argmax_run is not None and snr_map_run.is_cuda and argmax_run.is_cuda
+              and snr_map_run.dtype == torch.float32 and argmax_run.dtype == torch.int32
+              and snr_map_run.is_contiguous() and argmax_run.is_contiguous()
+              and snr_map_run.numel() == self.npix and tuple(argmax_run.shape) == (3, self.npix))
+        if not ok:
+            raise ValueError("expected contiguous CUDA tensors float32 [npix] and int32 [3][npix]")
+        _check(lib().nsfrb_stream_set_running_sigma(self._h, float(alpha), snr_map_run.data_ptr(), argmax_run.data_ptr()))
+        self._running = (snr_map_run, argmax_run)
 
     def cluster(self, snr_map: torch.Tensor, argmax: torch.Tensor, psf: torch.Tensor, mask: torch.Tensor, topn: int = 10,
                 stream=None) -> ClusterResult:

@@ -537,3 +537,85 @@ def test_pipelined_host_pushes_equal_device_pushes():
         pb.stream_push(chunks[0], ref)
         torch.cuda.synchronize()
         assert np.array_equal(o[0].numpy(), ref.snr_map.cpu().numpy())
+
+
+def _check_running(wl, d, out_snr, out_arg, ores, inst, var, label):
+    """Running-sigma maps vs RunningStreamOracle: S/N within tol; arg-max exact where the oracle's winner beats every
+    other (trial, width) maximum by more than 2 tol, otherwise the GPU's cell is adjudicated by the oracle:
+    S_run(cell) = snr_at(cell) * sigma_inst / sigma_run must be within 2 tol of the oracle's maximum."""
+    snr = out_snr.cpu().numpy()
+    arg = out_arg.cpu().numpy().T
+    tol = 1e-4 + 1e-4 * np.abs(ores.snr)
+    defined = ores.argmax[:, 0] >= 0
+    assert np.array_equal(arg[:, 0] >= 0, defined), label
+    assert np.all(np.isneginf(snr[~defined]))
+    assert np.all(np.abs(snr[defined] - ores.snr[defined]) <= tol[defined]), label
+    flat = np.sort(ores.best.reshape(ores.best.shape[0], -1), axis=1)
+    margin = flat[:, -1] - flat[:, -2]
+    adjudicated = 0
+    for p in np.nonzero(defined)[0]:
+        if tuple(arg[p]) == tuple(ores.argmax[p]):
+            continue
+        assert margin[p] <= 2 * tol[p] or arg[p, 0] == ores.argmax[p, 0] and arg[p, 1] == ores.argmax[p, 1], (label, p)
+        k, j, t = (int(x) for x in arg[p])
+        s_inst = oracle.snr_at(inst["hist"], d, wl.width_list, p, k, j, t, raw_end_min=inst["raw_end_min"], t_offset=inst["lo"])
+        s_run = s_inst * inst["sigma"][p, k] / np.sqrt(var[p, k])
+        assert abs(s_run - ores.snr[p]) <= 2 * tol[p], (label, p)
+        adjudicated += 1
+    return adjudicated
+
+
+@pytest.mark.parametrize("alpha,own_cubes,dup", [(0.1, False, False), (0.5, True, False), (1.0, False, True)])
+def test_stream_running_sigma_matches_oracle(alpha, own_cubes, dup):
+    from dataclasses import replace
+    nsfrb = _nsfrb()
+    wl = W.config("c1")
+    if dup:
+        wl = replace(wl, dm_list=np.asarray([400.0, 0.0, 400.0, 1000.0, 0.0, 1400.0]))
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    n_push = 6
+    src = W.ChunkSource(wl, d, n_push, "cuda")
+    so = oracle.RunningStreamOracle(wl.nchan, wl.npix, wl.nt, d, wl.width_list, alpha)
+    plain = oracle.StreamOracle(wl.nchan, wl.npix, wl.nt, d, wl.width_list)
+    total_adj = 0
+    with nsfrb.Plan.for_workload(wl) as plan:
+        out = plan.alloc_outputs()
+        rs = torch.zeros(wl.npix, device="cuda")
+        ra = torch.zeros((3, wl.npix), dtype=torch.int32, device="cuda")
+        if own_cubes:
+            shape = (len(wl.dm_list), len(wl.width_list), wl.npix)
+            cs, ct = torch.zeros(shape, device="cuda"), torch.zeros(shape, dtype=torch.int32, device="cuda")
+            plan.stream_set_cubes(cs, ct)
+        plan.stream_set_running_sigma(alpha, rs, ra)
+        for i in range(n_push):
+            chunk = src.next()
+            if i == 4:
+                chunk[:, 3:19, 77] += 2.5          # a wide bright pulse: this push's own sigma is inflated (L130)
+            plan.stream_push(chunk, out)
+            torch.cuda.synchronize()
+            ch = chunk.cpu().numpy()
+            n_prev = so.n
+            ores = so.push(ch, nthreads=8)
+            pres = plain.push(ch, nthreads=8, details=True)
+            lo = max(0, so.n - so.L)
+            inst = dict(hist=so.hist, raw_end_min=n_prev - lo, lo=lo, sigma=pres.sigma)
+            total_adj += _check_running(wl, d, rs, ra, ores, inst, so.var, f"push {i}")
+            # the plain outputs of the same push are untouched by the mode
+            PU.check(so.hist, d, wl.width_list, out.snr_map.cpu().numpy(), out.argmax.cpu().numpy().T.copy(), wl.threshold,
+                     raw_end_min=n_prev - lo, t_offset=lo, label=f"plain push {i}")
+            if alpha == 1.0:
+                assert np.allclose(rs.cpu().numpy(), out.snr_map.cpu().numpy(), rtol=1e-6, atol=1e-6, equal_nan=True)
+            if i == 4 and alpha < 1.0:
+                assert rs[77].item() > 1.1 * out.snr_map[77].item()      # the bias is (partly) removed
+        assert total_adj <= 0.05 * n_push * wl.npix
+        # reset restarts the running variance: the first push after it equals the plain maps again
+        plan.stream_reset()
+        plan.stream_push(src.next(), out)
+        torch.cuda.synchronize()
+        assert np.allclose(rs.cpu().numpy(), out.snr_map.cpu().numpy(), rtol=1e-6, atol=1e-6, equal_nan=True)
+        # switching the mode off stops the writes
+        plan.stream_set_running_sigma(0.0, None, None)
+        rs.fill_(123.0)
+        plan.stream_push(src.next(), out)
+        torch.cuda.synchronize()
+        assert float(rs.min()) == 123.0
