@@ -31,7 +31,7 @@ from paper_2510_18136_b200 import workloads as W  # noqa: E402
 
 CHUNK_DURATION_MS = 25 * W.TSAMP_S * 1e3  # 3355 ms (25 samples x 134 ms)
 # DRAM bytes (read + write) of one launch of the dominant kernel, from `ncu --set full` (profiles/r01_v3.md)
-NCU_TRAFFIC_BYTES = {"c2": 7.04e9}  # 6.83 GB read + 0.24 GB written
+NCU_TRAFFIC_BYTES = {"c2": 7.04e9}  # 6.84 GB read + 0.20 GB written (profiles/r01_v4_next.md)
 
 
 # ---------------------------------------------------------------------------- helpers
