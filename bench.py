@@ -512,7 +512,7 @@ def run_median_arm(args):
     per_step = time_steps(step, args.steps, args.warmup)
     ms = float(np.mean(per_step)) / ncubes
     nbytes = cubes[0].numel() * 8 + meds.numel() * 4
-    kern = "k_median_reg<32>" if nt <= 32 else "k_median_tile"
+    kern = f"k_median_reg<{nt}>" if nt <= 32 else "k_median_stream"
     print(json.dumps({"metric": "GB/s (median subtraction, NEXT 1)", "value": nbytes / (ms * 1e-3) / 1e9, "unit": "GB/s", "n_gpus": 1,
                       "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
                       "dtype": "f32", "data": "synthetic",

@@ -226,7 +226,7 @@ int nsfrb_bin_time(const float *cube, int nchan, int nt, int64_t npix, int facto
  *   out     device, same shape; may be the same pointer as cube (in place), must not overlap it otherwise
  *   median  device, [nchan][npix] float32, written (may be NULL)
  * Asynchronous on `stream`; one launch.  NSFRB_EINVAL for null pointers, non-positive sizes, nchan > 65535 or
- * nt > 43007 (the series of a tile must fit in shared memory).
+ * nt > 65535 (16-bit histogram counters).
  */
 int nsfrb_median_subtract(const float *cube, int nchan, int nt, int64_t npix, float *out, float *median, void *stream);
 

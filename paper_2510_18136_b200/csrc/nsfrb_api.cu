@@ -680,7 +680,7 @@ int nsfrb_median_subtract(const float *cube, int nchan, int nt, int64_t npix, fl
     if (!cube || !out) return fail(NSFRB_EINVAL, "null pointer");
     if (nchan < 1 || nt < 1 || npix < 1) return fail(NSFRB_EINVAL, "non-positive size");
     if (nchan > 65535) return fail(NSFRB_EINVAL, "too many channels");
-    if (nt > median_max_nt()) return fail(NSFRB_EINVAL, "nt too large for the shared-memory tile (max 43007)");
+    if (nt > median_max_nt()) return fail(NSFRB_EINVAL, "nt too large (max 65535)");
     if ((long long)nchan * npix > 0x7fffffffLL * 256) return fail(NSFRB_EINVAL, "too many series");
     CU(launch_median(cube, out, median, nchan, nt, (long long)npix, static_cast<cudaStream_t>(stream)),
        "k_median launch");

@@ -183,7 +183,6 @@ cudaError_t launch_bin(const float *in, float *out, int nchan, int nt, long long
 // out may alias in; med ([nchan][npix]) may be null; nt <= median_max_nt()
 cudaError_t launch_median(const float *in, float *out, float *med, int nchan, int nt, long long npix, cudaStream_t st);
 int median_max_nt();
-int median_tile_pixels(int nt);
 cudaError_t launch_psf_mask(const float *psf, long long n, long long lo, double frac, uint8_t *mask, double *value,
                             cudaStream_t st);
 int cluster_max_top();

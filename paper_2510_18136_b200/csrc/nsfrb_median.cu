@@ -3,13 +3,11 @@
 //   k_median_reg<NT>  nt <= 32 (the paper's 25-sample chunks): one thread per series (lanes = adjacent pixels, so
 //                     every row access is coalesced), the series in registers, Batcher's odd-even merge network
 //                     specialised at compile time for the exact length and for the two middle outputs.
-//   k_median_tile<P>  longer series: a [P pixels][nt] tile of order-preserving integer keys in shared memory, exact
-//                     radix select of all P series at once (4 passes of 8 bits, shared-memory histograms split over
-//                     32/P sub-histograms per series, one warp scans a series' 256 counters), the upper middle
-//                     element by one more pass (warp per series), subtraction on the way out.
+//   k_median_stream   longer series (<= 65 535 samples): lanes = adjacent pixels again, nothing but lane-private 8-bit
+//                     histograms on chip; three streaming reads of the series (histogram, candidates, subtraction)
+//                     and one write for noise-like data; exact for any data (more histogram passes when a bucket
+//                     stays crowded).
 #include "nsfrb_internal.h"
-
-#include <cstdlib>
 
 namespace nsfrb {
 namespace {
@@ -113,144 +111,155 @@ __global__ void __launch_bounds__(256) k_median_reg(const float *in, float *out,
     }
 }
 
-constexpr int kTileThreads = 512;
-constexpr int kHistWords = 32 * 256;   // [P][S][256] counters with P*S = 32: 32 KB whatever the tile shape
+// ---- long series, streaming form: lanes = adjacent pixels, one warp = 32 series of one channel.  Nothing but the
+// histograms is kept on chip, so every row access is a coalesced 128-byte line whatever nt and npix are.
+//   pass H (one read of the series): lane-private 8-bit histograms of the keys that match the prefix found so far
+//                                    ([256 bins][32 lanes] 16-bit counters: no atomics, no bank conflicts);
+//                                    repeated on the next 8 bits only while some series still has > kCap matching keys
+//   pass C (one read):               the <= kCap matching keys of every series go to shared memory (over the histograms),
+//                                    together with the smallest key above the bucket; exact selection among them
+//   pass W (one read, one write):    out = x - median
+// Noise-like data needs H, C, W: three reads and one write (2x the minimal traffic), all of it streaming.
+constexpr int kMsWarps = 4;
+constexpr int kCap = 128;                       // candidate keys per series: [kCap][32] uint32 = the 16 KB of the histograms
+constexpr int kMsSmemPerWarp = 256 * 32 * 2;    // bytes
 
-template <int P>
-__global__ void __launch_bounds__(kTileThreads) k_median_tile(const float *in, float *out,   // may alias
-                                                              float *__restrict__ med, int nt, long long npix,
-                                                              int stride)
+// f(x, t) for t = 0..nt-1 over one series (row stride npix), with the loads of the next kMsU rows already requested
+// while the current kMsU are processed (two register batches: up to 64 rows in flight per lane).
+constexpr int kMsU = 16;
+template <class F>
+__device__ __forceinline__ void for_rows(const float *src, int nt, long long npix, F &&f)
 {
-    constexpr int S = 32 / P;            // sub-histograms per series (lanes spread over them: fewer same-bin conflicts)
+    float a[kMsU], b[kMsU];
+    const int nb = nt / kMsU;
+    const float *q = src;              // running pointer: rows are requested strictly in order
+    auto load = [&](float (&x)[kMsU], int) {
+#pragma unroll
+        for (int i = 0; i < kMsU; ++i) {
+            x[i] = *q;
+            q += npix;
+        }
+    };
+    auto run = [&](const float (&x)[kMsU], int t0) {
+#pragma unroll
+        for (int i = 0; i < kMsU; ++i) f(x[i], t0 + i);
+    };
+    if (nb > 0) load(a, 0);
+    for (int ib = 0; ib < nb; ib += 2) {
+        if (ib + 1 < nb) load(b, (ib + 1) * kMsU);
+        run(a, ib * kMsU);
+        if (ib + 1 < nb) {
+            if (ib + 2 < nb) load(a, (ib + 2) * kMsU);
+            run(b, (ib + 1) * kMsU);
+        }
+    }
+    for (int t = nb * kMsU; t < nt; ++t) f(src[(long long)t * npix], t);
+}
+
+__global__ void __launch_bounds__(kMsWarps * 32, 3) k_median_stream(const float *in, float *out,   // may alias
+                                                                 float *__restrict__ med, int nt, long long npix,
+                                                                 int blocks_per_chan, long long nwork)
+{
     extern __shared__ uint32_t smem_u32[];
-    uint32_t *hist = smem_u32;           // [P][S][256]
-    uint32_t *keys = smem_u32 + kHistWords;   // [P][stride], stride odd
-    __shared__ uint32_t s_prefix[P];
-    __shared__ int s_k[P];
-    __shared__ float smed[P];
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int NW = kTileThreads / 32;
-    const long long c = blockIdx.y, p0 = (long long)blockIdx.x * P;
-    const int np = (int)min((long long)P, npix - p0);
-    const float *src = in + c * nt * npix + p0;
-    const int total = nt * P;
-    // asynchronous 4-byte copies straight into the transposed tile: no register dependence, so a thread keeps all of
-    // its loads in flight (rows of P pixels are neither 16-byte aligned nor a multiple of 16 bytes in general)
-    {
-        const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(keys);
-        for (int idx = tid; idx < total; idx += kTileThreads) {
-            const int t = idx / P, p = idx % P;
-            if (p < np)
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sbase + 4u * (uint32_t)(p * stride + t)),
-                             "l"(src + (long long)t * npix + p)
-                             : "memory");
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    }
-    for (int i = tid; i < kHistWords; i += kTileThreads) hist[i] = 0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long work = (long long)blockIdx.x * kMsWarps + warp;    // (channel, block of 32 pixels)
+    if (work >= nwork) return;
+    uint16_t *hist = reinterpret_cast<uint16_t *>(smem_u32 + warp * (kMsSmemPerWarp / 4));   // [256][32]
+    uint32_t *cand = smem_u32 + warp * (kMsSmemPerWarp / 4);                                 // [kCap][32], same bytes
+    const long long c = work / blocks_per_chan, p = (work - c * blocks_per_chan) * 32 + lane;
+    const bool live = p < npix;
+    const float *src = in + c * nt * npix + (live ? p : 0);
     const int k1 = (nt - 1) >> 1, k2 = nt >> 1;
-    if (tid < P) {
-        s_prefix[tid] = 0;
-        s_k[tid] = k1;
-    }
-    asm volatile("cp.async.wait_group 0;" ::: "memory");
-    __syncthreads();
-    // ---- exact order statistic k1 of every series: 4 passes of 8 bits, all warps over all series
-    for (int pass = 0; pass < 4; ++pass) {
-        const int shift = 24 - 8 * pass;
-        // P >= 16 (short series): a warp per series; P <= 8 (long series): the whole CTA walks one series at a time.
-        // Pass 0 also turns the float bits the copies delivered into order-preserving keys, in place.
-        const int pstep = P >= 16 ? NW : 1, tstep = P >= 16 ? 32 : kTileThreads;
-        for (int p = P >= 16 ? warp : 0; p < np; p += pstep) {
-            uint32_t *row = keys + p * stride;
-            uint32_t *hp = hist + ((p * S + (lane & (S - 1))) << 8);
-            const uint32_t prefix = s_prefix[p];
-            if (pass == 0) {
-#pragma unroll 4
-                for (int t = P >= 16 ? lane : tid; t < nt; t += tstep) {
-                    const uint32_t key = ord_key(__uint_as_float(row[t]));
-                    row[t] = key;
-                    atomicAdd(hp + (key >> 24), 1u);
-                }
-            } else {
-#pragma unroll 4
-                for (int t = P >= 16 ? lane : tid; t < nt; t += tstep) {
-                    const uint32_t key = row[t];
-                    if (((key ^ prefix) >> (shift + 8)) == 0u) atomicAdd(hp + ((key >> shift) & 255u), 1u);
-                }
+    uint32_t prefix = 0;
+    int nbits = 0;                 // leading key bits already fixed
+    int k = k1;                    // rank of the wanted key among the keys that match the prefix
+    int count = live ? nt : 0;     // how many keys match the prefix
+    // ---- pass H, as often as needed
+    while (__any_sync(0xffffffffu, count > kCap && nbits < 32)) {
+        for (int i = lane; i < 256 * 32 / 2; i += 32) reinterpret_cast<uint32_t *>(hist)[i] = 0;
+        __syncwarp();
+        const int shift = 24 - nbits;
+        const bool all = nbits == 0;
+        const bool on = live && nbits < 32;
+        if (on)
+            for_rows(src, nt, npix, [&](float x, int) {
+                const uint32_t key = ord_key(x);
+                if (all || ((key ^ prefix) >> (shift + 8)) == 0u) ++hist[((key >> shift) & 255u) * 32 + lane];
+            });
+        __syncwarp();
+        if (on) {                  // the bin that holds rank k
+            int run = 0, b = 0, h = 0;
+            for (; b < 256; ++b) {
+                h = hist[b * 32 + lane];
+                if (k < run + h) break;
+                run += h;
             }
+            prefix |= (uint32_t)b << shift;
+            k -= run;
+            count = h;
         }
-        __syncthreads();
-        for (int p = warp; p < np; p += NW) {      // lane l owns digits 8l..8l+7
-            uint32_t cnt[8];
-            uint32_t tot = 0;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                uint32_t v = 0;
-#pragma unroll
-                for (int q = 0; q < S; ++q) {
-                    uint32_t *h = &hist[((p * S + q) << 8) + 8 * lane + i];
-                    v += *h;
-                    *h = 0;
-                }
-                cnt[i] = v;
-                tot += v;
-            }
-            uint32_t incl = tot;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t x = __shfl_up_sync(0xffffffffu, incl, o);
-                if (lane >= o) incl += x;
-            }
-            const uint32_t excl = incl - tot, k = (uint32_t)s_k[p];
-            if (excl <= k && k < incl) {
-                uint32_t run = excl;
-                int d = 0;
-                bool found = false;
-#pragma unroll
-                for (int i = 0; i < 8; ++i)
-                    if (!found) {
-                        if (k < run + cnt[i]) {
-                            found = true;
-                            d = i;
-                        } else
-                            run += cnt[i];
-                    }
-                s_prefix[p] |= (uint32_t)(8 * lane + d) << shift;
-                s_k[p] = (int)(k - run);
-            }
-        }
-        __syncthreads();
+        nbits += 8;                // (uniform: every series of the warp moves on together)
+        __syncwarp();
     }
-    // ---- even nt: the next order statistic (same value if it repeats, else the next key up); the median
-    for (int p = warp; p < np; p += NW) {
-        const uint32_t *row = keys + p * stride;
-        const uint32_t prefix = s_prefix[p];
-        uint32_t hi = prefix;
-        if (k2 != k1) {
+    // ---- pass C: candidates and the smallest key above the bucket
+    const bool undecided = live && nbits < 32;
+    uint32_t key1 = prefix, key2 = prefix;
+    if (__any_sync(0xffffffffu, undecided) || k2 != k1) {
+        const uint32_t hi_bound = nbits >= 32 ? prefix : (prefix | (0xffffffffu >> nbits));   // largest key of the bucket
+        uint32_t nxt = 0xffffffffu;
+        int n = 0;
+        if (live)
+            for_rows(src, nt, npix, [&](float x, int) {
+                const uint32_t key = ord_key(x);
+                if (key > hi_bound) nxt = min(nxt, key);
+                else if (undecided && (nbits == 0 || ((key ^ prefix) >> (32 - nbits)) == 0u)) cand[(n++) * 32 + lane] = key;
+            });
+        if (undecided) {           // exact selection among the n <= kCap candidates: the remaining bits, one at a time
+            const int r = k;
+            uint32_t pfx = prefix;
+            for (int b = 31 - nbits; b >= 0; --b) {
+                int cnt = 0;
+                for (int i = 0; i < n; ++i) cnt += ((cand[i * 32 + lane] ^ pfx) >> b) == 0u;
+                if (k >= cnt) {
+                    k -= cnt;
+                    pfx |= 1u << b;
+                }
+            }
+            key1 = pfx;
             int le = 0;
-            uint32_t nxt = 0xffffffffu;
-            for (int t = lane; t < nt; t += 32) {
-                const uint32_t q = row[t];
-                le += q <= prefix;
-                nxt = q > prefix ? min(nxt, q) : nxt;
+            uint32_t up = 0xffffffffu;
+            for (int i = 0; i < n; ++i) {
+                const uint32_t q = cand[i * 32 + lane];
+                le += q <= key1;
+                up = q > key1 ? min(up, q) : up;
             }
-            le = __reduce_add_sync(0xffffffffu, le);
-            nxt = __reduce_min_sync(0xffffffffu, nxt);
-            if (le <= k2) hi = nxt;
-        }
-        if (lane == 0) {
-            const float m = middle(ord_val(prefix), ord_val(hi));
-            smed[p] = m;
-            if (med) med[c * npix + p0 + p] = m;
+            key2 = r + 1 < le ? key1 : (up != 0xffffffffu ? up : nxt);
+        } else {                   // all 32 bits fixed: `count` keys equal key1, the wanted one is the k-th of them
+            key2 = k + 1 < count ? key1 : nxt;
         }
     }
-    __syncthreads();
-    float *dst = out + c * nt * npix + p0;
-    for (int idx = tid; idx < total; idx += kTileThreads) {
-        const int t = idx / P, p = idx % P;
-        if (p < np) dst[(long long)t * npix + p] = ord_val(keys[p * stride + t]) - smed[p];
+    if (!live) return;
+    const float m = k2 != k1 ? middle(ord_val(key1), ord_val(key2)) : ord_val(key1);
+    if (med) med[c * npix + p] = m;
+    // ---- pass W
+    float *dst = out + c * nt * npix + p;
+    for_rows(src, nt, npix, [&](float x, int t) { dst[(long long)t * npix] = x - m; });
+}
+
+cudaError_t launch_stream(const float *in, float *out, float *med, int nchan, int nt, long long npix, cudaStream_t st)
+{
+    const size_t smem = (size_t)kMsWarps * kMsSmemPerWarp;
+    static bool granted_dev[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!granted_dev[dev & 63]) {
+        cudaError_t e = cudaFuncSetAttribute(k_median_stream, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        granted_dev[dev & 63] = true;
     }
+    const long long bpc = (npix + 31) / 32, nwork = bpc * nchan;
+    k_median_stream<<<(unsigned)((nwork + kMsWarps - 1) / kMsWarps), kMsWarps * 32, smem, st>>>(in, out, med, nt, npix, (int)bpc, nwork);
+    return cudaGetLastError();
 }
 
 template <int NT>
@@ -261,38 +270,9 @@ cudaError_t launch_reg(const float *in, float *out, float *med, int nchan, long 
     return cudaGetLastError();
 }
 
-template <int P>
-cudaError_t launch_tile(const float *in, float *out, float *med, int nchan, int nt, long long npix, int stride,
-                        cudaStream_t st)
-{
-    const size_t smem = ((size_t)P * stride + kHistWords) * sizeof(uint32_t);
-    static size_t granted_dev[64] = {};   // only ever raised (another call may be using the kernel concurrently)
-    int dev = 0;
-    cudaGetDevice(&dev);
-    size_t &granted = granted_dev[dev & 63];
-    if (smem > 48 * 1024 && smem > granted) {
-        cudaError_t e = cudaFuncSetAttribute(k_median_tile<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        granted = smem;
-    }
-    dim3 grid((unsigned)((npix + P - 1) / P), (unsigned)nchan);
-    k_median_tile<P><<<grid, kTileThreads, smem, st>>>(in, out, med, nt, npix, stride);
-    return cudaGetLastError();
-}
-
 } // namespace
 
-int median_max_nt() { return ((200 - 32) * 1024 / 4 - 1) | 1; }
-
-int median_tile_pixels(int nt)
-{
-    const int stride = nt | 1;
-    int p = 32;
-    if (const char *e = getenv("NSFRB_MEDIAN_P")) return atoi(e);
-    while (p > 8 && (size_t)p * stride * 4 > (72 - 32) * 1024) p >>= 1;   // three CTAs per SM while rows stay >= 32 bytes
-    while (p > 1 && (size_t)p * stride * 4 > (200 - 32) * 1024) p >>= 1;  // (32 KB of every CTA are the histograms)
-    return p;
-}
+int median_max_nt() { return 65535; }   // 16-bit histogram counters of k_median_stream
 
 cudaError_t launch_median(const float *in, float *out, float *med, int nchan, int nt, long long npix, cudaStream_t st)
 {
@@ -308,15 +288,7 @@ cudaError_t launch_median(const float *in, float *out, float *med, int nchan, in
 #undef NSFRB_MEDIAN_REG
     default: break;
     }
-    const int stride = nt | 1;
-    switch (median_tile_pixels(nt)) {
-    case 32: return launch_tile<32>(in, out, med, nchan, nt, npix, stride, st);
-    case 16: return launch_tile<16>(in, out, med, nchan, nt, npix, stride, st);
-    case 8: return launch_tile<8>(in, out, med, nchan, nt, npix, stride, st);
-    case 4: return launch_tile<4>(in, out, med, nchan, nt, npix, stride, st);
-    case 2: return launch_tile<2>(in, out, med, nchan, nt, npix, stride, st);
-    default: return launch_tile<1>(in, out, med, nchan, nt, npix, stride, st);
-    }
+    return launch_stream(in, out, med, nchan, nt, npix, st);
 }
 
 } // namespace nsfrb

@@ -164,7 +164,7 @@ def test_cluster_after_stream_push():
 @pytest.mark.parametrize("nchan,nt,npix", [
     (1, 1, 1), (2, 2, 33), (3, 3, 77), (2, 5, 300), (2, 8, 64), (1, 16, 1000), (2, 17, 129), (16, 25, 1024),
     (2, 31, 95), (2, 32, 257), (2, 33, 257), (3, 64, 100), (2, 100, 77), (1, 257, 65), (2, 1000, 90), (2, 2048, 75),
-    (1, 2304, 40), (1, 4097, 21), (1, 16384, 7), (1, 30000, 3), (1, 43007, 2)])
+    (1, 2304, 40), (1, 4097, 21), (1, 16384, 7), (1, 30000, 3), (1, 43007, 2), (1, 65535, 1)])
 def test_median_subtract_matches_oracle(nchan, nt, npix):
     nsfrb = _nsfrb()
     rng = np.random.default_rng(nt * 131 + npix)
@@ -196,12 +196,37 @@ def test_median_subtract_every_register_length():
         assert np.array_equal(out.cpu().numpy(), want), nt
 
 
+@pytest.mark.parametrize("nt", [130, 1000, 4096, 5001])
+def test_median_subtract_crowded_buckets(nt):
+    """Series whose keys crowd one histogram bucket force the extra histogram passes of k_median_stream: a large
+    offset (all keys share the top byte, then the second), constants (all 32 bits decided, multiplicity > the candidate
+    capacity), two-valued series whose two middle elements sit in different buckets, lanes that need different numbers
+    of passes in one warp, and non-finite-free extremes."""
+    nsfrb = _nsfrb()
+    rng = np.random.default_rng(nt)
+    npix = 70
+    a = rng.normal(size=(2, nt, npix)).astype(np.float32)
+    a[0, :, 0:8] += 1000.0                                   # top two bytes shared
+    a[0, :, 8:12] = a[0, :, 8:12] * 1e-3 + 65536.0           # only the low mantissa bits differ
+    a[0, :, 12] = 3.25                                        # constant
+    a[0, :, 13] = np.where(np.arange(nt) < nt // 2, -1.0, 2.0)     # even nt: the middle pair straddles two buckets
+    a[0, :, 14] = np.where(np.arange(nt) % 3 == 0, 1e-30, 1e30)
+    a[0, :, 15] = np.round(a[0, :, 15])                       # few distinct values, heavy ties
+    a[1, :, 5] = np.float32(1.5e38) * np.sign(a[1, :, 5])     # near +-FLT_MAX / 2
+    a[1, : nt // 2, 6] = 0.0
+    a[1, nt // 2:, 6] = -0.0
+    want, wmed = oracle.median_subtract(a)
+    out, med = nsfrb.median_subtract(torch.from_numpy(a).cuda())
+    assert np.array_equal(med.cpu().numpy(), wmed)
+    assert np.array_equal(out.cpu().numpy(), want)
+
+
 def test_median_subtract_rejects_bad_arguments():
     nsfrb = _nsfrb()
     L = nsfrb.lib()
     d = torch.zeros((1, 4, 4), device="cuda")
     assert L.nsfrb_median_subtract(d.data_ptr(), 1, 0, 4, d.data_ptr(), None, None) == nsfrb.NSFRB_EINVAL
-    assert L.nsfrb_median_subtract(d.data_ptr(), 1, 43008, 4, d.data_ptr(), None, None) == nsfrb.NSFRB_EINVAL
+    assert L.nsfrb_median_subtract(d.data_ptr(), 1, 65536, 4, d.data_ptr(), None, None) == nsfrb.NSFRB_EINVAL
     assert L.nsfrb_median_subtract(None, 1, 4, 4, d.data_ptr(), None, None) == nsfrb.NSFRB_EINVAL
 
 
