@@ -48,6 +48,17 @@ struct StreamParams {
     int32_t *toa_cube;
     float *sig_out;
     int32_t t_offset;
+    const float *dlt;  // INCR: exact mean minus its float rounding, and 1/sigma, per (unique trial, pixel)
+    const float *rsig;
+};
+
+// host mirror of k_stream_stats's parameter block (nsfrb_stream_kernel.cuh)
+struct StatsParams {
+    const float *ring;
+    double *s1, *s2;
+    float *mu, *dlt, *rsig, *sig_out;
+    int32_t row_lo, add, first, pad;
+    long long ring_lo, lo_prev, n_prev, lo, n;
 };
 
 struct StreamCfg {
@@ -55,6 +66,9 @@ struct StreamCfg {
     int PFD = 6;                                    // L2 prefetch distance in tiles
     int CMAX = 25;                                  // ends per pass (shared-memory budget)
     int NW = 0, NSUPER = 1;
+    float light_cost = 0.25f;                       // cost of a light tile relative to a plain dedispersion tile (segment balance)
+    int LIGHT = 1;                                  // INCR only: plain runs are summed once for all trials of a thread (light tiles)
+    int INCR = 1;                                   // 1: mean/sigma kept incrementally by k_stream_stats (the march stops at the last start range)
     size_t smem = 0;
     int threads() const { return 32 * GPC * SEG; }
 };
@@ -75,9 +89,23 @@ bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamC
     c = StreamCfg();
     c.NW = std::max(pl->nw_used, 1);
     int kk = 8, gpc = 2, seg = 2, tt = 2, minb = 3, pfd = 6;
+    {
+        const char *e = getenv("NSFRB_STREAM_STATS"); // "march": the march itself accumulates mean and variance over the whole ring (round-1 v4 behaviour)
+        c.INCR = (e && std::strcmp(e, "march") == 0) ? 0 : 1;
+        if (const char *lt = getenv("NSFRB_STREAM_LIGHT")) c.LIGHT = atoi(lt) != 0;
+        if (!c.INCR) c.LIGHT = 0;
+        if (const char *lc = getenv("NSFRB_STREAM_LIGHT_COST")) c.light_cost = (float)atof(lc);
+    }
     if (pl->nchan > 24) { // the thread holds nchan*TT raw rows in registers: one time step per tile, more registers
         tt = 1;
         minb = 2;
+    } else if (c.LIGHT) {
+        // light tiles wait on memory, not on the issue slots, and a second time segment only adds its imbalance: one
+        // segment per CTA (64-thread CTAs, up to 255 registers) with four steps per tile measured best on C2
+        // (k_stream 2.38 ms against 2.72 ms for SEG=2, TT=2)
+        seg = 1;
+        tt = 4;
+        minb = 4;
     }
     if (variant && *variant) {
         if (sscanf(variant, "%d,%d,%d,%d,%d,%d", &kk, &gpc, &seg, &tt, &minb, &pfd) < 4) {
@@ -108,7 +136,10 @@ bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamC
             }
             carry = std::max(carry, s);
         }
-        if (pl->nchan * tt + carry + kk * (tt + 4) + 36 > 165) minb = std::min(minb, 2);
+        // fewer CTAs per SM while the estimate exceeds the registers a thread may have at that residency
+        const int est = pl->nchan * tt + carry + kk * (tt + 4) + 36;
+        const int threads = 32 * std::min(gpc, ngroups) * seg;
+        while (minb > 1 && est > std::min(255, 65536 / (minb * threads)) - 5) --minb;
     }
     c.KK = kk; c.GPC = gpc; c.SEG = seg; c.TT = tt; c.PFD = std::max(0, std::min(pfd, 24 / tt)); // the ring's guard rows cover 24 rows of look-ahead
     c.NSUPER = (ngroups + gpc - 1) / gpc;
@@ -141,7 +172,7 @@ std::string make_prologue(const nsfrb_plan *pl, const StreamCfg &c)
     std::string s = "// generated by nsfrb_stream.cu for one plan\n";
     auto def = [&](const char *n, long long v) { s += "#define " + std::string(n) + " " + std::to_string(v) + "\n"; };
     def("NPIX", pl->npix); def("NCHAN", pl->nchan); def("NU", pl->nuniq); def("KK", c.KK); def("GPC", c.GPC);
-    def("SEG", c.SEG); def("TT", c.TT); def("NW", c.NW); def("CMAX", c.CMAX); def("NSUPER", c.NSUPER); def("MINB", c.MINB); def("PFD", c.PFD); def("NW_ALL", pl->nw); def("ROWS", 2 * (pl->dmax_all + 40) + 2 * pl->nt);
+    def("SEG", c.SEG); def("TT", c.TT); def("NW", c.NW); def("CMAX", c.CMAX); def("NSUPER", c.NSUPER); def("MINB", c.MINB); def("PFD", c.PFD); def("INCR", c.INCR); def("LIGHT", c.LIGHT); def("NW_ALL", pl->nw); def("ROWS", 2 * (pl->dmax_all + 40) + 2 * pl->nt);
     s += "static __device__ constexpr short D_TAB[NU][NCHAN] = {";
     for (int u = 0; u < pl->nuniq; ++u) {
         s += u ? ",{" : "{";
@@ -267,9 +298,14 @@ struct StreamState {
     StreamCfg cfg;
     cudaLibrary_t lib[2] = {nullptr, nullptr}; // [0] plain, [1] with the cube outputs compiled in
     cudaKernel_t fn[2] = {nullptr, nullptr};
+    cudaKernel_t fn_stats[2] = {nullptr, nullptr}; // k_stream_stats of the same module (INCR)
     float *ring = nullptr; // [pixel block][G + 2L + G][nchan][32]
     float *base = nullptr; // [nchan][npix]  first sample ever, removed from every stored sample
     float *mu0 = nullptr;  // [nuniq][npix]
+    // incremental statistics (k_stream_stats): float64 sums of D and D^2 over the valid samples of every (unique trial,
+    // pixel), and what k_stream's reduction needs of them
+    double *st1 = nullptr, *st2 = nullptr;
+    float *dlt = nullptr, *rsig = nullptr;
     SPartial *partials = nullptr;
     float *mws = nullptr;  // running maxima per (pixel block, supergroup, trial, width, lane)
     int32_t *aws = nullptr;
@@ -319,6 +355,8 @@ __global__ void __launch_bounds__(256) k_stream_push(const V *__restrict__ chunk
         dst[(size_t)L * nchan * kPer] = v;
     }
 }
+
+
 
 __device__ __forceinline__ bool sbetter(const SPartial &a, const SPartial &b)
 {
@@ -421,7 +459,10 @@ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 // Segment boundaries of one pass: multiples of TT, >= the end zone, never inside a width's start range.
 void segment_bounds(const nsfrb_plan *pl, const StreamCfg &c, int len, int i0, int C, int32_t bound[9])
 {
-    const int Rtot = std::max(0, len - pl->dmin_all);
+    int Rtot = std::max(0, len - pl->dmin_all);
+    // INCR: mean and sigma come from k_stream_stats, so nothing lies beyond the last start range (own step
+    // w + i0 + C - 1 of the widest width; a trial's group step is never ahead of its own step)
+    if (c.INCR) Rtot = std::min(Rtot, std::max(pl->wmax_used, 0) + i0 + C);
     const int Rceil = round_up(Rtot, c.TT);
     for (int q = 0; q <= 8; ++q) bound[q] = Rceil;
     bound[0] = 0;
@@ -442,10 +483,12 @@ void segment_bounds(const nsfrb_plan *pl, const StreamCfg &c, int len, int i0, i
     for (int t = 0; t < ntile; ++t) {
         const int r0 = t * c.TT + 1, r1 = (t + 1) * c.TT + spread; // own-frame steps the tile can touch
         float cost = 1.f + (r0 <= i0 + C ? 0.5f : 0.f);
+        bool met = r0 <= i0 + C;
         for (int i = 0; i < pl->nw_used; ++i) {
             const int a = pl->widths_used[i] + i0, z = a + C - 1;
-            if (a <= r1 && z >= r0) cost += 0.7f;
+            if (a <= r1 && z >= r0) { cost += 0.7f; met = true; }
         }
+        if (c.LIGHT && !met) cost = c.light_cost; // a light tile (plain run): the trials share one sum of the rows
         cum[t + 1] = cum[t] + cost;
     }
     for (int q = 1; q < c.SEG; ++q) {
@@ -493,6 +536,7 @@ int stream_kernel(nsfrb_plan *pl, StreamState *ss, int cubes, std::string &err)
     SCU(cudaLibraryGetKernel(&ss->fn[cubes], ss->lib[cubes], "k_stream"), "cudaLibraryGetKernel(k_stream)");
     SCU(cudaFuncSetAttribute((const void *)ss->fn[cubes], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ss->cfg.smem),
         "k_stream shared-memory attribute");
+    if (ss->cfg.INCR) SCU(cudaLibraryGetKernel(&ss->fn_stats[cubes], ss->lib[cubes], "k_stream_stats"), "cudaLibraryGetKernel(k_stream_stats)");
     return NSFRB_OK;
 }
 
@@ -510,6 +554,14 @@ int stream_init(nsfrb_plan *pl, int chunk_nt, std::string &err)
     const size_t mu_b = (size_t)pl->nuniq * pl->npix * sizeof(float);
     SCU(cudaMalloc(reinterpret_cast<void **>(&ss->mu0), mu_b), "mu0 alloc");
     SCU(cudaMemset(ss->mu0, 0, mu_b), "mu0 clear");
+    size_t st_b = 0;
+    if (ss->cfg.INCR) {
+        st_b = 2 * mu_b * 2 + 2 * mu_b;
+        SCU(cudaMalloc(reinterpret_cast<void **>(&ss->st1), 2 * mu_b), "statistics alloc");
+        SCU(cudaMalloc(reinterpret_cast<void **>(&ss->st2), 2 * mu_b), "statistics alloc");
+        SCU(cudaMalloc(reinterpret_cast<void **>(&ss->dlt), mu_b), "statistics alloc");
+        SCU(cudaMalloc(reinterpret_cast<void **>(&ss->rsig), mu_b), "statistics alloc");
+    }
     const size_t m_b = (size_t)((pl->npix + 31) / 32) * ss->cfg.NSUPER * ss->cfg.GPC * ss->cfg.KK * ss->cfg.NW * 32 * sizeof(float);
     SCU(cudaMalloc(reinterpret_cast<void **>(&ss->mws), m_b), "maxima workspace alloc");
     SCU(cudaMalloc(reinterpret_cast<void **>(&ss->aws), m_b), "arg workspace alloc");
@@ -530,7 +582,7 @@ int stream_init(nsfrb_plan *pl, int chunk_nt, std::string &err)
     }
     ss->snr_cube = pl->cube_snr;
     ss->toa_cube = pl->cube_toa;
-    ss->bytes = ring_b + row * sizeof(float) + mu_b + 2 * m_b + s_b;
+    ss->bytes = ring_b + row * sizeof(float) + mu_b + 2 * m_b + s_b + st_b;
     return NSFRB_OK;
 }
 
@@ -541,6 +593,7 @@ void stream_free(nsfrb_plan *p)
     if (!p || !p->stream) return;
     StreamState *ss = p->stream;
     cudaFree(ss->ring); cudaFree(ss->base); cudaFree(ss->mu0); cudaFree(ss->partials); cudaFree(ss->mws); cudaFree(ss->aws); cudaFree(ss->sws); cudaFree(ss->d_canon);
+    cudaFree(ss->st1); cudaFree(ss->st2); cudaFree(ss->dlt); cudaFree(ss->rsig);
     cudaFree(ss->sig); cudaFree(ss->var); cudaFree(ss->own_cs); cudaFree(ss->own_ct);
     for (auto &l : ss->lib) if (l) cudaLibraryUnload(l);
     cudaGetLastError();
@@ -615,6 +668,18 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
     const int64_t lo = std::max<int64_t>(0, n - L);
     const int len = (int)(n - lo);
 
+    // ---- a1, a3 (INCR), first half: the samples that leave the valid sets, while their raw rows are still in the ring
+    const int64_t lo_prev = std::max<int64_t>(0, n_prev - L);
+    StatsParams tp;
+    tp.ring = ss->ring; tp.s1 = ss->st1; tp.s2 = ss->st2; tp.mu = ss->mu0; tp.dlt = ss->dlt; tp.rsig = ss->rsig; tp.sig_out = nullptr;
+    tp.pad = 0; tp.lo_prev = lo_prev; tp.n_prev = n_prev; tp.lo = lo; tp.n = n;
+    const dim3 stat_grid((pl->npix + 31) / 32, (pl->nuniq + 7) / 8);
+    if (c.INCR && lo > lo_prev && n_prev > 0) {
+        tp.row_lo = ss->guard + (int)(lo_prev % L); tp.ring_lo = lo_prev; tp.add = 0; tp.first = 0;
+        void *args[] = {&tp};
+        SCU(cudaLaunchKernel((const void *)ss->fn_stats[variant], stat_grid, dim3(256), args, 0, st), "k_stream_stats launch");
+        ++*launches;
+    }
     // ---- a8: ring update
     {
         const bool v4 = (pl->npix % 4 == 0) && ((reinterpret_cast<uintptr_t>(chunk) & 15u) == 0);
@@ -632,6 +697,13 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         ++*launches;
     }
     pl->n_received = n;
+    if (c.INCR) { // second half: the samples that enter; mean, 1/sigma (and sigma itself for the running-sigma mode)
+        tp.row_lo = ss->guard + (int)(lo % L); tp.ring_lo = lo; tp.add = 1; tp.first = n_prev == 0 ? 1 : 0;
+        tp.sig_out = running ? ss->sig : nullptr;
+        void *args[] = {&tp};
+        SCU(cudaLaunchKernel((const void *)ss->fn_stats[variant], stat_grid, dim3(256), args, 0, st), "k_stream_stats launch");
+        ++*launches;
+    }
     if (pl->profiling && pl->ev[1]) cudaEventRecord(pl->ev[1], st);
 
     // ---- k_stream: one pass per batch of CMAX ends
@@ -652,7 +724,7 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         SCU(cudaGetLastError(), "k_cube_fill launch");
         ++*launches;
     }
-    if (running)   // NaN = "this trial has no valid sample yet"
+    if (running && !c.INCR)   // NaN = "this trial has no valid sample yet"
         SCU(cudaMemsetAsync(ss->sig, 0xff, (size_t)pl->nuniq * pl->npix * sizeof(float), st), "sigma preset");
     for (int b = 0; b < npass; ++b) {
         StreamParams sp;
@@ -665,7 +737,8 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         sp.slice0 = b * c.NSUPER;
         sp.mws = ss->mws; sp.aws = ss->aws; sp.sws = ss->sws;
         sp.snr_cube = cs; sp.toa_cube = ct; sp.t_offset = (int32_t)(lo & 0x7fffffff);
-        sp.sig_out = running ? ss->sig : nullptr;
+        sp.sig_out = (running && !c.INCR) ? ss->sig : nullptr;
+        sp.dlt = ss->dlt; sp.rsig = ss->rsig;
         segment_bounds(pl, c, len, sp.i0, sp.C, sp.bound);
         void *args[] = {&sp};
         dim3 grid((pl->npix + 31) / 32, c.NSUPER);

@@ -8,7 +8,7 @@
 // ahead of time with the BASELINE config-2 prologue as a build check.
 //
 // Prologue (see nsfrb_jit.cu: make_stream_prologue):
-//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD NW_ALL CUBES   integers (NW_ALL: length of the caller's width list; CUBES = 1 compiles the cube outputs in)
+//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD INCR LIGHT NW_ALL CUBES   integers (INCR, LIGHT: see StreamParams and Worker::light; NW_ALL: length of the caller's width list; CUBES = 1 compiles the cube outputs in)
 //   D_TAB[NU][NCHAN]   integer delays d[u][c] of the unique trials, DM ascending
 //   DMAX_TAB[NU]       dmax_u                 K_OF_U[NU]  lowest original dm index of the trial
 //   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index   RSQ_W[NW]  1/sqrt(width)
@@ -64,6 +64,11 @@ struct StreamParams {
     int *toa_cube;      // same shape: its window start (absolute, t_offset added); -1 where no window exists
     float *sig_out;     // [NU][NPIX] this push's sigma of every unique trial (running-sigma mode), or null
     int t_offset;
+    // INCR = 1: mean and sigma are kept incrementally by k_stream_stats (nsfrb_stream.cu); mu0 then holds the exact mean
+    // rounded to float, dlt the remainder (exact mean - mu0) and rsig = 1/sigma (0 where sigma = 0), all [NU][NPIX];
+    // the march stops after the last start range and accumulates no sum of squares
+    const float *dlt;
+    const float *rsig;
 };
 
 namespace sk {
@@ -217,6 +222,60 @@ template <int G> struct Worker {
         });
     }
 
+
+#if LIGHT
+    // ---- plain runs (no end stored, no start range met): only the suffix sums move.  Over a run of n steps trial kk adds
+    //   sum_c sum_{m = o(kk,c)}^{n-1+o(kk,c)} W_c[m]  =  sum_c sum_{m<n} W_c[m]  +  edge(kk) at the exit  -  edge(kk) at the entry,
+    // W_c[m] the raw window of channel c counted from the run's first row and edge(kk) = sum_c sum_{m<o(kk,c)} W_c[m], the
+    // part of the carried halo below the trial's offset.  The first term is common to the KK trials: a light tile adds
+    // the TT rows that leave the window (NCHAN*TT adds for all trials together) instead of dedispersing every trial.
+    template <int KKI> __device__ __forceinline__ float edge_of() const
+    {
+        float a0 = 0.f, a1 = 0.f;
+        sfor<0, NCHAN>([&](auto c) {
+            sfor<0, T::o(KKI, V(c))>([&](auto m) {
+                if constexpr (((V(c) + V(m)) & 1) == 0) a0 += carry[T::coff(V(c)) + V(m)];
+                else a1 += carry[T::coff(V(c)) + V(m)];
+            });
+        });
+        return a0 + a1;
+    }
+    __device__ __forceinline__ void run_begin()
+    {
+        sfor<0, KK>([&](auto kk) { Q[V(kk)] -= edge_of<V(kk)>(); });
+    }
+    // g: sum of the rows that left, centred on mu[0] per step; n steps
+    __device__ __forceinline__ void run_end(float g, int n)
+    {
+        const float fn = (float)n;
+        float cd = 0.f; // mu[0] - mu[kk]
+        sfor<0, KK>([&](auto kk) {
+            if constexpr (V(kk) > 0) cd += dmu[V(kk)];
+            Q[V(kk)] += (g + edge_of<V(kk)>()) + fn * cd;
+        });
+    }
+    __device__ __forceinline__ void light(float (&cur)[NCHAN * TT], int rb, bool more, bool pf, float &g)
+    {
+        auto Wn = [&](auto c, auto m) -> float {
+            if constexpr (V(m) < T::span(V(c))) return carry[T::coff(V(c)) + V(m)];
+            else return cur[V(c) * TT + (V(m) - T::span(V(c)))];
+        };
+        float a0 = -(float)TT * mu[0], a1 = 0.f, a2 = 0.f, a3 = 0.f;
+        sfor<0, NCHAN>([&](auto c) {
+            sfor<0, TT>([&](auto tt) {
+                const float v = Wn(c, tt);
+                constexpr int sel = (V(c) * TT + V(tt)) & 3;
+                if constexpr (sel == 0) a0 += v; else if constexpr (sel == 1) a1 += v; else if constexpr (sel == 2) a2 += v; else a3 += v;
+            });
+        });
+        sfor<0, NCHAN>([&](auto c) {
+            sfor<0, T::span(V(c))>([&](auto m) { carry[T::coff(V(c)) + V(m)] = Wn(c, IC<V(m) + TT>{}); });
+        });
+        if (more) load_new(cur, rb + TT);
+        if (PFD > 0 && pf) prefetch_l2(rb + PFD * TT);
+        g += (a0 + a1) + (a2 + a3);
+    }
+#endif
     // One tile: group steps rb+1 .. rb+TT.  On entry cur holds the TT new rows of every channel; on exit
     // (if `more`) the rows of the next tile have been requested into the same registers.
     // `cells`: the tile stores ends or meets a start range (one code body serves plain and cell tiles: the
@@ -266,7 +325,9 @@ template <int G> struct Worker {
                     x = (ro >= 1 && ro <= len - DMAX_TAB[T::u(V(kk))]) ? x : 0.f;
                 }
                 Q[V(kk)] += x;
+#if !INCR
                 S2[V(kk)] = fmaf(x, x, S2[V(kk)]);
+#endif
                 Dv[V(kk)][V(tt)] = Q[V(kk)];
             });
         });
@@ -417,6 +478,20 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
             const int fast_stop = r_end < r_fast_end - TT + 1 ? r_end : r_fast_end - TT + 1; // rb < fast_stop <=> tile fully valid
             while (rb < fast_stop) {
                 const bool cells = classify();
+#if LIGHT
+                if (!cells) { // a plain run: up to the tile before the next start range (or the end of the unmasked part)
+                    const int stop = plain_until < fast_stop ? plain_until : fast_stop;
+                    const int rb0 = rb;
+                    float g = 0.f;
+                    w.run_begin();
+                    do {
+                        w.light(cur, rb, rb + TT < r_end, pf, g);
+                        rb += TT;
+                    } while (rb < stop);
+                    w.run_end(g, rb - rb0);
+                    continue;
+                }
+#endif
                 w.template tile<false>(cur, rb, rb + TT < r_end, pf, cells);
                 rb += TT;
             }
@@ -433,7 +508,9 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     // segment totals and the widths this segment evaluated
     sfor<0, KK>([&](auto kk) {
         S1s[((gl * KK + V(kk)) * SEG + seg) * 32 + lane] = w.Q[V(kk)];
+#if !INCR
         S2s[((gl * KK + V(kk)) * SEG + seg) * 32 + lane] = w.S2[V(kk)];
+#endif
     });
     if (lane == 0) {
         rng[(gl * SEG + seg) * 2 + 0] = w.jfirst;
@@ -455,8 +532,15 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     sfor<0, SEG>([&](auto q) {
                         off[V(q)] = s1;
                         s1 += S1s[((gl * KK + V(kk)) * SEG + V(q)) * 32 + lane];
+#if !INCR
                         s2 += S2s[((gl * KK + V(kk)) * SEG + V(q)) * 32 + lane];
+#endif
                     });
+#if INCR
+                    (void)s2;
+                    const float delta = P.dlt[(long long)u * NPIX + pix];
+                    const float rsig = P.rsig[(long long)u * NPIX + pix]; // 0 where sigma = 0 => S = 0 (definition)
+#else
                     const float invT = 1.f / (float)Tk;
                     const float delta = s1 * invT;
                     const float var = fmaxf(fmaf(-delta, delta, s2 * invT), 0.f);
@@ -465,6 +549,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     if (P.slice0 == 0 && live) P.mu0[(long long)u * NPIX + pix] = w.mu[V(kk)] + delta;
 #if CUBES
                     if (P.sig_out && P.slice0 == 0 && live) P.sig_out[(long long)u * NPIX + pix] = sigma;
+#endif
 #endif
                     sfor<0, SEG>([&](auto q) {
                         const int j0 = rng[(gl * SEG + V(q)) * 2 + 0], j1 = rng[(gl * SEG + V(q)) * 2 + 1];
@@ -543,5 +628,109 @@ extern "C" __global__ void __launch_bounds__(sk::kThreads, MINB) k_stream(const 
     const int g = blockIdx.y * GPC + gl; // DM group of this warp; NSUPER*GPC groups exist (the last may be padding)
     sk::dispatch<0, NSUPER * GPC>(g, P, smem, gl, seg, lane, pix, live);
 }
+
+#if INCR
+// a1, a3 kept incrementally: S1 = sum D_u, S2 = sum D_u^2 over the valid samples V_u = [lo, n - dmax_u) of every (unique
+// trial u, pixel), in float64, carried from push to push.  The launch with add = 0 runs BEFORE the ring update and takes
+// out the samples that leave V_u with this push (their raw rows are about to be overwritten); the one with add = 1 runs
+// after it, puts in the samples that enter, and writes what k_stream needs: the mean (as a float, plus the remainder
+// dlt = mean - float(mean)) and 1/sigma (population; 0 where sigma = 0).  A sample's D is formed from
+// the same stored ring values in the same order when it enters and when it leaves, so the two contributions cancel to
+// float64 rounding.  Lane = pixel, warp = trial; the trial's shifts are immediates.
+struct StatsParams {
+    const float *ring;
+    double *s1, *s2;      // [NU][NPIX]
+    float *mu, *dlt, *rsig, *sig_out;
+    int row_lo;           // ring row that holds the raw sample of absolute index ring_lo
+    int add, first, pad;
+    long long ring_lo, lo_prev, n_prev, lo, n;
+};
+
+namespace sk {
+
+template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &P, int lane, int pix, bool live)
+{
+    constexpr long long dm = DMAX_TAB[U];
+    const long long b_prev = P.lo_prev > P.n_prev - dm ? P.lo_prev : P.n_prev - dm; // end of the previous valid set
+    long long ta, tb;
+    if (P.add) {
+        ta = b_prev > P.lo ? b_prev : P.lo;
+        tb = P.lo > P.n - dm ? P.lo : P.n - dm;
+    } else {
+        ta = P.lo_prev;
+        tb = P.lo < b_prev ? P.lo : b_prev;
+    }
+    const float *rp = P.ring + ((long long)blockIdx.x * ROWS + P.row_lo + (ta - P.ring_lo)) * (NCHAN * 32) + lane;
+    double a1 = 0.0, a2 = 0.0;
+    int i = (int)(tb - ta);
+    // (a sample's D is the same expression in both loops: it must not depend on where the sample falls in a range)
+    for (; i >= 4; i -= 4, rp += 4 * NCHAN * 32) { // four samples per round: 4*NCHAN loads in flight
+        float e[4][4] = {};
+        sfor<0, 4>([&](auto q) {
+            sfor<0, NCHAN>([&](auto c) { e[V(q)][V(c) & 3] += __ldg(rp + ((D_TAB[U][V(c)] + V(q)) * NCHAN + V(c)) * 32); });
+        });
+        sfor<0, 4>([&](auto q) {
+            const double D = (double)((e[V(q)][0] + e[V(q)][1]) + (e[V(q)][2] + e[V(q)][3]));
+            a1 += D;
+            a2 = fma(D, D, a2);
+        });
+    }
+    for (; i > 0; --i, rp += NCHAN * 32) {
+        float e[4] = {0.f, 0.f, 0.f, 0.f};
+        sfor<0, NCHAN>([&](auto c) { e[V(c) & 3] += __ldg(rp + (D_TAB[U][V(c)] * NCHAN + V(c)) * 32); });
+        const double D = (double)((e[0] + e[1]) + (e[2] + e[3]));
+        a1 += D;
+        a2 = fma(D, D, a2);
+    }
+    if (!live) return;
+    const long long o = (long long)U * NPIX + pix;
+    if (!P.add) {
+        if (tb > ta) { P.s1[o] -= a1; P.s2[o] -= a2; }
+        return;
+    }
+    if (!P.first) { a1 += P.s1[o]; a2 += P.s2[o]; }
+    P.s1[o] = a1;
+    P.s2[o] = a2;
+    const long long Tk = tb - P.lo; // tb = max(lo, n - dmax_u)
+    float m = 0.f, dl = 0.f, rs = 0.f, sg = __int_as_float(0x7fc00000); // NaN sigma = "no valid sample yet"
+    if (Tk >= 1) {
+        const double mean = a1 / (double)Tk, msq = a2 / (double)Tk;
+        double var = msq - mean * mean;
+        if (!(var > msq * 1e-13)) var = 0.0; // below the cancellation floor of the float64 sums: a constant series
+        const double sigma = sqrt(var);
+        m = (float)mean;
+        dl = (float)(mean - (double)m);
+        rs = sigma > 0.0 ? (float)(1.0 / sigma) : 0.f;
+        sg = (float)sigma;
+    }
+    P.mu[o] = m;
+    P.dlt[o] = dl;
+    P.rsig[o] = rs;
+    if (P.sig_out) P.sig_out[o] = sg;
+}
+
+template <int U0, int N> __device__ __forceinline__ void stats_dispatch(int u, const StatsParams &P, int lane, int pix, bool live)
+{
+    if constexpr (N == 1) {
+        stats_trial<U0>(P, lane, pix, live);
+    } else {
+        if (u < U0 + N / 2) stats_dispatch<U0, N / 2>(u, P, lane, pix, live);
+        else stats_dispatch<U0 + N / 2, N - N / 2>(u, P, lane, pix, live);
+    }
+}
+
+} // namespace sk
+
+extern "C" __global__ void __launch_bounds__(256) k_stream_stats(const StatsParams P)
+{
+    const int lane = threadIdx.x & 31;
+    const int u = blockIdx.y * 8 + (threadIdx.x >> 5);
+    if (u >= NU) return;
+    int pix = blockIdx.x * 32 + lane;
+    const bool live = pix < NPIX;
+    if (!live) pix = NPIX - 1;
+    sk::stats_dispatch<0, NU>(u, P, lane, pix, live);
+}
+#endif
 
 #endif
