@@ -30,8 +30,8 @@ sys.path.insert(0, ROOT)
 from paper_2510_18136_b200 import workloads as W  # noqa: E402
 
 CHUNK_DURATION_MS = 25 * W.TSAMP_S * 1e3  # 3355 ms (25 samples x 134 ms)
-# DRAM bytes (read + write) of one launch of the dominant kernel, from `ncu --set full` (profiles/r01_v3.md)
-NCU_TRAFFIC_BYTES = {"c2": 7.04e9}  # 6.84 GB read + 0.20 GB written (profiles/r01_v4_next.md)
+# DRAM bytes (read + write) of one launch of the dominant kernel, from `ncu --set full`
+NCU_TRAFFIC_BYTES = {"c2": 5.73e9}  # 5.56 GB read + 0.18 GB written by one k_stream launch (profiles/r01_v5.md)
 
 
 # ---------------------------------------------------------------------------- helpers
