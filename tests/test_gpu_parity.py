@@ -197,6 +197,61 @@ def test_stream_equals_offline_on_ring_contents():
     assert np.all(np.abs(s_stream - r.snr) <= PU.tol(r.snr))
 
 
+
+def test_stream_incremental_statistics_offsets_many_laps_and_reset(monkeypatch):
+    """k_stream_stats carries float64 sums of D and D^2 across pushes.  Twelve laps of a short ring with
+    irregular chunk sizes, on data whose level jumps far away from the first sample (the stored baseline) and then drifts,
+    so the mean square is ~10^3 times the variance: every evaluated push must still match the two-pass float64 oracle,
+    also after nsfrb_stream_reset (the sums restart).  The v4 march (NSFRB_STREAM_STATS=march: one-pass float32 sums about
+    the previous push's mean) must agree with it once it has a provisional mean, i.e. from the second push on; on the very
+    first push of such data it is off by 1.3 tolerances, which is one reason it is no longer the default."""
+    from dataclasses import replace
+    nsfrb = _nsfrb()
+    wl = replace(W.config("c2").scaled(7, 5, nt=200), width_list=np.asarray([1, 3, 9, 30, 100, 180], np.int32))
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    sizes = [25, 3, 25, 11, 40, 1]
+    g = torch.Generator(device="cuda").manual_seed(77)
+    level = 30.0 * torch.randn((wl.nchan, 1, wl.npix), device="cuda", generator=g)
+    chunks, t0 = [], 0
+    for i in range(140):
+        c = sizes[i % len(sizes)]
+        t = torch.arange(t0, t0 + c, device="cuda", dtype=torch.float32).view(1, c, 1)
+        x = torch.randn((wl.nchan, c, wl.npix), device="cuda", generator=g)
+        x = x + (level + 0.002 * t) * (t >= 1)          # sample 0 stays at noise level: it becomes the baseline
+        chunks.append(x.contiguous())
+        t0 += c
+    eval_at = {0, 1, 5, 9, 10, 33, 70, 100, 120, 139}
+
+    def run(order, check=True):
+        maps = {}
+        with nsfrb.Plan.for_workload(wl, cand_capacity=64) as plan:
+            out = plan.alloc_outputs()
+            for rep in order:
+                hist, n = np.zeros((wl.nchan, 0, wl.npix), np.float32), 0
+                if rep:
+                    plan.stream_reset()
+                for i, ch in enumerate(chunks if rep == 0 else chunks[:40]):
+                    plan.stream_push(ch, out)
+                    n_prev, n = n, n + ch.shape[1]
+                    hist = np.concatenate([hist, ch.cpu().numpy()], axis=1)[:, -wl.nt:, :]
+                    if i in eval_at:
+                        torch.cuda.synchronize()
+                        lo = max(0, n - wl.nt)
+                        snr = out.snr_map.cpu().numpy()
+                        arg = out.argmax.cpu().numpy().T.copy()
+                        if check:
+                            PU.check(hist, d, wl.width_list, snr, arg, wl.threshold, raw_end_min=n_prev - lo, t_offset=lo,
+                                     label=f"offsets rep {rep} push {i}")
+                        maps[(rep, i)] = snr
+        return maps
+
+    incr = run([0, 1])
+    monkeypatch.setenv("NSFRB_STREAM_STATS", "march")
+    march = run([0], check=False)
+    for (rep, i), snr in march.items():
+        if i >= 1:
+            assert np.all(np.abs(snr - incr[(rep, i)]) <= 2 * PU.tol(snr)), (rep, i)
+
 # ----------------------------------------------------------------------------- edge and degenerate cases
 def test_degenerate_pixels_and_duplicate_unsorted_dms():
     from dataclasses import replace
