@@ -551,29 +551,45 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     if (P.sig_out && P.slice0 == 0 && live) P.sig_out[(long long)u * NPIX + pix] = sigma;
 #endif
 #endif
-                    sfor<0, SEG>([&](auto q) {
-                        const int j0 = rng[(gl * SEG + V(q)) * 2 + 0], j1 = rng[(gl * SEG + V(q)) * 2 + 1];
-                        if (j0 >= 0)
-                            for (int j = j0; j <= j1; ++j) {
-                                const float m = w.mg[(V(kk) * NW + j) * 32];
-                                if (m > -kInf) {
-                                    const int wj = W_TAB[j];
-                                    const float B = fmaf(-(float)wj, delta, m + off[V(q)]);
-                                    const float S = (B * RSQ_W[j]) * rsig; // RSQ_W[j] = 1/sqrt(w_j), correctly rounded
-                                    const int ii = P.i0 + w.ag[(V(kk) * NW + j) * 32];
-                                    const int t = Tk - ii - wj;
-                                    if (better(S, K_OF_U[u], J_OF_W[j], t, bs, bk, bj, bt)) { bs = S; bk = K_OF_U[u]; bj = J_OF_W[j]; bt = t; }
+                    // the running maxima of all widths of the trial come back from the workspace in one batch of
+                    // independent loads (a width nobody visited holds stale values: read, then ignored) -- one round
+                    // trip per trial instead of two dependent ones per (trial, width)
+                    constexpr int JB = NW < 32 ? NW : 32; // widths per batch
+                    sfor<0, (NW + JB - 1) / JB>([&](auto jb) {
+                    constexpr int jlo = V(jb) * JB, jn = NW - jlo < JB ? NW - jlo : JB;
+                    float mv[JB];
+                    int av[JB];
+                    sfor<0, jn>([&](auto j) {
+                        mv[V(j)] = w.mg[(V(kk) * NW + jlo + V(j)) * 32];
+                        av[V(j)] = w.ag[(V(kk) * NW + jlo + V(j)) * 32];
+                    });
+                    sfor<0, jn>([&](auto jc) {
+                        constexpr int j = jlo + V(jc);
+                        bool has = false; // did a segment evaluate the width (a width belongs to one segment)?
+                        float offj = 0.f;
+                        sfor<0, SEG>([&](auto q) {
+                            const int j0 = rng[(gl * SEG + V(q)) * 2 + 0], j1 = rng[(gl * SEG + V(q)) * 2 + 1];
+                            if (j0 >= 0 && j >= j0 && j <= j1) { has = true; offj = off[V(q)]; }
+                        });
+                        const float m = mv[V(jc)];
+                        if (has && m > -kInf) {
+                            constexpr int wj = W_TAB[j];
+                            const float B = fmaf(-(float)wj, delta, m + offj);
+                            const float S = (B * RSQ_W[j]) * rsig; // RSQ_W[j] = 1/sqrt(w_j), correctly rounded
+                            const int ii = P.i0 + av[V(jc)];
+                            const int t = Tk - ii - wj;
+                            if (better(S, K_OF_U[u], J_OF_W[j], t, bs, bk, bj, bt)) { bs = S; bk = K_OF_U[u]; bj = J_OF_W[j]; bt = t; }
 #if CUBES
-                                    if (P.snr_cube && live) { // cube entry: max over the passes of a push, ties to the smaller t
-                                        const long long ci = ((long long)K_OF_U[u] * NW_ALL + J_OF_W[j]) * NPIX + pix;
-                                        if (P.slice0 == 0 || S >= P.snr_cube[ci]) {
-                                            P.snr_cube[ci] = S;
-                                            P.toa_cube[ci] = (int)(((unsigned)P.t_offset + (unsigned)t) & 0x7fffffffu);
-                                        }
-                                    }
-#endif
+                            if (P.snr_cube && live) { // cube entry: max over the passes of a push, ties to the smaller t
+                                const long long ci = ((long long)K_OF_U[u] * NW_ALL + J_OF_W[j]) * NPIX + pix;
+                                if (P.slice0 == 0 || S >= P.snr_cube[ci]) {
+                                    P.snr_cube[ci] = S;
+                                    P.toa_cube[ci] = (int)(((unsigned)P.t_offset + (unsigned)t) & 0x7fffffffu);
                                 }
                             }
+#endif
+                        }
+                    });
                     });
                 }
             }
