@@ -522,18 +522,21 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     float bs = -kInf;
     int bk = -1, bj = -1, bt = -1;
     if (seg == 0) {
-        sfor<0, KK>([&](auto kk) {
-            constexpr int u = G * KK + V(kk);
-            if constexpr (u < NU) {
+        // (a real loop over the thread's trials, tables indexed at run time: this code runs once per march, and
+        // unrolled over KK trials x NW widths it was 150 KB of instructions fetched for a single pass)
+#pragma unroll 1
+        for (int kk = 0; kk < KK; ++kk) {
+            const int u = G * KK + kk;
+            if (u < NU) {
                 const int Tk = P.len - DMAX_TAB[u];
                 if (Tk >= 1) {
                     float off[SEG];
                     float s1 = 0.f, s2 = 0.f;
                     sfor<0, SEG>([&](auto q) {
                         off[V(q)] = s1;
-                        s1 += S1s[((gl * KK + V(kk)) * SEG + V(q)) * 32 + lane];
+                        s1 += S1s[((gl * KK + kk) * SEG + V(q)) * 32 + lane];
 #if !INCR
-                        s2 += S2s[((gl * KK + V(kk)) * SEG + V(q)) * 32 + lane];
+                        s2 += S2s[((gl * KK + kk) * SEG + V(q)) * 32 + lane];
 #endif
                     });
 #if INCR
@@ -546,7 +549,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     const float var = fmaxf(fmaf(-delta, delta, s2 * invT), 0.f);
                     const float sigma = sqrtf(var);
                     const float rsig = sigma > 0.f ? 1.f / sigma : 0.f; // sigma = 0 => S = 0 (definition)
-                    if (P.slice0 == 0 && live) P.mu0[(long long)u * NPIX + pix] = w.mu[V(kk)] + delta;
+                    if (P.slice0 == 0 && live) P.mu0[(long long)u * NPIX + pix] += delta; // (still the value loaded into w.mu at the start)
 #if CUBES
                     if (P.sig_out && P.slice0 == 0 && live) P.sig_out[(long long)u * NPIX + pix] = sigma;
 #endif
@@ -560,8 +563,8 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     float mv[JB];
                     int av[JB];
                     sfor<0, jn>([&](auto j) {
-                        mv[V(j)] = w.mg[(V(kk) * NW + jlo + V(j)) * 32];
-                        av[V(j)] = w.ag[(V(kk) * NW + jlo + V(j)) * 32];
+                        mv[V(j)] = w.mg[(kk * NW + jlo + V(j)) * 32];
+                        av[V(j)] = w.ag[(kk * NW + jlo + V(j)) * 32];
                     });
                     sfor<0, jn>([&](auto jc) {
                         constexpr int j = jlo + V(jc);
@@ -593,7 +596,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     });
                 }
             }
-        });
+        }
         red[(gl * 32 + lane) * 4 + 0] = bs;
         reinterpret_cast<int *>(red)[(gl * 32 + lane) * 4 + 1] = bk;
         reinterpret_cast<int *>(red)[(gl * 32 + lane) * 4 + 2] = bj;
