@@ -101,11 +101,12 @@ bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamC
         minb = 2;
     } else if (c.LIGHT) {
         // light tiles wait on memory, not on the issue slots, and a second time segment only adds its imbalance: one
-        // segment per CTA (64-thread CTAs, up to 255 registers) with four steps per tile measured best on C2
-        // (k_stream 2.38 ms against 2.72 ms for SEG=2, TT=2)
+        // segment per CTA (64-thread CTAs, up to 255 registers) with three steps per tile and an L2 prefetch distance of
+        // four tiles measured best on C2 (profiles/r01_v5.md)
         seg = 1;
-        tt = 4;
+        tt = 3;
         minb = 4;
+        pfd = 4;
     }
     if (variant && *variant) {
         if (sscanf(variant, "%d,%d,%d,%d,%d,%d", &kk, &gpc, &seg, &tt, &minb, &pfd) < 4) {
