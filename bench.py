@@ -31,7 +31,7 @@ from paper_2510_18136_b200 import workloads as W  # noqa: E402
 
 CHUNK_DURATION_MS = 25 * W.TSAMP_S * 1e3  # 3355 ms (25 samples x 134 ms)
 # DRAM bytes (read + write) of one launch of the dominant kernel, from `ncu --set full`
-NCU_TRAFFIC_BYTES = {"c2": 5.73e9}  # 5.56 GB read + 0.18 GB written by one k_stream launch (profiles/r01_v5.md)
+NCU_TRAFFIC_BYTES = {"c2": 5.58e9}  # 5.40 GB read + 0.18 GB written by one k_stream launch (profiles/r01_v6.md)
 
 
 # ---------------------------------------------------------------------------- helpers

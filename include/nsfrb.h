@@ -112,6 +112,10 @@ int nsfrb_search(nsfrb_plan *plan, const float *cube, void *stream,
  *   arrived in this push are evaluated: n_prev <= t + w_j - 1 + dmax_k < n, t >= lo;
  *   reported t is the absolute sample index since the first push (mod 2^31).
  * 1 <= chunk_nt <= nt.  Outputs as nsfrb_search.
+ * The sums behind mu_k and sigma_k (sum of D_k and of D_k^2 over the valid samples, float64 per trial and pixel) are
+ * plan state carried from push to push: a push adds the samples that enter the valid set and subtracts those that
+ * leave it; nsfrb_stream_reset clears them together with the ring.  The memory they take (24 B per trial and pixel) is
+ * counted in nsfrb_plan_info's workspace_bytes.
  * The first push of a plan compiles the plan-specialised kernel with NVRTC (seconds to a minute, growing with
  * ndm*nchan) and allocates the ring (2*(nt + guard)*nchan*npix*4 B); a compile failure returns NSFRB_ECUDA with
  * the compiler log.  Compiled kernels are cached on disk (NSFRB_JIT_CACHE=<dir>, default /tmp/nsfrb_jit_cache_<uid>, private to the user;
