@@ -32,6 +32,28 @@ def test_duplicate_trials_and_unused_widths_are_dropped_from_the_kernel():
     assert "W_TAB[NW] = {1,5}" in src and "J_OF_W[NW] = {1,0}" in src  # width 400 > ring: no cell, not compiled in
 
 
+def test_default_shape_and_modes_are_in_the_prologue(monkeypatch):
+    """Default: incremental statistics + light tiles, one time segment, three steps per tile (DESIGN.md 5.2);
+    NSFRB_STREAM_STATS=march restores the whole-ring march with the v4 shape; above 24 channels one step per tile."""
+    wl = W.config("c2")
+    src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
+    for d in ("#define INCR 1", "#define LIGHT 1", "#define SEG 1", "#define TT 3", "#define KK 8", "#define GPC 2", "#define PFD 4"):
+        assert d in src, d
+    assert "k_stream_stats" in src
+    monkeypatch.setenv("NSFRB_STREAM_STATS", "march")
+    src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
+    for d in ("#define INCR 0", "#define LIGHT 0", "#define SEG 2", "#define TT 2"):
+        assert d in src, d
+    monkeypatch.delenv("NSFRB_STREAM_STATS")
+    monkeypatch.setenv("NSFRB_STREAM_LIGHT", "0")
+    src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
+    assert "#define INCR 1" in src and "#define LIGHT 0" in src and "#define SEG 2" in src
+    monkeypatch.delenv("NSFRB_STREAM_LIGHT")
+    wl5 = W.config("c5")
+    src = nsfrb.jit_stream_kernel(wl5.nx, wl5.ny, wl5.nchan, 1536, wl5.freqs_GHz, wl5.tsamp_s, wl5.dm_list[:16], wl5.width_list, 25).decode()
+    assert "#define NCHAN 64" in src and "#define TT 1" in src and "#define SEG 2" in src
+
+
 def test_bad_variant_is_rejected():
     wl = W.config("c1")
     with pytest.raises(nsfrb.NsfrbError):
@@ -50,7 +72,9 @@ def test_kernel_cross_compiles_to_sm100a():
         f.write(cubin)
     try:
         out = subprocess.run([cuobjdump, "-res-usage", path], capture_output=True, text=True).stdout
-        assert "Function k_stream" in out
+        assert "Function k_stream:" in out
+        assert "Function k_stream_stats:" in out      # the incremental statistics live in the same module
+        assert " LOCAL:0" in out.split("Function k_stream:")[1].splitlines()[1]   # no register array fell to local memory
         elf = subprocess.run([cuobjdump, "-elf", path], capture_output=True, text=True).stdout
         assert "sm_100a" in elf or "SM100a" in elf or "EF_CUDA_SM100" in elf, elf[:400]
     finally:
