@@ -66,7 +66,7 @@ struct StreamCfg {
     int PFD = 6;                                    // L2 prefetch distance in tiles
     int CMAX = 25;                                  // ends per pass (shared-memory budget)
     int NW = 0, NSUPER = 1;
-    float light_cost = 0.25f;                       // cost of a light tile relative to a plain dedispersion tile (segment balance)
+    float light_cost = 1.0f;                        // time of a light tile relative to a plain dedispersion tile (segment balance): it waits on memory; 1.0 measured best on C2 with SEG=2 (profiles/r01_v5.md)
     int LIGHT = 1;                                  // INCR only: plain runs are summed once for all trials of a thread (light tiles)
     int INCR = 1;                                   // 1: mean/sigma kept incrementally by k_stream_stats (the march stops at the last start range)
     size_t smem = 0;
