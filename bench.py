@@ -565,6 +565,34 @@ def run_cluster_arm(args):
                                    "note": "latency-bound: one launch, three dependent phases"}}))
 
 
+def measure_onchip_peaks(nsfrb_mod, iters=2000):
+    """The achieved on-chip ceilings of this GPU (nsfrb_measure_peaks: FADD/FMNMX/FMNMX3 issue, the search's
+    2 FADD + 1 FMNMX3 cell pair, conflict-free shared-memory streams), with the SM clock derived from the two timings."""
+    pk = nsfrb_mod.measure_peaks(iters)
+    out = {}
+    for name, (per_s, per_clk_sm) in pk.items():
+        out[name] = {"per_s": per_s, "per_clk_per_sm": per_clk_sm,
+                     "implied_sm_mhz": per_s / per_clk_sm / 148 / 1e6 if per_clk_sm > 0 else None}
+    return out
+
+
+def run_peaks_arm(args):
+    """--op peaks: the measured denominators of the offline (alu) roofline."""
+    from paper_2510_18136_b200 import nsfrb
+    torch.cuda.set_device(0)
+    sampler = ClockSampler(0)
+    sampler.start()
+    pk = None
+    t0 = time.perf_counter()
+    while pk is None or time.perf_counter() - t0 < 1.0:   # keep the load up long enough for nvidia-smi to see it
+        pk = measure_onchip_peaks(nsfrb, 4000)
+    clocks = sampler.stop()
+    print(json.dumps({"metric": "T lane-ops/s (FADD issue) and T words/s (shared memory), measured", "unit": "T/s",
+                      "value": pk["fadd"]["per_s"] / 1e12, "n_gpus": 1, "higher_is_better": True, "data": "synthetic",
+                      "config": {"workload": "on-chip peaks: 2 CTAs x 1024 threads per SM, 8 independent chains per thread"},
+                      "peaks": pk, "clocks": clocks}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -576,7 +604,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cubes", action="store_true", help="c2: also write the S/N and TOA cubes every push (NEXT 3)")
     ap.add_argument("--running", action="store_true", help="c2: also the running-sigma maps every push (NEXT 1)")
-    ap.add_argument("--op", default="search", choices=["search", "bin", "cluster", "median"],
+    ap.add_argument("--op", default="search", choices=["search", "bin", "cluster", "median", "peaks"],
                     help="bin: time the binning kernel (NEXT 2); cluster: top-10 + PSF clustering (NEXT 3); "
                          "median: per-pixel median subtraction (NEXT 1)")
     ap.add_argument("--bin-factor", type=int, default=5)
@@ -589,6 +617,9 @@ def main():
     elif args.op == "median" and args.impl == "cuda":
         if rank == 0:
             run_median_arm(args)
+    elif args.op == "peaks" and args.impl == "cuda":
+        if rank == 0:
+            run_peaks_arm(args)
     elif args.op == "cluster" and args.impl == "cuda":
         if rank == 0:
             run_cluster_arm(args)

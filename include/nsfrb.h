@@ -20,8 +20,12 @@
  * smallest (k, j, t) attaining it; candidates = pixels with snr > threshold (strict).
  *
  * Threading: a plan serves one call at a time.  Calls enqueue work on the given stream and
- * return; outputs are valid once the caller has synchronised that stream.  No call
- * synchronises the device except nsfrb_plan_create/destroy and the *_host variants.
+ * return; outputs are valid once the caller has synchronised that stream.  nsfrb_plan_create,
+ * nsfrb_plan_prepare, nsfrb_plan_destroy and the *_host variants synchronise the device; so does
+ * the FIRST nsfrb_search / nsfrb_stream_push of a plan that was not prepared (it compiles the
+ * plan's kernel and allocates its workspaces then); every later call only enqueues.
+ * Every call runs on the device that was current at nsfrb_plan_create, whatever device is
+ * current in the calling thread, and leaves the caller's current device unchanged.
  * Errors: 0 on success, negative code otherwise; nsfrb_last_error() gives the text.
  */
 #ifndef NSFRB_H
@@ -86,6 +90,21 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt,
                       const double *freqs_GHz, double tsamp_s,
                       const double *dm_list, int ndm,
                       const int32_t *width_list, int nwidth, float threshold);
+
+/*
+ * Optional: do now what the first nsfrb_search / nsfrb_stream_push of a plan would otherwise do lazily -- compile the
+ * plan-specialised kernel (NVRTC; seconds to a minute, cached on disk, see NSFRB_JIT_CACHE in DESIGN.md) and allocate
+ * the workspaces -- so that those calls only enqueue work.  PAPER.md:L75: the trial grids and shift tables are fixed and
+ * "loaded onto the GPU" ahead of the search.
+ *   mode NSFRB_PREPARE_SEARCH: offline kernel + two pixel-batch workspaces (about 1 GiB each);
+ *        chunk_nt is ignored
+ *   mode NSFRB_PREPARE_STREAM: real-time kernel for pushes of chunk_nt samples + the ring and its statistics
+ * Synchronises the device (allocation, memset).  Idempotent.  NSFRB_EINVAL for a bad mode or chunk_nt outside [1, nt];
+ * NSFRB_ENOMEM / NSFRB_ECUDA as for the calls it prepares (a compile failure carries the NVRTC log).
+ */
+#define NSFRB_PREPARE_SEARCH 0
+#define NSFRB_PREPARE_STREAM 1
+int nsfrb_plan_prepare(nsfrb_plan *plan, int mode, int chunk_nt);
 
 /*
  * Offline search of one cube (definition at the top of this file).
@@ -290,6 +309,21 @@ int nsfrb_jit_stream_kernel(int nx, int ny, int nchan, int nt, const double *fre
 int nsfrb_jit_search_kernel(int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
                             const double *dm_list, int ndm, const int32_t *width_list, int nwidth,
                             int want_cubin, char *out, size_t capacity, size_t *needed);
+
+/*
+ * Measured on-chip ceilings of the current device, for the offline roofline ("the builder writes two
+ * microbenchmarks (FADD/FMNMX chain; conflict-free LDS stream) and uses the achieved numbers").  Runs one short
+ * kernel per instruction mix on every SM (about 0.1 s in all with iters = 2000); synchronises `stream`.
+ *   nsfrb_peaks_count()   number of tests;  nsfrb_peaks_name(i)  its name (static string, "" out of range):
+ *     fadd, fmnmx, fmnmx3, ffma, fadd2_fmnmx3_pair (two differences + one 3-input maximum, the search's cell pair),
+ *     viaddmnmx, iadd  -- lane-operations issued;   lds32, lds128 -- conflict-free 4-byte words out of shared memory
+ *   per_s        host, [count] float64: operations (or words) per second over the whole GPU, timed with CUDA events
+ *   per_clk_sm   host, [count] float64: the same per SM clock and SM, from clock64 spans of the slowest CTA
+ * NSFRB_EINVAL for null pointers or iters < 1; NSFRB_ECUDA on a CUDA error.
+ */
+int nsfrb_peaks_count(void);
+const char *nsfrb_peaks_name(int test);
+int nsfrb_measure_peaks(int iters, double *per_s, double *per_clk_sm, void *stream);
 
 /* Thread-local text of the last error; never NULL. */
 const char *nsfrb_last_error(void);

@@ -51,7 +51,7 @@ void nsfrb::free_plan(nsfrb_plan *p)
     cudaFree(p->d_cluster_ws);
     for (auto &e : p->ev) if (e) cudaEventDestroy(e);
     stream_free(p);
-    search3_free(p);
+    search4_free(p);
     cudaGetLastError();
     delete p;
 }
@@ -121,12 +121,11 @@ void build_dd_tables(nsfrb_plan *pl)
     pl->tab_cap = round_up(std::max(cap, 4), 4);
 }
 
-// Enqueue search + finalize + compaction over the workspace as it stands.
+// Generic path (plans k_search4 does not take): search + finalize + compaction over the full-size workspace d_W.
 int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offset, cudaStream_t st, float *snr_map,
                int32_t *argmax, nsfrb_cand *cands, uint32_t cap, uint32_t *ncands, int *launches)
 {
-    int slices = (pl->nw_used > 0) ? pl->n_groups * pl->n_wb : 0;
-    bool finalized = false;
+    const int slices = (pl->nw_used > 0) ? pl->n_groups * pl->n_wb : 0;
     if (slices > 0) {
         SearchParams sp;
         sp.W = pl->d_W; sp.delays_u = pl->d_delays_u; sp.dmax_u = pl->d_dmax_u; sp.k_of_u = pl->d_k_of_u;
@@ -135,13 +134,7 @@ int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offse
         sp.origin = origin; sp.len = len; sp.raw_end_min = raw_end_min;
         sp.nuniq = pl->nuniq; sp.nw = pl->nw_used; sp.n_groups = pl->n_groups; sp.n_wb = pl->n_wb;
         sp.H = pl->H; sp.RS = pl->RS; sp.wmax = pl->wmax_used; sp.tab_cap = pl->tab_cap;
-        if (search3_usable(pl)) { // plan-specialised kernel (same algorithm, compiled per plan)
-            std::string err;
-            if (int rc = search3_launch(pl, st, snr_map, argmax, &finalized, err)) return fail(rc, err);
-            slices = search3_slices(pl);
-        } else {
-            CU(launch_search(sp, pl->smem_search, st), "k_search launch");
-        }
+        CU(launch_search(sp, pl->smem_search, st), "k_search launch");
         ++*launches;
     }
     mark(pl, 2, st);
@@ -151,16 +144,49 @@ int run_search(nsfrb_plan *pl, int origin, int len, int raw_end_min, int t_offse
     fp.npix = pl->npix; fp.nchan = pl->nchan; fp.pitch = pl->pitch; fp.ring_L = pl->nt;
     fp.origin = origin; fp.len = len; fp.raw_end_min = raw_end_min; fp.slices = slices; fp.t_offset = t_offset;
     fp.j_of_used = pl->d_j_of_used;
-    if (!finalized) {
-        CU(launch_finalize(fp, pl->smem_final, st), "k_finalize launch");
-        ++*launches;
-    }
+    CU(launch_finalize(fp, pl->smem_final, st), "k_finalize launch");
+    ++*launches;
     mark(pl, 3, st);
     CU(cudaMemsetAsync(ncands, 0, sizeof(uint32_t), st), "memset ncands");
     CU(launch_compact(snr_map, argmax, pl->npix, pl->threshold, cands, cap, ncands, st), "k_compact launch");
     ++*launches;
     mark(pl, 4, st);
     pl->ev_valid = pl->profiling;
+    return NSFRB_OK;
+}
+
+// Calls run on the plan's device whatever device is current in the calling thread; the caller's device is restored.
+struct DeviceGuard {
+    int prev = -1;
+    cudaError_t err = cudaSuccess;
+    explicit DeviceGuard(int dev)
+    {
+        int cur = -1;
+        err = cudaGetDevice(&cur);
+        if (err == cudaSuccess && cur != dev) {
+            err = cudaSetDevice(dev);
+            if (err == cudaSuccess) prev = cur;
+        }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define ON_PLAN_DEVICE(pl)              \
+    DeviceGuard guard__((pl)->device);  \
+    if (guard__.err != cudaSuccess) return fail_cuda(guard__.err, "cudaSetDevice(plan device)")
+
+// full-size time-contiguous copy of the cube (generic path only), allocated on first use
+int ensure_full_workspace(nsfrb_plan *pl)
+{
+    if (pl->d_W) return NSFRB_OK;
+    const size_t wb = (size_t)pl->npix * pl->nchan * (size_t)pl->pitch * sizeof(float);
+    cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&pl->d_W), wb);
+    if (e == cudaSuccess) e = cudaMemset(pl->d_W, 0, wb);
+    if (e != cudaSuccess) {
+        cudaFree(pl->d_W);
+        pl->d_W = nullptr;
+        return e == cudaErrorMemoryAllocation ? fail(NSFRB_ENOMEM, "workspace allocation failed") : fail_cuda(e, "workspace alloc");
+    }
+    pl->workspace_bytes += wb;
     return NSFRB_OK;
 }
 
@@ -365,7 +391,7 @@ int nsfrb::plan_host_init(nsfrb_plan **out, int nx, int ny, int nchan, int nt, c
     pl->n_groups = (pl->nuniq + kSearchWarps - 1) / kSearchWarps;
     pl->n_wb = std::max(1, (pl->nw_used + kWidthBatch - 1) / kWidthBatch);
     pl->H = round_up(std::max(pl->wmax_used, 1) + kBlockLen + 32, 32);
-    {   // a power-of-two ring makes every wrap one AND (k_search3); take it when the shared memory allows
+    {   // a power-of-two ring makes every wrap one AND (generic k_search); take it when the shared memory allows
         int h2 = 32;
         while (h2 < pl->H) h2 <<= 1;
         const int RS0 = round_up(kBlockLen + pl->dmax_all, 4);
@@ -430,6 +456,26 @@ int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const
     return NSFRB_OK;
 }
 
+int nsfrb_plan_prepare(nsfrb_plan *pl, int mode, int chunk_nt)
+{
+    if (!pl) return fail(NSFRB_EINVAL, "plan is null");
+    ON_PLAN_DEVICE(pl);
+    std::string err;
+    if (mode == NSFRB_PREPARE_SEARCH) {
+        if (search4_usable(pl)) {
+            if (int rc = search4_prepare(pl, err)) return fail(rc, err);
+            return NSFRB_OK;
+        }
+        return ensure_full_workspace(pl);
+    }
+    if (mode == NSFRB_PREPARE_STREAM) {
+        if (chunk_nt < 1 || chunk_nt > pl->nt) return fail(NSFRB_EINVAL, "chunk_nt must be in [1, nt]");
+        if (int rc = stream_prepare(pl, chunk_nt, err)) return fail(rc, err);
+        return NSFRB_OK;
+    }
+    return fail(NSFRB_EINVAL, "mode must be NSFRB_PREPARE_SEARCH or NSFRB_PREPARE_STREAM");
+}
+
 int nsfrb_search(nsfrb_plan *pl, const float *cube, void *stream, float *snr_map, int32_t *argmax, nsfrb_cand *cands,
                  uint32_t cand_capacity, uint32_t *ncands)
 {
@@ -438,21 +484,27 @@ int nsfrb_search(nsfrb_plan *pl, const float *cube, void *stream, float *snr_map
     if ((reinterpret_cast<uintptr_t>(cube) & 15u) != 0) return fail(NSFRB_EINVAL, "cube is not 16-byte aligned");
     if (int rc = check_outputs(snr_map, argmax, cands, cand_capacity, ncands)) return rc;
     if (pl->n_received != 0) return fail(NSFRB_ESTATE, "plan holds streamed samples; call nsfrb_stream_reset first");
+    ON_PLAN_DEVICE(pl);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    if (!pl->d_W) { // time-contiguous copy of the cube, allocated on first use
-        const size_t wb = (size_t)pl->npix * pl->nchan * (size_t)pl->pitch * sizeof(float);
-        cudaError_t e = cudaMalloc(reinterpret_cast<void **>(&pl->d_W), wb);
-        if (e == cudaSuccess) e = cudaMemset(pl->d_W, 0, wb);
-        if (e != cudaSuccess) {
-            cudaFree(pl->d_W);
-            pl->d_W = nullptr;
-            return e == cudaErrorMemoryAllocation ? fail(NSFRB_ENOMEM, "workspace allocation failed") : fail_cuda(e, "workspace alloc");
-        }
-        pl->workspace_bytes += wb;
-    }
     int launches = 0;
+    if (search4_usable(pl)) { // plan-specialised kernel over pixel batches; it also writes snr_map/argmax (a6)
+        mark(pl, 0, st);
+        std::string err;
+        if (int rc = search4_launch(pl, cube, st, snr_map, argmax, &launches, (pl->profiling && pl->ev[1]) ? pl->ev[1] : nullptr, err))
+            return fail(rc, err);
+        mark(pl, 2, st);
+        mark(pl, 3, st);
+        CU(cudaMemsetAsync(ncands, 0, sizeof(uint32_t), st), "memset ncands");
+        CU(launch_compact(snr_map, argmax, pl->npix, pl->threshold, cands, cand_capacity, ncands, st), "k_compact launch");
+        ++launches;
+        mark(pl, 4, st);
+        pl->ev_valid = pl->profiling;
+        pl->last_launches = launches;
+        return NSFRB_OK;
+    }
+    if (int rc = ensure_full_workspace(pl)) return rc;
     mark(pl, 0, st);
-    CU(launch_transpose(cube, pl->d_W, pl->npix, pl->nchan, pl->nt, pl->pitch, st), "k_transpose launch");
+    CU(launch_transpose(cube, pl->d_W, pl->npix, pl->nchan, pl->nt, pl->pitch, 0, pl->npix, st), "k_transpose launch");
     ++launches;
     mark(pl, 1, st);
     const int rc = run_search(pl, 0, pl->nt, 0, 0, st, snr_map, argmax, cands, cand_capacity, ncands, &launches);
@@ -468,6 +520,7 @@ int nsfrb_stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, void *st
     if ((reinterpret_cast<uintptr_t>(chunk) & 15u) != 0) return fail(NSFRB_EINVAL, "chunk is not 16-byte aligned");
     if (chunk_nt < 1 || chunk_nt > pl->nt) return fail(NSFRB_EINVAL, "chunk_nt must be in [1, nt]");
     if (int rc = check_outputs(snr_map, argmax, cands, cand_capacity, ncands)) return rc;
+    ON_PLAN_DEVICE(pl);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     int launches = 0;
     mark(pl, 0, st);
@@ -519,6 +572,7 @@ int nsfrb_search_host(nsfrb_plan *pl, const float *cube_host, void *stream, floa
     if (!pl) return fail(NSFRB_EINVAL, "plan is null");
     if (!cube_host) return fail(NSFRB_EINVAL, "cube is null");
     if (int rc = check_outputs(snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host)) return rc;
+    ON_PLAN_DEVICE(pl);
     const size_t bytes = (size_t)pl->nchan * pl->nt * (size_t)pl->npix * sizeof(float);
     if (int rc = ensure_host_staging(pl, bytes, cand_capacity)) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -534,6 +588,7 @@ int nsfrb_stream_push_host(nsfrb_plan *pl, const float *chunk_host, int chunk_nt
     if (!chunk_host) return fail(NSFRB_EINVAL, "chunk is null");
     if (chunk_nt < 1 || chunk_nt > pl->nt) return fail(NSFRB_EINVAL, "chunk_nt must be in [1, nt]");
     if (int rc = check_outputs(snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host)) return rc;
+    ON_PLAN_DEVICE(pl);
     const size_t bytes = (size_t)pl->nchan * chunk_nt * (size_t)pl->npix * sizeof(float);
     if (int rc = ensure_host_staging(pl, bytes, cand_capacity)) return rc;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -552,7 +607,7 @@ int nsfrb_stream_push_host_async(nsfrb_plan *pl, const float *chunk_host, int ch
     if (!chunk_host) return fail(NSFRB_EINVAL, "chunk is null");
     if (chunk_nt < 1 || chunk_nt > pl->nt) return fail(NSFRB_EINVAL, "chunk_nt must be in [1, nt]");
     if (int rc = check_outputs(snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host)) return rc;
-    CU(cudaSetDevice(pl->device), "set device");
+    ON_PLAN_DEVICE(pl);
     const size_t bytes = (size_t)pl->nchan * chunk_nt * (size_t)pl->npix * sizeof(float);
     const int b = pl->pipe ? (int)(pl->pipe->count & 1) : 0;
     if (int rc = pipe_slot(pl, b, bytes, cand_capacity)) return rc;
@@ -609,8 +664,8 @@ int nsfrb_plan_get_info(const nsfrb_plan *pl, nsfrb_plan_info *info)
     info->npix = pl->npix; info->nchan = pl->nchan; info->nt = pl->nt; info->ndm = pl->ndm; info->nwidth = pl->nw;
     info->ndm_unique = pl->nuniq; info->dmax = pl->dmax_all; info->wmax = pl->wmax_used;
     info->n_groups = pl->n_groups; info->n_width_batches = pl->n_wb; info->series_per_cta = kSearchWarps;
-    info->block_len = kBlockLen; info->ring_len = pl->H; info->search_threads = kSearchWarps * 32;
-    info->search_smem_bytes = (int64_t)pl->smem_search; info->workspace_bytes = (int64_t)(pl->workspace_bytes + stream_bytes(pl));
+    info->block_len = kBlockLen; info->ring_len = search4_usable(pl) ? search4_ring_len(pl) : pl->H; info->search_threads = kSearchWarps * 32;
+    info->search_smem_bytes = (int64_t)pl->smem_search; info->workspace_bytes = (int64_t)(pl->workspace_bytes + stream_bytes(pl) + search4_bytes(pl));
     info->cells_per_pixel = pl->cells_per_pixel; info->shift_adds_per_pixel = pl->shift_adds_per_pixel;
     return NSFRB_OK;
 }
@@ -648,7 +703,7 @@ int nsfrb_jit_search_kernel(int nx, int ny, int nchan, int nt, const double *fre
     nsfrb_plan *pl = nullptr;
     if (int rc = plan_host_init(&pl, nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, ndm, width_list, nwidth, 0.f)) return rc;
     std::string src, err;
-    int rc = search3_source(pl, src, err);
+    int rc = search4_source(pl, src, err);
     free_plan(pl);
     if (rc) return fail(rc, err);
     std::vector<char> bin;
@@ -711,7 +766,7 @@ int nsfrb_cluster(nsfrb_plan *pl, const float *snr_map, const int32_t *argmax, c
         return fail(NSFRB_EINVAL, "null pointer");
     if (mh < 1 || mw < 1) return fail(NSFRB_EINVAL, "non-positive PSF size");
     if (topn < 1 || topn > cluster_max_top()) return fail(NSFRB_EINVAL, "topn outside 1..32");
-    CU(cudaSetDevice(pl->device), "set device");
+    ON_PLAN_DEVICE(pl);
     if (!pl->d_cluster_ws) {
         const size_t bytes = 256 + (size_t)cluster_grid(pl->npix) * cluster_max_top() * sizeof(unsigned long long);
         CU(cudaMalloc(&pl->d_cluster_ws, bytes), "cluster workspace");
@@ -724,6 +779,16 @@ int nsfrb_cluster(nsfrb_plan *pl, const float *snr_map, const int32_t *argmax, c
                       static_cast<cudaStream_t>(stream)),
        "k_cluster launch");
     pl->last_launches = 1;
+    return NSFRB_OK;
+}
+
+int nsfrb_peaks_count(void) { return peaks_num_tests(); }
+const char *nsfrb_peaks_name(int test) { return peaks_name(test); }
+int nsfrb_measure_peaks(int iters, double *per_s, double *per_clk_sm, void *stream)
+{
+    if (!per_s || !per_clk_sm) return fail(NSFRB_EINVAL, "null pointer");
+    if (iters < 1) return fail(NSFRB_EINVAL, "iters < 1");
+    CU(measure_peaks(iters, per_s, per_clk_sm, static_cast<cudaStream_t>(stream)), "peak microbenchmarks");
     return NSFRB_OK;
 }
 

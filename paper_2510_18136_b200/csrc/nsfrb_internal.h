@@ -55,7 +55,7 @@ struct SearchParams {
 };
 
 struct StreamState;
-struct Search3State;
+struct Search4State;
 
 struct FinalParams {
     const float *W;
@@ -122,8 +122,8 @@ struct nsfrb_plan {
     float run_alpha = 0.f;       // running-sigma mode (nsfrb_stream_set_running_sigma): caller's outputs, or null = off
     float *run_snr = nullptr;
     int32_t *run_arg = nullptr;
-    // offline path: plan-specialised k_search3 (nsfrb_search_kernel.cuh), compiled at the first nsfrb_search
-    nsfrb::Search3State *search3 = nullptr;
+    // offline path: plan-specialised k_search4 (nsfrb_search_kernel.cuh) + its pixel-batch workspaces (nsfrb_offline.cu)
+    nsfrb::Search4State *search4 = nullptr;
     // pipelined host-buffer pushes (nsfrb_stream_push_host_async): two staging slots, a copy and a compute stream
     struct HostPipe {
         cudaStream_t s_copy = nullptr, s_comp = nullptr;
@@ -148,18 +148,24 @@ int plan_host_init(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const do
                    const double *dm_list, int ndm, const int32_t *width_list, int nwidth, float threshold);
 void free_plan(nsfrb_plan *p);
 
-// ---- plan-specialised offline kernel (nsfrb_stream.cu holds the NVRTC plumbing for both kernels)
-// True if the plan can use k_search3 (at most 32 usable widths; NSFRB_SEARCH_JIT=0 forces the generic k_search).
-bool search3_usable(const nsfrb_plan *pl);
-int search3_source(const nsfrb_plan *pl, std::string &src, std::string &err);
-// compiles on first use; fills pl->d_partials; *finalized = the kernel also wrote snr_map/argmax (fused a6)
-int search3_launch(nsfrb_plan *pl, cudaStream_t st, float *snr_map, int32_t *argmax, bool *finalized, std::string &err);
-void search3_free(nsfrb_plan *p);
-int search3_slices(const nsfrb_plan *pl); // partial records per pixel written by the last search3_launch
+// ---- plan-specialised offline kernel and its batch pipeline (nsfrb_offline.cu)
+// True if the plan can use k_search4 (at most 32 usable widths, tiles fit shared memory; NSFRB_SEARCH_JIT=0 forces the
+// generic k_search).
+bool search4_usable(const nsfrb_plan *pl);
+int search4_source(const nsfrb_plan *pl, std::string &src, std::string &err);
+int search4_prepare(nsfrb_plan *pl, std::string &err); // compile + workspaces; idempotent
+// layout change + one launch per pixel batch; the kernels write snr_map/argmax (fused a6).  ev_layout (may be null) is
+// recorded after the first batch's layout kernel.
+int search4_launch(nsfrb_plan *pl, const float *cube, cudaStream_t st, float *snr_map, int32_t *argmax, int *launches,
+                   cudaEvent_t ev_layout, std::string &err);
+void search4_free(nsfrb_plan *p);
+size_t search4_bytes(const nsfrb_plan *p);
+int search4_ring_len(const nsfrb_plan *pl);
 
 // ---- real-time path (nsfrb_stream.cu)
 void stream_free(nsfrb_plan *p);
 void stream_reset(nsfrb_plan *p);
+int stream_prepare(nsfrb_plan *pl, int chunk_nt, std::string &err); // allocate + compile ahead of the first push
 int stream_set_cubes(nsfrb_plan *pl, float *snr_cube, int32_t *toa_cube, std::string &err);
 int stream_set_running(nsfrb_plan *pl, double alpha, float *snr_run, int32_t *arg_run, std::string &err);
 size_t stream_bytes(const nsfrb_plan *p); // device bytes the real-time path holds (0 before the first push)
@@ -173,7 +179,8 @@ int stream_source(const nsfrb_plan *pl, int chunk_nt, const char *variant, std::
 int stream_compile(const std::string &src, std::vector<char> &cubin, std::string &log);
 
 
-cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, int nt, int pitch,
+// W[p - p_begin][c][t] = cube[c][t][p] - cube[c][0][p] for p in [p_begin, p_begin + p_count)
+cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, int nt, int pitch, int p_begin, int p_count,
                              cudaStream_t st);
 cudaError_t launch_search(const SearchParams &p, size_t smem_bytes, cudaStream_t st);
 cudaError_t launch_finalize(const FinalParams &p, size_t smem_bytes, cudaStream_t st);
@@ -193,6 +200,10 @@ cudaError_t launch_cluster(const float *snr_map, const int32_t *argmax, int npix
                            unsigned int *ticket, nsfrb_cand *top, double *wsnr, int32_t *members, int32_t *result,
                            cudaStream_t st);
 size_t search_smem_bytes(int nchan, int RS, int H, int tab_cap);
+// on-chip ceilings (nsfrb_peaks.cu)
+int peaks_num_tests();
+const char *peaks_name(int t);
+cudaError_t measure_peaks(int iters, double *per_s, double *per_clk_sm, cudaStream_t st);
 size_t final_smem_bytes(int nt);
 
 } // namespace nsfrb

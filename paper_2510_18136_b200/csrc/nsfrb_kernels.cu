@@ -37,26 +37,26 @@ __device__ __forceinline__ bool better(float s, int k, int j, float bs, int bk, 
 // sums at the scale of the fluctuations instead of the sky level.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_transpose(const float *__restrict__ cube, float *__restrict__ W,
-                                                   int npix, int nchan, int nt, int pitch)
+                                                   int npix, int nchan, int nt, int pitch, int p_begin, int p_end)
 {
     // 64 pixels x 64 samples per CTA: 256-byte runs on both the read (pixel-contiguous) and the write
     // (time-contiguous) side; 65-float rows keep both shared-memory phases conflict-free or 2-way
     __shared__ float tile[64][65];
     const int c = blockIdx.z;
-    const int p0 = blockIdx.x * 64, t0 = blockIdx.y * 64;
+    const int p0 = p_begin + blockIdx.x * 64, t0 = blockIdx.y * 64;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const size_t chan0 = (size_t)c * nt * (size_t)npix;
     {
         const int pa = p0 + lane, pb = p0 + 32 + lane;
-        const float ba = (pa < npix) ? __ldg(cube + chan0 + pa) : 0.f;
-        const float bb = (pb < npix) ? __ldg(cube + chan0 + pb) : 0.f;
+        const float ba = (pa < p_end) ? __ldg(cube + chan0 + pa) : 0.f;
+        const float bb = (pb < p_end) ? __ldg(cube + chan0 + pb) : 0.f;
 #pragma unroll 4
         for (int r = warp; r < 64; r += 8) {
             const int t = t0 + r;
             if (t < nt) {
                 const float *row = cube + chan0 + (size_t)t * npix;
-                if (pa < npix) tile[r][lane] = __ldcs(row + pa) - ba;
-                if (pb < npix) tile[r][32 + lane] = __ldcs(row + pb) - bb;
+                if (pa < p_end) tile[r][lane] = __ldcs(row + pa) - ba;
+                if (pb < p_end) tile[r][32 + lane] = __ldcs(row + pb) - bb;
             }
         }
     }
@@ -64,8 +64,8 @@ __global__ void __launch_bounds__(256) k_transpose(const float *__restrict__ cub
 #pragma unroll 4
     for (int r = warp; r < 64; r += 8) {
         const int p = p0 + r;
-        if (p < npix) {
-            float *dst = W + ((size_t)p * nchan + c) * (size_t)pitch + t0;
+        if (p < p_end) {
+            float *dst = W + ((size_t)(p - p_begin) * nchan + c) * (size_t)pitch + t0;
             if (t0 + lane < nt) dst[lane] = tile[lane][r];
             if (t0 + 32 + lane < nt) dst[32 + lane] = tile[32 + lane][r];
         }
@@ -337,10 +337,12 @@ cudaError_t launch_bin(const float *in, float *out, int nchan, int nt, long long
 // ------------------------------------------------------------------------------------------
 size_t final_smem_bytes(int nt) { return ((size_t)nt + 2) * sizeof(float); }
 
-cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, int nt, int pitch, cudaStream_t st)
+cudaError_t launch_transpose(const float *cube, float *W, int npix, int nchan, int nt, int pitch, int p_begin, int p_count,
+                             cudaStream_t st)
 {
-    dim3 grid((npix + 63) / 64, (nt + 63) / 64, nchan), block(256);
-    k_transpose<<<grid, block, 0, st>>>(cube, W, npix, nchan, nt, pitch);
+    if (p_count <= 0) return cudaSuccess;
+    dim3 grid((p_count + 63) / 64, (nt + 63) / 64, nchan), block(256);
+    k_transpose<<<grid, block, 0, st>>>(cube, W, npix, nchan, nt, pitch, p_begin, p_begin + p_count);
     return cudaGetLastError();
 }
 

@@ -1,0 +1,297 @@
+// Offline path of the library (nsfrb_search): the plan-specialised kernel k_search4 (nsfrb_search_kernel.cuh, compiled
+// with NVRTC by nsfrb_plan_prepare or the first nsfrb_search) and the pixel-batch pipeline around it.
+//
+// The cube arrives as [chan][time][pixel]; the search wants one pixel's channels time-contiguous.  Instead of a second
+// cube-sized buffer the plan owns two workspaces of one pixel BATCH each: k_transpose fills the first one, and every
+// k_search4 launch searches batch i out of one workspace while its CTAs move batch i+1 into the other (SIDE, see the
+// kernel), so the layout change of all but the first batch is hidden under the search.  Stream order between the launches
+// is the only synchronisation.
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "nsfrb_internal.h"
+
+namespace nsfrb {
+
+namespace {
+
+const char kSearchKernelSrc[] =
+#include "nsfrb_search_kernel_src.inc"
+    ;
+
+constexpr size_t kSmemLimit = 227 * 1024;
+constexpr int kWmid = 80;       // widths 17..kWmid are served from the ring without a bound (it never prunes them)
+constexpr int kSideTile = 8 * (256 + 4); // floats of the transposing tile (8 pixels x SROWS + 4)
+
+// host mirror of the kernel's parameter block (nsfrb_search_kernel.cuh)
+struct Search4Params {
+    const float *W;
+    Partial *partials;
+    int32_t npix, p0, npb;
+    int32_t *counter;
+    float *snr_map;
+    int32_t *argmax;
+    float *scratch;
+    const float *cube;
+    float *Wn;
+    int32_t n0, nnb;
+};
+
+int env_int(const char *name, int dflt)
+{
+    const char *e = getenv(name);
+    return (e && *e) ? atoi(e) : dflt;
+}
+
+void append_table(std::string &s, const char *decl, const std::vector<int> &v)
+{
+    s += decl;
+    s += " = {";
+    for (size_t i = 0; i < v.size(); ++i) {
+        if (i) s += ",";
+        s += std::to_string(v[i]);
+    }
+    s += "};\n";
+}
+
+int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+} // namespace
+
+struct Search4State {
+    cudaLibrary_t lib = nullptr;
+    cudaKernel_t fn = nullptr;
+    size_t smem = 0;
+    int ngroups = 0;
+    int batch = 0, nbatch = 1; // pixels per batch (a multiple of 8 when nbatch > 1)
+    bool side = false;         // the kernel moves the next batch itself
+    float *W[2] = {nullptr, nullptr};
+    float *scratch = nullptr;   // [grid][16][dpitch] dedispersed series of the items in flight (L2-resident)
+    int grid = 0, dpitch = 0;   // persistent CTAs (one per SM)
+    int32_t *counter = nullptr; // [npix] tickets of the per-pixel reduction
+    size_t bytes = 0;
+};
+
+namespace {
+
+// geometry shared by the prologue and the launch: ring length, shared memory, batch size
+struct Geo {
+    int H, RS, lba, chain, ringt, side, batch, nbatch, ngroups, dpitch, sdir, prune;
+    size_t smem;
+};
+
+// mirrors kSmemFloats of the kernel: raw tile | rings (two planes), 8-slot minima twice, 32-slot minima | results, sums, side tile
+size_t search4_smem(const nsfrb_plan *pl, int H, int RS, int chain, bool side)
+{
+    const size_t nfl = (size_t)pl->nchan * RS + 4 + (size_t)16 * ((H + 16) + 2 * (H / 8) + H / 32) + 16 * 8 +
+                       (size_t)16 * 2 * chain + 16 * 4 + (side ? kSideTile : 0);
+    return nfl * sizeof(float) + 64;
+}
+
+bool search4_geo(const nsfrb_plan *pl, Geo &g)
+{
+    g.ngroups = (pl->nuniq + 15) / 16;
+    // pixel batches: about NSFRB_SEARCH_BATCH_MB (default 1024) of workspace each, at least ~8192 items per launch
+    const size_t bpp = (size_t)pl->nchan * pl->pitch * sizeof(float);
+    const size_t target = (size_t)std::max(1, env_int("NSFRB_SEARCH_BATCH_MB", 1024)) << 20;
+    long long nb = (long long)(target / bpp);
+    nb = std::max<long long>(nb, (8192 + g.ngroups - 1) / g.ngroups);
+    if (env_int("NSFRB_SEARCH_BATCH_PIX", 0) > 0) nb = env_int("NSFRB_SEARCH_BATCH_PIX", 0); // tests: force small batches
+    nb = std::max<long long>(8, nb & ~7LL);
+    if (nb >= pl->npix) { g.batch = pl->npix; g.nbatch = 1; }
+    else { g.batch = (int)nb; g.nbatch = (pl->npix + g.batch - 1) / g.batch; }
+    g.side = (g.nbatch > 1 && env_int("NSFRB_SEARCH_SIDE", 1) != 0) ? 1 : 0;
+    g.sdir = std::max(0, std::min(16, env_int("NSFRB_SEARCH_SDIR", 4)));   // widths up to here are evaluated without a bound
+    g.prune = env_int("NSFRB_SEARCH_PRUNE", 1) != 0;
+    g.dpitch = round_up(pl->nt, 512);
+    // ring: wmax + one block + the rows the bounds read, a multiple of 64; a power of two (every wrap one AND) when shared
+    // memory allows.  Sweep A: 512-sample blocks with one 16-trial chain per thread when the raw tile fits, else 256-sample
+    // blocks (NSFRB_SEARCH_CHAIN=8: two 8-trial chains, all threads busy; 16: one 16-trial chain on half the threads).
+    const int hmin = round_up(std::max(pl->wmax_used, 1) + kBlockLen + 32, 64);
+    int h2 = 64;
+    while (h2 < hmin) h2 <<= 1;
+    struct Shape { int lba, chain; };
+    const int chain256 = env_int("NSFRB_SEARCH_CHAIN", pl->nchan >= 32 ? 16 : 8) == 16 ? 16 : 8;
+    const Shape shapes[2] = {{512, 16}, {256, chain256}};
+    bool ok = false;
+    for (int si = (env_int("NSFRB_SEARCH_LBA", 512) == 512 ? 0 : 1); si < 2 && !ok; ++si)
+        for (int hs = 0; hs < 2 && !ok; ++hs)
+            for (int sd = g.side; sd >= 0 && !ok; --sd) {
+                const int H = hs == 0 ? h2 : hmin, RS = round_up(shapes[si].lba + pl->dmax_all, 4);
+                if (search4_smem(pl, H, RS, shapes[si].chain, sd != 0) <= kSmemLimit) {
+                    g.H = H; g.RS = RS; g.lba = shapes[si].lba; g.chain = shapes[si].chain; g.side = sd;
+                    ok = true;
+                }
+            }
+    if (!ok) return false;
+    g.smem = search4_smem(pl, g.H, g.RS, g.chain, g.side != 0);
+    g.ringt = round_up(pl->nt, kBlockLen) <= g.H ? 1 : 0; // every block of the series fits the ring: nothing is overwritten
+    // the per-pixel reduction of long series rebuilds one prefix series (nt + 2 floats) + 2 words per thread in the same memory
+    const size_t fin = ((size_t)pl->nt + 2 + 2 * 512) * sizeof(float);
+    return g.ringt || fin <= g.smem;
+}
+
+std::string search4_prologue(const nsfrb_plan *pl, const Geo &g)
+{
+    std::string s = "// generated by nsfrb_offline.cu for one plan (offline kernel)\n";
+    auto def = [&](const char *n, long long v) { s += "#define " + std::string(n) + " " + std::to_string(v) + "\n"; };
+    def("NCHAN", pl->nchan); def("NU", pl->nuniq); def("NW", std::max(pl->nw_used, 1)); def("RS", g.RS); def("H", g.H);
+    def("PITCH", pl->pitch); def("DPITCH", g.dpitch); def("NT", pl->nt); def("WMID", std::min(kWmid, g.H - kBlockLen - 32));
+    def("SDIR", g.sdir); def("LBA", g.lba); def("CHAIN", g.chain); def("RINGT", g.ringt); def("SIDE", g.side); def("PRUNE", g.prune);
+    s += "static __device__ constexpr short D_TAB[NU][NCHAN] = {";
+    for (int u = 0; u < pl->nuniq; ++u) {
+        s += u ? ",{" : "{";
+        for (int ch = 0; ch < pl->nchan; ++ch) {
+            if (ch) s += ",";
+            s += std::to_string(pl->delays_u[(size_t)u * pl->nchan + ch]);
+        }
+        s += "}";
+    }
+    s += "};\n";
+    std::vector<int> dmax(pl->dmax_u.begin(), pl->dmax_u.end()), kof(pl->k_of_u.begin(), pl->k_of_u.end());
+    append_table(s, "static __device__ constexpr int DMAX_TAB[NU]", dmax);
+    append_table(s, "static __device__ constexpr int K_OF_U[NU]", kof);
+    std::vector<int> w(pl->widths_used.begin(), pl->widths_used.end());
+    if (w.empty()) w.push_back(0x3fffffff);
+    append_table(s, "static __device__ constexpr int W_TAB[NW]", w);
+    std::vector<int> jw(pl->j_of_used.begin(), pl->j_of_used.end());
+    if (jw.empty()) jw.push_back(0);
+    append_table(s, "static __device__ constexpr int J_OF_W[NW]", jw);
+    return s;
+}
+
+int fail_cuda(cudaError_t e, const char *what, std::string &err)
+{
+    err = std::string(what) + ": " + cudaGetErrorString(e);
+    cudaGetLastError();
+    return e == cudaErrorMemoryAllocation ? NSFRB_ENOMEM : NSFRB_ECUDA;
+}
+#define OCU(call, what)                                              \
+    do {                                                             \
+        cudaError_t e__ = (call);                                    \
+        if (e__ != cudaSuccess) return fail_cuda(e__, what, err);    \
+    } while (0)
+
+} // namespace
+
+bool search4_usable(const nsfrb_plan *pl)
+{
+    const char *e = getenv("NSFRB_SEARCH_JIT");
+    if (e && std::strcmp(e, "0") == 0) return false;
+    Geo g;
+    return pl->nw_used >= 1 && pl->nw_used <= 32 && pl->n_wb == 1 && search4_geo(pl, g);
+}
+
+int search4_source(const nsfrb_plan *pl, std::string &src, std::string &err)
+{
+    Geo g;
+    if (pl->nw_used > 32 || !search4_geo(pl, g)) { err = "k_search4 handles at most 32 usable widths and needs its tiles to fit shared memory"; return NSFRB_EINVAL; }
+    src = search4_prologue(pl, g);
+    src += kSearchKernelSrc;
+    return NSFRB_OK;
+}
+
+void search4_free(nsfrb_plan *p)
+{
+    if (!p || !p->search4) return;
+    if (p->search4->lib) cudaLibraryUnload(p->search4->lib);
+    cudaFree(p->search4->counter);
+    cudaFree(p->search4->scratch);
+    cudaFree(p->search4->W[0]);
+    cudaFree(p->search4->W[1]);
+    cudaGetLastError();
+    delete p->search4;
+    p->search4 = nullptr;
+}
+
+size_t search4_bytes(const nsfrb_plan *p) { return (p && p->search4) ? p->search4->bytes : 0; }
+int search4_ring_len(const nsfrb_plan *pl)
+{
+    Geo g;
+    return search4_geo(pl, g) ? g.H : pl->H;
+}
+
+// Compile the kernel and allocate the batch workspaces (nsfrb_plan_prepare; also the first nsfrb_search).
+int search4_prepare(nsfrb_plan *pl, std::string &err)
+{
+    if (pl->search4) return NSFRB_OK;
+    Geo g;
+    if (!search4_geo(pl, g)) { err = "k_search4 does not fit this plan"; return NSFRB_EINVAL; }
+    Search4State *s4 = new Search4State();
+    pl->search4 = s4;
+    std::string src, log;
+    std::vector<char> cubin;
+    int rc = search4_source(pl, src, err);
+    if (!rc && (rc = stream_compile(src, cubin, log))) err = "k_search4 compile failed: " + log;
+    if (rc) { search4_free(pl); return rc; }
+    s4->ngroups = g.ngroups; s4->smem = g.smem; s4->batch = g.batch; s4->nbatch = g.nbatch; s4->side = g.side != 0;
+    cudaError_t e = cudaLibraryLoadData(&s4->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
+    if (e == cudaSuccess) e = cudaLibraryGetKernel(&s4->fn, s4->lib, "k_search4");
+    if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)s4->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s4->smem);
+    const size_t wb = (size_t)g.batch * pl->nchan * (size_t)pl->pitch * sizeof(float);
+    for (int b = 0; b < (g.nbatch > 1 ? 2 : 1) && e == cudaSuccess; ++b) {
+        e = cudaMalloc(reinterpret_cast<void **>(&s4->W[b]), wb);
+        if (e == cudaSuccess) e = cudaMemset(s4->W[b], 0, wb);
+        if (e == cudaSuccess) s4->bytes += wb;
+    }
+    if (e == cudaSuccess) { // one CTA per SM, each with the dedispersed series of its item in flight
+        int nsm = 0;
+        e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, pl->device);
+        s4->grid = std::max(1, nsm);
+        s4->dpitch = g.dpitch;
+        const size_t sb = (size_t)s4->grid * 16 * g.dpitch * sizeof(float);
+        if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&s4->scratch), sb);
+        if (e == cudaSuccess) e = cudaMemset(s4->scratch, 0, sb);
+        if (e == cudaSuccess) s4->bytes += sb;
+    }
+    if (e == cudaSuccess) {
+        e = cudaMalloc(reinterpret_cast<void **>(&s4->counter), (size_t)pl->npix * sizeof(int32_t));
+        if (e == cudaSuccess) e = cudaMemset(s4->counter, 0, (size_t)pl->npix * sizeof(int32_t));
+        if (e == cudaSuccess) s4->bytes += (size_t)pl->npix * sizeof(int32_t);
+    }
+    if (e != cudaSuccess) {
+        const int code = fail_cuda(e, "k_search4 load / workspace", err);
+        search4_free(pl);
+        return code;
+    }
+    return NSFRB_OK;
+}
+
+// a8-like layout change of the first batch + one k_search4 launch per batch; writes snr_map and argmax
+int search4_launch(nsfrb_plan *pl, const float *cube, cudaStream_t st, float *snr_map, int32_t *argmax, int *launches,
+                   cudaEvent_t ev_layout, std::string &err)
+{
+    if (int rc = search4_prepare(pl, err)) return rc;
+    Search4State *s4 = pl->search4;
+    const int nb = s4->batch;
+    auto count = [&](int i) { return std::min(nb, pl->npix - i * nb); };
+    OCU(launch_transpose(cube, s4->W[0], pl->npix, pl->nchan, pl->nt, pl->pitch, 0, count(0), st), "k_transpose launch");
+    ++*launches;
+    if (ev_layout) cudaEventRecord(ev_layout, st);
+    for (int i = 0; i < s4->nbatch; ++i) {
+        const bool more = i + 1 < s4->nbatch;
+        if (more && !s4->side) {
+            OCU(launch_transpose(cube, s4->W[(i + 1) & 1], pl->npix, pl->nchan, pl->nt, pl->pitch, (i + 1) * nb, count(i + 1), st),
+                "k_transpose launch");
+            ++*launches;
+        }
+        Search4Params sp;
+        sp.W = s4->W[i & 1]; sp.partials = pl->d_partials; sp.npix = pl->npix; sp.p0 = i * nb; sp.npb = count(i);
+        sp.counter = s4->counter; sp.snr_map = snr_map; sp.argmax = argmax; sp.scratch = s4->scratch;
+        sp.cube = cube; sp.Wn = s4->W[(i + 1) & 1];
+        sp.n0 = (i + 1) * nb; sp.nnb = (more && s4->side) ? count(i + 1) : 0;
+        void *args[] = {&sp};
+        const long long blocks = (long long)sp.npb * s4->ngroups;
+        if (blocks <= 0 || blocks > 0x7fffffffLL) { err = "too many CTAs for one launch"; return NSFRB_EINVAL; }
+        OCU(cudaLaunchKernel((const void *)s4->fn, dim3((unsigned)std::min<long long>(blocks, s4->grid)), dim3(512), args, s4->smem, st),
+            "k_search4 launch");
+        ++*launches;
+    }
+    return NSFRB_OK;
+}
+
+} // namespace nsfrb

@@ -25,9 +25,6 @@ namespace {
 const char kStreamKernelSrc[] =
 #include "nsfrb_stream_kernel_src.inc"
     ;
-const char kSearchKernelSrc[] =
-#include "nsfrb_search_kernel_src.inc"
-    ;
 
 struct SPartial {
     float snr;
@@ -633,6 +630,18 @@ int stream_set_running(nsfrb_plan *pl, double alpha, float *snr_run, int32_t *ar
     return NSFRB_OK;
 }
 
+// Ring, statistics and workspaces + the compiled kernel for chunks of chunk_nt samples (nsfrb_plan_prepare).
+int stream_prepare(nsfrb_plan *pl, int chunk_nt, std::string &err)
+{
+    if (!pl->stream) {
+        if (int rc = stream_init(pl, chunk_nt, err)) {
+            stream_free(pl);
+            return rc;
+        }
+    }
+    return stream_kernel(pl, pl->stream, (pl->cube_snr || pl->run_snr) ? 1 : 0, err);
+}
+
 int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t st, float *snr_map, int32_t *argmax,
                 int *launches, std::string &err)
 {
@@ -643,6 +652,20 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         }
     }
     StreamState *ss = pl->stream;
+    if (chunk_nt > ss->cfg.CMAX) {
+        // a longer chunk than the kernel was compiled for would run ceil(chunk_nt / CMAX) passes per push: compile for
+        // the longer one instead (CMAX is the only shape parameter that depends on the chunk; the workspaces do not)
+        StreamCfg c2;
+        std::string e2;
+        if (choose_cfg(pl, chunk_nt, getenv("NSFRB_STREAM_VARIANT"), c2, e2) && c2.CMAX > ss->cfg.CMAX) {
+            SCU(cudaStreamSynchronize(st), "stream sync before the kernel is replaced");
+            for (int v = 0; v < 2; ++v) {
+                if (ss->lib[v]) cudaLibraryUnload(ss->lib[v]);
+                ss->lib[v] = nullptr; ss->fn[v] = nullptr; ss->fn_stats[v] = nullptr;
+            }
+            ss->cfg = c2;
+        }
+    }
     const bool running = pl->run_snr != nullptr;
     if (running) {   // needs this push's sigma per (unique trial, pixel) and the per-(trial, width) maxima
         const size_t nb = (size_t)pl->nuniq * pl->npix * sizeof(float);
@@ -727,6 +750,8 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
     }
     if (running && !c.INCR)   // NaN = "this trial has no valid sample yet"
         SCU(cudaMemsetAsync(ss->sig, 0xff, (size_t)pl->nuniq * pl->npix * sizeof(float), st), "sigma preset");
+    if (running && !ss->var_init) // the recursion of a trial starts at its first valid push: NaN = "not started" (also after a reset)
+        SCU(cudaMemsetAsync(ss->var, 0xff, (size_t)pl->nuniq * pl->npix * sizeof(float), st), "running variance preset");
     for (int b = 0; b < npass; ++b) {
         StreamParams sp;
         sp.ring = ss->ring; sp.mu0 = ss->mu0; sp.partials = ss->partials;
@@ -763,164 +788,6 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
     k_stream_finalize<<<(pl->npix + 255) / 256, 256, 0, st>>>(ss->partials, nslice, pl->npix, (int)(lo & 0x7fffffff), snr_map, argmax);
     SCU(cudaGetLastError(), "k_stream_finalize launch");
     ++*launches;
-    return NSFRB_OK;
-}
-
-// ------------------------------------------------------------------------------------------------
-// offline path: plan-specialised k_search3
-// ------------------------------------------------------------------------------------------------
-struct Search3State {
-    cudaLibrary_t lib = nullptr;
-    cudaKernel_t fn = nullptr;
-    size_t smem = 0;
-    int trials = 16, ngroups = 0; // trials per CTA, DM groups per pixel
-    bool fused = false;           // the kernel also reduces over groups and finds the arg-max time
-    int32_t *counter = nullptr;   // [npix] tickets of the fused reduction
-};
-
-namespace {
-
-struct Search3Params {
-    const float *W;
-    Partial *partials;
-    int32_t npix;
-    int32_t *counter;
-    float *snr_map;
-    int32_t *argmax;
-};
-
-constexpr int kWmid = 80; // widths 17..kWmid are served from the ring without a bound (it never prunes them)
-
-// trials per CTA: 16 (512 threads); NSFRB_SEARCH_TRIALS=8 selects 256-thread CTAs (measured slower on C3-C5:
-// the raw tile and the first-trial channel sum are then shared by half as many trials)
-int search3_trials()
-{
-    const char *e = getenv("NSFRB_SEARCH_TRIALS");
-    return (e && atoi(e) == 8) ? 8 : 16;
-}
-
-size_t search3_smem(const nsfrb_plan *pl, int trials)
-{
-    const size_t nfl = (size_t)pl->nchan * pl->RS + 4 + (size_t)trials * kStageStride + (size_t)trials * pl->H +
-                       (size_t)trials * (pl->H / 32) + (size_t)trials * 8;
-    return nfl * sizeof(float) + 16;
-}
-
-// the fused per-pixel reduction needs the winning series' prefix (nt + 2 floats) and 2 words of scratch per thread
-// in the kernel's dynamic shared memory
-bool search3_fused(const nsfrb_plan *pl, int trials)
-{
-    const char *e = getenv("NSFRB_SEARCH_FUSED");
-    if (e && std::strcmp(e, "0") == 0) return false;
-    // short series: the fused tail (a few block-wide barriers per pixel, one CTA per SM) costs more than a separate
-    // k_finalize launch saves (C4, nt = 512: +48 ms vs 22 ms); long series: it reads the winner from L2 instead of HBM
-    // (C3, nt = 4096: 13.7 -> 6 ms; C5: 19.6 -> 3 ms).  NSFRB_SEARCH_FUSED=1 forces it on.
-    if (pl->nt < 2048 && !(e && std::strcmp(e, "1") == 0)) return false;
-    return ((size_t)pl->nt + 2 + 2 * (size_t)trials * 32) * sizeof(float) <= search3_smem(pl, trials);
-}
-
-std::string search3_prologue(const nsfrb_plan *pl)
-{
-    std::string s = "// generated by nsfrb_stream.cu for one plan (offline kernel)\n";
-    auto def = [&](const char *n, long long v) { s += "#define " + std::string(n) + " " + std::to_string(v) + "\n"; };
-    def("NCHAN", pl->nchan); def("NU", pl->nuniq); def("NW", std::max(pl->nw_used, 1)); def("RS", pl->RS); def("H", pl->H);
-    def("PITCH", pl->pitch); def("NT", pl->nt); def("WMID", std::min(kWmid, pl->H - kBlockLen - 32));
-    const int trials = search3_trials();
-    def("TRIALS", trials);
-    def("FUSED", search3_fused(pl, trials) ? 1 : 0);
-    {
-        const char *e = getenv("NSFRB_SEARCH_CHAIN16");
-        def("CHAIN16", e ? (atoi(e) != 0) : (pl->nchan >= 32)); // one 16-trial dedispersion chain per group when the channel sum is long
-    }
-    def("MINB", std::max<long long>(1, std::min<long long>(65536 / (trials * 32 * 128), (227 * 1024) / (long long)(search3_smem(pl, trials) + 1024))));
-    s += "static __device__ constexpr short D_TAB[NU][NCHAN] = {";
-    for (int u = 0; u < pl->nuniq; ++u) {
-        s += u ? ",{" : "{";
-        for (int ch = 0; ch < pl->nchan; ++ch) {
-            if (ch) s += ",";
-            s += std::to_string(pl->delays_u[(size_t)u * pl->nchan + ch]);
-        }
-        s += "}";
-    }
-    s += "};\n";
-    std::vector<int> dmax(pl->dmax_u.begin(), pl->dmax_u.end()), kof(pl->k_of_u.begin(), pl->k_of_u.end());
-    append_table(s, "static __device__ constexpr int DMAX_TAB[NU]", dmax);
-    append_table(s, "static __device__ constexpr int K_OF_U[NU]", kof);
-    std::vector<int> w(pl->widths_used.begin(), pl->widths_used.end());
-    if (w.empty()) w.push_back(0x3fffffff);
-    append_table(s, "static __device__ constexpr int W_TAB[NW]", w);
-    std::vector<int> jw(pl->j_of_used.begin(), pl->j_of_used.end());
-    if (jw.empty()) jw.push_back(0);
-    append_table(s, "static __device__ constexpr int J_OF_W[NW]", jw);
-    return s;
-}
-
-} // namespace
-
-bool search3_usable(const nsfrb_plan *pl)
-{
-    const char *e = getenv("NSFRB_SEARCH_JIT");
-    if (e && std::strcmp(e, "0") == 0) return false;
-    return pl->nw_used >= 1 && pl->nw_used <= 32 && pl->n_wb == 1;
-}
-
-int search3_source(const nsfrb_plan *pl, std::string &src, std::string &err)
-{
-    if (pl->nw_used > 32) { err = "k_search3 handles at most 32 usable widths"; return NSFRB_EINVAL; }
-    src = search3_prologue(pl);
-    src += kSearchKernelSrc;
-    return NSFRB_OK;
-}
-
-void search3_free(nsfrb_plan *p)
-{
-    if (!p || !p->search3) return;
-    if (p->search3->lib) cudaLibraryUnload(p->search3->lib);
-    cudaFree(p->search3->counter);
-    cudaGetLastError();
-    delete p->search3;
-    p->search3 = nullptr;
-}
-
-int search3_slices(const nsfrb_plan *pl) { return pl->search3 ? pl->search3->ngroups : 0; }
-
-int search3_launch(nsfrb_plan *pl, cudaStream_t st, float *snr_map, int32_t *argmax, bool *finalized, std::string &err)
-{
-    *finalized = false;
-    if (!pl->search3) {
-        Search3State *s3 = new Search3State();
-        pl->search3 = s3;
-        std::string src, log;
-        std::vector<char> cubin;
-        int rc = search3_source(pl, src, err);
-        if (!rc && (rc = stream_compile(src, cubin, log))) err = "k_search3 compile failed: " + log;
-        if (rc) { search3_free(pl); return rc; }
-        s3->trials = search3_trials();
-        s3->ngroups = (pl->nuniq + s3->trials - 1) / s3->trials;
-        s3->smem = search3_smem(pl, s3->trials);
-        s3->fused = search3_fused(pl, s3->trials);
-        cudaError_t e = cudaLibraryLoadData(&s3->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
-        if (e == cudaSuccess) e = cudaLibraryGetKernel(&s3->fn, s3->lib, "k_search3");
-        if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)s3->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s3->smem);
-        if (e == cudaSuccess && s3->fused) {
-            e = cudaMalloc(reinterpret_cast<void **>(&s3->counter), (size_t)pl->npix * sizeof(int32_t));
-            if (e == cudaSuccess) e = cudaMemset(s3->counter, 0, (size_t)pl->npix * sizeof(int32_t));
-        }
-        if (e != cudaSuccess) {
-            const int code = fail_cuda(e, "k_search3 load", err);
-            search3_free(pl);
-            return code;
-        }
-    }
-    Search3Params sp;
-    sp.W = pl->d_W; sp.partials = pl->d_partials; sp.npix = pl->npix;
-    sp.counter = pl->search3->counter; sp.snr_map = snr_map; sp.argmax = argmax;
-    *finalized = pl->search3->fused;
-    void *args[] = {&sp};
-    const long long blocks = (long long)pl->npix * pl->search3->ngroups;
-    if (blocks <= 0 || blocks > 0x7fffffffLL) { err = "too many CTAs for one launch"; return NSFRB_EINVAL; }
-    SCU(cudaLaunchKernel((const void *)pl->search3->fn, dim3((unsigned)blocks), dim3(pl->search3->trials * 32), args, pl->search3->smem, st),
-        "k_search3 launch");
     return NSFRB_OK;
 }
 

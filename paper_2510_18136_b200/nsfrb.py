@@ -46,7 +46,8 @@ EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stre
            "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
            "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes",
            "nsfrb_psf_mask", "nsfrb_cluster", "nsfrb_median_subtract",
-           "nsfrb_stream_push_host_async", "nsfrb_stream_wait", "nsfrb_stream_set_running_sigma")
+           "nsfrb_stream_push_host_async", "nsfrb_stream_wait", "nsfrb_stream_set_running_sigma",
+           "nsfrb_peaks_count", "nsfrb_peaks_name", "nsfrb_measure_peaks", "nsfrb_plan_prepare")
 
 _lib = None
 
@@ -110,6 +111,14 @@ def lib() -> ctypes.CDLL:
         L.nsfrb_psf_mask.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, vp, vp, vp]
         L.nsfrb_cluster.restype = ctypes.c_int
         L.nsfrb_cluster.argtypes = [vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp]
+        L.nsfrb_plan_prepare.restype = ctypes.c_int
+        L.nsfrb_plan_prepare.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+        L.nsfrb_peaks_count.restype = ctypes.c_int
+        L.nsfrb_peaks_count.argtypes = []
+        L.nsfrb_peaks_name.restype = ctypes.c_char_p
+        L.nsfrb_peaks_name.argtypes = [ctypes.c_int]
+        L.nsfrb_measure_peaks.restype = ctypes.c_int
+        L.nsfrb_measure_peaks.argtypes = [ctypes.c_int, f64p, f64p, vp]
         L.nsfrb_last_error.restype = ctypes.c_char_p
         L.nsfrb_version.restype = ctypes.c_char_p
         _lib = L
@@ -172,6 +181,15 @@ def jit_search_kernel(nx, ny, nchan, nt, freqs_GHz, tsamp_s, dm_list, width_list
     buf = ctypes.create_string_buffer(need.value)
     _check(lib().nsfrb_jit_search_kernel(*args, buf, need.value, ctypes.byref(need)))
     return buf.raw[: need.value]
+
+
+def measure_peaks(iters: int = 2000) -> dict:
+    """nsfrb_measure_peaks: {test name: (operations or words per second, per SM clock per SM)} of the current device."""
+    L = lib()
+    n = L.nsfrb_peaks_count()
+    a, b = (ctypes.c_double * n)(), (ctypes.c_double * n)()
+    _check(L.nsfrb_measure_peaks(int(iters), a, b, int(torch.cuda.current_stream().cuda_stream)))
+    return {L.nsfrb_peaks_name(i).decode(): (float(a[i]), float(b[i])) for i in range(n)}
 
 
 def bin_time(cube: torch.Tensor, factor: int, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
@@ -266,6 +284,15 @@ class Plan:
         s = nsfrb_plan_info()
         _check(lib().nsfrb_plan_get_info(self._h, ctypes.byref(s)))
         return {n: int(getattr(s, n)) for n, _ in s._fields_}
+
+    def prepare(self, stream_chunk_nt: int | None = None):
+        """nsfrb_plan_prepare: compile the plan's kernel and allocate its workspaces now (offline search by default, the
+        real-time path for pushes of stream_chunk_nt samples otherwise)."""
+        if stream_chunk_nt is None:
+            _check(lib().nsfrb_plan_prepare(self._h, 0, 0))
+        else:
+            _check(lib().nsfrb_plan_prepare(self._h, 1, int(stream_chunk_nt)))
+        return self
 
     def last_launches(self) -> int:
         return int(lib().nsfrb_plan_last_launches(self._h))

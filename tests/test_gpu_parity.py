@@ -101,6 +101,33 @@ def test_scaled_configs(name, nx, ny, nt):
     _check_recovery(wl, d, pulses, snr)
 
 
+@pytest.mark.parametrize("name,nx,ny,nt,batch,side", [
+    ("c3", 12, 8, 1000, 16, "1"),    # six full batches, the next one moved by the search CTAs themselves
+    ("c3", 7, 5, 600, 8, "1"),       # ragged last batch (3 pixels), npix not a multiple of 8
+    ("c4", 9, 5, None, 16, "1"),     # three DM groups per pixel: 24 members share a group of 8 pixels; series inside the ring
+    ("c5", 5, 5, 700, 8, "1"),       # 64 channels, 16 groups: many more side rows than time blocks
+    ("c3", 7, 5, 600, 8, "0"),       # the same pipeline with standalone layout kernels
+    ("c5-16dm", 5, 4, 256, 8, "1"),  # one DM group, one time block, 64 channels: eight side steps after the only block
+])
+def test_offline_pixel_batches(monkeypatch, name, nx, ny, nt, batch, side):
+    """nsfrb_search walks the image in pixel batches through two workspaces; while batch i is searched its CTAs move
+    batch i+1 from the caller's [chan][time][pixel] cube into the other workspace.  Forced to tiny
+    batches here, the result must equal the oracle on every pixel, and the one-batch run bit for bit."""
+    from dataclasses import replace
+    wl = W.config(name.split("-")[0]).scaled(nx, ny, nt, n_pulses=4)
+    if name.endswith("16dm"):
+        wl = replace(wl, dm_list=wl.dm_list[:16])
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    cube = W.make_cube(wl, "cuda")
+    cube += 50.0 * torch.randn((wl.nchan, 1, wl.npix), device="cuda")    # per-(channel, pixel) offsets: the baseline removal
+    _inject_all(wl, cube, d)
+    st1, cs1, snr1, arg1 = _offline(wl, cube, label=f"{name} one batch")
+    monkeypatch.setenv("NSFRB_SEARCH_BATCH_PIX", str(batch))
+    monkeypatch.setenv("NSFRB_SEARCH_SIDE", side)
+    st, cs, snr, arg = _offline(wl, cube, label=f"{name} batches of {batch}")
+    assert np.array_equal(snr, snr1) and np.array_equal(arg, arg1)
+
+
 def _check_recovery(wl, d, pulses, snr, frac=0.7):
     """Injected single pulses come back at >= frac of the closed form S0 q / sqrt(1 + S0^2 q / T_k)
     (SURVEY 8(c) 'Injected pulse in noise'; the max over cells can only be higher)."""
@@ -479,7 +506,7 @@ def test_two_plans_with_different_shared_memory_needs_coexist():
 
 def test_more_than_32_widths_use_the_generic_kernel():
     """Plans with more than 32 usable widths run the generic k_search (two width batches); everything else runs
-    the plan-specialised k_search3 -- both against the oracle, and against each other on the same cube."""
+    the plan-specialised k_search4 -- both against the oracle, and against each other on the same cube."""
     from dataclasses import replace
     nsfrb = _nsfrb()
     wl40 = replace(W.config("c1"), nx=6, ny=5, nt=700, width_list=np.arange(1, 41, dtype=np.int32) * 3 - 2, name="w40")
@@ -487,7 +514,7 @@ def test_more_than_32_widths_use_the_generic_kernel():
     g = torch.Generator(device="cuda").manual_seed(41)
     cube = torch.randn((wl40.nchan, wl40.nt, wl40.npix), device="cuda", generator=g)
     st, cs, snr40, arg40 = _offline(wl40, cube, label="w40 generic")
-    # the first 32 of those widths through k_search3, then the maxima restricted to them must agree where they win
+    # the first 32 of those widths through k_search4, then the maxima restricted to them must agree where they win
     wl32 = replace(wl40, width_list=wl40.width_list[:32], name="w32")
     st, cs, snr32, arg32 = _offline(wl32, cube, label="w32 specialised")
     same = arg40[:, 1] < 32

@@ -82,12 +82,12 @@ def test_kernel_cross_compiles_to_sm100a():
 
 
 def test_offline_kernel_source_and_cubin():
-    """k_search3 (plan-specialised offline kernel): the source carries the plan, NVRTC cross-compiles it."""
+    """k_search4 (plan-specialised offline kernel): the source carries the plan, NVRTC cross-compiles it."""
     wl = W.config("c3")
     src = nsfrb.jit_search_kernel(*_args(wl)).decode()
     assert "#define NCHAN 16" in src and "#define NU 32" in src and "#define NW 24" in src and "#define NT 4096" in src
     assert "W_TAB[NW] = {1,2,3,4,5,6,7,9,12,16,22,30,40,55,75,102,139,189,257,350,476,648,882,1200}" in src
-    assert 'extern "C" __global__' in src and "k_search3" in src
+    assert 'extern "C" __global__' in src and "k_search4" in src
     cubin = nsfrb.jit_search_kernel(*_args(W.config("c1")), cubin=True)
     assert cubin[:4] == b"\x7fELF"
     with pytest.raises(nsfrb.NsfrbError):      # more than 32 usable widths: the generic kernel serves those plans
