@@ -25,7 +25,6 @@ const char kSearchKernelSrc[] =
 
 constexpr size_t kSmemLimit = 227 * 1024;
 constexpr int kWmid = 80;       // widths 17..kWmid are served from the ring without a bound (it never prunes them)
-constexpr int kSideTile = 8 * (256 + 4); // floats of the transposing tile (8 pixels x SROWS + 4)
 
 // host mirror of the kernel's parameter block (nsfrb_search_kernel.cuh)
 struct Search4Params {
@@ -36,9 +35,6 @@ struct Search4Params {
     float *snr_map;
     int32_t *argmax;
     float *scratch;
-    const float *cube;
-    float *Wn;
-    int32_t n0, nnb;
 };
 
 int env_int(const char *name, int dflt)
@@ -67,11 +63,10 @@ struct Search4State {
     cudaKernel_t fn = nullptr;
     size_t smem = 0;
     int ngroups = 0;
-    int batch = 0, nbatch = 1; // pixels per batch (a multiple of 8 when nbatch > 1)
-    bool side = false;         // the kernel moves the next batch itself
+    int batch = 0, nbatch = 1, pxi = 1; // pixels per batch; pixels per work item
     float *W[2] = {nullptr, nullptr};
     float *scratch = nullptr;   // [grid][16][dpitch] dedispersed series of the items in flight (L2-resident)
-    int grid = 0, dpitch = 0;   // persistent CTAs (one per SM)
+    int grid = 0, dpitch = 0, nwarp = 16; // persistent CTAs (16 / nwarp per SM)
     int32_t *counter = nullptr; // [npix] tickets of the per-pixel reduction
     size_t bytes = 0;
 };
@@ -80,21 +75,21 @@ namespace {
 
 // geometry shared by the prologue and the launch: ring length, shared memory, batch size
 struct Geo {
-    int H, RS, lba, chain, ringt, side, batch, nbatch, ngroups, dpitch, sdir, prune;
+    int H, nwarp, pxi, batch, nbatch, ngroups, dpitch, sdir, prune;
     size_t smem;
 };
 
-// mirrors kSmemFloats of the kernel: raw tile | rings (two planes), 8-slot minima twice, 32-slot minima | results, sums, side tile
-size_t search4_smem(const nsfrb_plan *pl, int H, int RS, int chain, bool side)
+// mirrors kSmemFloats of the kernel: rings (two planes), 8-slot and 32-slot minima twice | per-(pixel, trial) results
+size_t search4_smem(int H, int nwarp, int pxi)
 {
-    const size_t nfl = (size_t)pl->nchan * RS + 4 + (size_t)16 * ((H + 16) + 2 * (H / 8) + H / 32) + 16 * 8 +
-                       (size_t)16 * 2 * chain + 16 * 4 + (side ? kSideTile : 0);
+    const size_t nfl = (size_t)nwarp * ((H + 16) + 2 * (H / 8) + 2 * (H / 32)) + (size_t)pxi * nwarp * 8;
     return nfl * sizeof(float) + 64;
 }
 
 bool search4_geo(const nsfrb_plan *pl, Geo &g)
 {
-    g.ngroups = (pl->nuniq + 15) / 16;
+    g.nwarp = env_int("NSFRB_SEARCH_WARPS", 16) == 8 ? 8 : 16; // trials per CTA; 8: two CTAs per SM
+    g.ngroups = (pl->nuniq + g.nwarp - 1) / g.nwarp;
     // pixel batches: about NSFRB_SEARCH_BATCH_MB (default 1024) of workspace each, at least ~8192 items per launch
     const size_t bpp = (size_t)pl->nchan * pl->pitch * sizeof(float);
     const size_t target = (size_t)std::max(1, env_int("NSFRB_SEARCH_BATCH_MB", 1024)) << 20;
@@ -104,44 +99,35 @@ bool search4_geo(const nsfrb_plan *pl, Geo &g)
     nb = std::max<long long>(8, nb & ~7LL);
     if (nb >= pl->npix) { g.batch = pl->npix; g.nbatch = 1; }
     else { g.batch = (int)nb; g.nbatch = (pl->npix + g.batch - 1) / g.batch; }
-    g.side = (g.nbatch > 1 && env_int("NSFRB_SEARCH_SIDE", 1) != 0) ? 1 : 0;
-    g.sdir = std::max(0, std::min(16, env_int("NSFRB_SEARCH_SDIR", 4)));   // widths up to here are evaluated without a bound
+    g.sdir = std::max(0, std::min(16, env_int("NSFRB_SEARCH_SDIR", 8)));   // widths up to here are evaluated without a bound
     g.prune = env_int("NSFRB_SEARCH_PRUNE", 1) != 0;
     g.dpitch = round_up(pl->nt, 512);
+    // pixels per work item: the item's barriers are shared by them and the tail keeps one warp per pixel busy.  The scratch
+    // (pxi x nwarp series per CTA) is about 2 MB per CTA (measured best on C3-C5: 8 / 16 / 4 pixels; it then cycles through
+    // L2 and HBM, one block ahead of the search)
+    const size_t series = (size_t)g.nwarp * g.dpitch * sizeof(float);
+    g.pxi = (int)std::max<size_t>(1, std::min<size_t>(16, (2048u << 10) / series));
+    if (env_int("NSFRB_SEARCH_PXI", 0) > 0) g.pxi = std::min(16, env_int("NSFRB_SEARCH_PXI", 0));
+    g.pxi = std::min(g.pxi, g.nwarp);
     // ring: wmax + one block + the rows the bounds read, a multiple of 64; a power of two (every wrap one AND) when shared
-    // memory allows.  Sweep A: 512-sample blocks with one 16-trial chain per thread when the raw tile fits, else 256-sample
-    // blocks (NSFRB_SEARCH_CHAIN=8: two 8-trial chains, all threads busy; 16: one 16-trial chain on half the threads).
+    // memory allows
+    const size_t limit = kSmemLimit / (16 / g.nwarp) - (g.nwarp == 8 ? 1024 : 0);
     const int hmin = round_up(std::max(pl->wmax_used, 1) + kBlockLen + 32, 64);
     int h2 = 64;
     while (h2 < hmin) h2 <<= 1;
-    struct Shape { int lba, chain; };
-    const int chain256 = env_int("NSFRB_SEARCH_CHAIN", pl->nchan >= 32 ? 16 : 8) == 16 ? 16 : 8;
-    const Shape shapes[2] = {{512, 16}, {256, chain256}};
-    bool ok = false;
-    for (int si = (env_int("NSFRB_SEARCH_LBA", 512) == 512 ? 0 : 1); si < 2 && !ok; ++si)
-        for (int hs = 0; hs < 2 && !ok; ++hs)
-            for (int sd = g.side; sd >= 0 && !ok; --sd) {
-                const int H = hs == 0 ? h2 : hmin, RS = round_up(shapes[si].lba + pl->dmax_all, 4);
-                if (search4_smem(pl, H, RS, shapes[si].chain, sd != 0) <= kSmemLimit) {
-                    g.H = H; g.RS = RS; g.lba = shapes[si].lba; g.chain = shapes[si].chain; g.side = sd;
-                    ok = true;
-                }
-            }
-    if (!ok) return false;
-    g.smem = search4_smem(pl, g.H, g.RS, g.chain, g.side != 0);
-    g.ringt = round_up(pl->nt, kBlockLen) <= g.H ? 1 : 0; // every block of the series fits the ring: nothing is overwritten
-    // the per-pixel reduction of long series rebuilds one prefix series (nt + 2 floats) + 2 words per thread in the same memory
-    const size_t fin = ((size_t)pl->nt + 2 + 2 * 512) * sizeof(float);
-    return g.ringt || fin <= g.smem;
+    g.H = search4_smem(h2, g.nwarp, g.pxi) <= limit ? h2 : hmin;
+    if (search4_smem(g.H, g.nwarp, g.pxi) > limit) return false;
+    g.smem = search4_smem(g.H, g.nwarp, g.pxi);
+    return true;
 }
 
 std::string search4_prologue(const nsfrb_plan *pl, const Geo &g)
 {
     std::string s = "// generated by nsfrb_offline.cu for one plan (offline kernel)\n";
     auto def = [&](const char *n, long long v) { s += "#define " + std::string(n) + " " + std::to_string(v) + "\n"; };
-    def("NCHAN", pl->nchan); def("NU", pl->nuniq); def("NW", std::max(pl->nw_used, 1)); def("RS", g.RS); def("H", g.H);
+    def("NCHAN", pl->nchan); def("NU", pl->nuniq); def("NW", std::max(pl->nw_used, 1)); def("NWARP", g.nwarp); def("H", g.H);
     def("PITCH", pl->pitch); def("DPITCH", g.dpitch); def("NT", pl->nt); def("WMID", std::min(kWmid, g.H - kBlockLen - 32));
-    def("SDIR", g.sdir); def("LBA", g.lba); def("CHAIN", g.chain); def("RINGT", g.ringt); def("SIDE", g.side); def("PRUNE", g.prune);
+    def("SDIR", g.sdir); def("PXI", g.pxi); def("PRUNE", g.prune);
     s += "static __device__ constexpr short D_TAB[NU][NCHAN] = {";
     for (int u = 0; u < pl->nuniq; ++u) {
         s += u ? ",{" : "{";
@@ -228,11 +214,13 @@ int search4_prepare(nsfrb_plan *pl, std::string &err)
     int rc = search4_source(pl, src, err);
     if (!rc && (rc = stream_compile(src, cubin, log))) err = "k_search4 compile failed: " + log;
     if (rc) { search4_free(pl); return rc; }
-    s4->ngroups = g.ngroups; s4->smem = g.smem; s4->batch = g.batch; s4->nbatch = g.nbatch; s4->side = g.side != 0;
+    s4->ngroups = g.ngroups; s4->smem = g.smem; s4->batch = g.batch; s4->nbatch = g.nbatch; s4->pxi = g.pxi;
     cudaError_t e = cudaLibraryLoadData(&s4->lib, cubin.data(), nullptr, nullptr, 0, nullptr, nullptr, 0);
     if (e == cudaSuccess) e = cudaLibraryGetKernel(&s4->fn, s4->lib, "k_search4");
     if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)s4->fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s4->smem);
-    const size_t wb = (size_t)g.batch * pl->nchan * (size_t)pl->pitch * sizeof(float);
+    s4->nwarp = g.nwarp;
+    // (+ slack: sweep A reads up to one block + the largest delay past the end of a row; the values are never used)
+    const size_t wb = ((size_t)g.batch * pl->nchan * (size_t)pl->pitch + 1024 + pl->dmax_all) * sizeof(float);
     for (int b = 0; b < (g.nbatch > 1 ? 2 : 1) && e == cudaSuccess; ++b) {
         e = cudaMalloc(reinterpret_cast<void **>(&s4->W[b]), wb);
         if (e == cudaSuccess) e = cudaMemset(s4->W[b], 0, wb);
@@ -241,9 +229,9 @@ int search4_prepare(nsfrb_plan *pl, std::string &err)
     if (e == cudaSuccess) { // one CTA per SM, each with the dedispersed series of its item in flight
         int nsm = 0;
         e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, pl->device);
-        s4->grid = std::max(1, nsm);
+        s4->grid = std::max(1, nsm) * (16 / g.nwarp);
         s4->dpitch = g.dpitch;
-        const size_t sb = (size_t)s4->grid * 16 * g.dpitch * sizeof(float);
+        const size_t sb = (size_t)s4->grid * g.pxi * g.nwarp * g.dpitch * sizeof(float);
         if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&s4->scratch), sb);
         if (e == cudaSuccess) e = cudaMemset(s4->scratch, 0, sb);
         if (e == cudaSuccess) s4->bytes += sb;
@@ -273,8 +261,7 @@ int search4_launch(nsfrb_plan *pl, const float *cube, cudaStream_t st, float *sn
     ++*launches;
     if (ev_layout) cudaEventRecord(ev_layout, st);
     for (int i = 0; i < s4->nbatch; ++i) {
-        const bool more = i + 1 < s4->nbatch;
-        if (more && !s4->side) {
+        if (i + 1 < s4->nbatch) { // the next batch's layout change, stream-ordered behind the search that last read that buffer
             OCU(launch_transpose(cube, s4->W[(i + 1) & 1], pl->npix, pl->nchan, pl->nt, pl->pitch, (i + 1) * nb, count(i + 1), st),
                 "k_transpose launch");
             ++*launches;
@@ -282,12 +269,10 @@ int search4_launch(nsfrb_plan *pl, const float *cube, cudaStream_t st, float *sn
         Search4Params sp;
         sp.W = s4->W[i & 1]; sp.partials = pl->d_partials; sp.npix = pl->npix; sp.p0 = i * nb; sp.npb = count(i);
         sp.counter = s4->counter; sp.snr_map = snr_map; sp.argmax = argmax; sp.scratch = s4->scratch;
-        sp.cube = cube; sp.Wn = s4->W[(i + 1) & 1];
-        sp.n0 = (i + 1) * nb; sp.nnb = (more && s4->side) ? count(i + 1) : 0;
         void *args[] = {&sp};
-        const long long blocks = (long long)sp.npb * s4->ngroups;
-        if (blocks <= 0 || blocks > 0x7fffffffLL) { err = "too many CTAs for one launch"; return NSFRB_EINVAL; }
-        OCU(cudaLaunchKernel((const void *)s4->fn, dim3((unsigned)std::min<long long>(blocks, s4->grid)), dim3(512), args, s4->smem, st),
+        const long long items = (long long)((sp.npb + s4->pxi - 1) / s4->pxi) * s4->ngroups;
+        if (items <= 0 || items > 0x7fffffffLL) { err = "too many work items for one launch"; return NSFRB_EINVAL; }
+        OCU(cudaLaunchKernel((const void *)s4->fn, dim3((unsigned)std::min<long long>(items, s4->grid)), dim3(32 * s4->nwarp), args, s4->smem, st),
             "k_search4 launch");
         ++*launches;
     }
