@@ -80,9 +80,9 @@ struct Geo {
 };
 
 // mirrors kSmemFloats of the kernel: rings (two planes), 8-slot and 32-slot minima twice | per-(pixel, trial) results
-size_t search4_smem(int H, int nwarp, int pxi)
+size_t search4_smem(int H, int nwarp, int pxi, int nt)
 {
-    const size_t nfl = (size_t)nwarp * ((H + 16) + 2 * (H / 8) + 2 * (H / 32)) + (size_t)pxi * nwarp * 8;
+    const size_t nfl = (size_t)nwarp * ((H + 16) + 2 * (H / 8) + 2 * (H / 32)) + (size_t)pxi * nwarp * (8 + (nt + 255) / 256 + 2);
     return nfl * sizeof(float) + 64;
 }
 
@@ -115,9 +115,9 @@ bool search4_geo(const nsfrb_plan *pl, Geo &g)
     const int hmin = round_up(std::max(pl->wmax_used, 1) + kBlockLen + 32, 64);
     int h2 = 64;
     while (h2 < hmin) h2 <<= 1;
-    g.H = search4_smem(h2, g.nwarp, g.pxi) <= limit ? h2 : hmin;
-    if (search4_smem(g.H, g.nwarp, g.pxi) > limit) return false;
-    g.smem = search4_smem(g.H, g.nwarp, g.pxi);
+    g.H = search4_smem(h2, g.nwarp, g.pxi, pl->nt) <= limit ? h2 : hmin;
+    if (search4_smem(g.H, g.nwarp, g.pxi, pl->nt) > limit) return false;
+    g.smem = search4_smem(g.H, g.nwarp, g.pxi, pl->nt);
     return true;
 }
 

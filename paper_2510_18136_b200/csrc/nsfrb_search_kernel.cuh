@@ -402,7 +402,8 @@ template <bool INSIDE> __device__ __forceinline__ void prefix_block(float (&p8)[
 
 // shared memory: rings, 8-slot minima (twice), 32-slot minima (twice) | per-(pixel, trial) results
 constexpr int kRingFloats = NWARP * (RINGF + 2 * NG + 2 * NR);
-constexpr int kSmemFloats = kRingFloats + PXI * NWARP * 8;
+constexpr int NBLK = (NT + LB - 1) / LB;                 // blocks of the longest series
+constexpr int kSmemFloats = kRingFloats + PXI * NWARP * 8 + PXI * NWARP * NBLK + PXI * NWARP * 2;
 
 // sweep A of one pixel: group G's delays are immediates here, and only here
 template <int G> __device__ __forceinline__ void sweep_a(const float *Wp, float *scr, int tid)
@@ -429,6 +430,8 @@ __device__ __forceinline__ void run_item(const Search4Params &P, float *smem, in
     float *rm8s = rings + NWARP * RINGF;         // [NWARP][2 NG]   min of P over each 8-slot group, stored twice
     float *rm32s = rm8s + NWARP * 2 * NG;        // [NWARP][2 NR]   min of P over each 32-slot row, stored twice
     float *red = rm32s + NWARP * 2 * NR;         // [PXI][NWARP][8] per-(pixel, trial) results
+    float *cb = red + PXI * NWARP * 8;           // [PXI][NWARP][NBLK] the prefix before every block (the tail restarts there)
+    float *tl = cb + PXI * NWARP * NBLK;         // [PXI][NWARP][2] tail: partial arg-max per slice
     __shared__ int sbest[PXI];                   // best S/N of each pixel so far (float bits, >= 0)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -461,14 +464,29 @@ __device__ __forceinline__ void run_item(const Search4Params &P, float *smem, in
             // ---- a1, a3: exact mean and sigma of the series (one pass; D is centred on the first sample of every channel)
             float rsig;
             {
-                float s1 = 0.f, s2 = 0.f;
-                for (int i = 4 * lane; i < T_k; i += 128) {
+                float s1 = 0.f, s2 = 0.f, s1b = 0.f, s2b = 0.f;
+                int i = 4 * lane;
+                for (; i + 388 <= T_k; i += 512) { // four independent 16-byte loads in flight per lane
+                    const float4 v0 = __ldcg(reinterpret_cast<const float4 *>(drow + i));
+                    const float4 v1 = __ldcg(reinterpret_cast<const float4 *>(drow + i + 128));
+                    const float4 v2 = __ldcg(reinterpret_cast<const float4 *>(drow + i + 256));
+                    const float4 v3 = __ldcg(reinterpret_cast<const float4 *>(drow + i + 384));
+                    s1 += (v0.x + v0.y) + (v0.z + v0.w); s1b += (v1.x + v1.y) + (v1.z + v1.w);
+                    s1 += (v2.x + v2.y) + (v2.z + v2.w); s1b += (v3.x + v3.y) + (v3.z + v3.w);
+                    s2 = fmaf(v0.x, v0.x, s2); s2 = fmaf(v0.y, v0.y, s2); s2 = fmaf(v0.z, v0.z, s2); s2 = fmaf(v0.w, v0.w, s2);
+                    s2b = fmaf(v1.x, v1.x, s2b); s2b = fmaf(v1.y, v1.y, s2b); s2b = fmaf(v1.z, v1.z, s2b); s2b = fmaf(v1.w, v1.w, s2b);
+                    s2 = fmaf(v2.x, v2.x, s2); s2 = fmaf(v2.y, v2.y, s2); s2 = fmaf(v2.z, v2.z, s2); s2 = fmaf(v2.w, v2.w, s2);
+                    s2b = fmaf(v3.x, v3.x, s2b); s2b = fmaf(v3.y, v3.y, s2b); s2b = fmaf(v3.z, v3.z, s2b); s2b = fmaf(v3.w, v3.w, s2b);
+                }
+                for (; i < T_k; i += 128) {
                     const float4 v = __ldcg(reinterpret_cast<const float4 *>(drow + i));
                     const float e[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
                     for (int q = 0; q < 4; ++q)
                         if (i + q < T_k) { s1 += e[q]; s2 = fmaf(e[q], e[q], s2); }
                 }
+                s1 += s1b;
+                s2 += s2b;
                 s1 = warp_sum(s1);
                 s2 = warp_sum(s2);
                 const float invT = 1.f / (float)T_k;
@@ -506,6 +524,7 @@ __device__ __forceinline__ void run_item(const Search4Params &P, float *smem, in
                     na = __ldcg(reinterpret_cast<const float4 *>(dp + t0 + LB));
                     nb = __ldcg(reinterpret_cast<const float4 *>(dp + t0 + LB) + 1);
                 }
+                if (lane == 0) cb[(px * NWARP + warp) * NBLK + t0 / LB] = T.carry;
                 if (t0 + LB <= T_k) search_block<true>(T, p8, ring, rm8, rm32, &sbest[px], lane, t0, T_k, sqw_lane, is_large);
                 else search_block<false>(T, p8, ring, rm8, rm32, &sbest[px], lane, t0, T_k, sqw_lane, is_large);
                 T.g0 = wrapG(T.g0 + LB / 8);
@@ -556,71 +575,100 @@ __device__ __forceinline__ void run_item(const Search4Params &P, float *smem, in
     }
     __syncthreads();
 
-    // ================= tail: warp q finishes pixel q
-    if (warp < npx) {
-        const int px = warp, p = P.p0 + lp0 + px;
-        // best trial of the group (lane w holds trial w's record)
-        float s = -S4_INF, rmu = 0.f, rsg = 0.f;
-        int k = -1, j = -1, uu = -1;
+    // ================= tail: NWARP / npx warps per pixel: best trial, then the arg-max time -- the prefix of the winning series
+    // once more (block by block from the saved carries, the same operations as sweep B: the same P bit for bit) into its
+    // scratch row, and one scan of the winning width
+    const int nsl = NWARP / npx;                 // warps (slices) per pixel
+    const bool part = warp < npx * nsl;
+    const int px = part ? warp / nsl : 0, sl = part ? warp - px * nsl : 0;
+    const int p = P.p0 + lp0 + px;
+    float s = -S4_INF, rmu = 0.f, rsg = 0.f, mu_b = 0.f;
+    int k = -1, j = -1, uu = -1, wb = -1;
+    if (part) { // (every slice of a pixel repeats this selection: lane w holds trial w's record)
         if (lane < NWARP) {
             const float *r = red + (px * NWARP + lane) * 8;
             s = r[0]; k = reinterpret_cast<const int *>(r)[1]; j = reinterpret_cast<const int *>(r)[2];
-            uu = reinterpret_cast<const int *>(r)[3]; rmu = r[4]; rsg = r[5];
+            uu = reinterpret_cast<const int *>(r)[3]; rmu = r[4]; rsg = r[5]; mu_b = r[7];
         }
-        int wb = (k >= 0) ? lane : -1;
+        wb = (k >= 0) ? lane : -1;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             const float so = __shfl_xor_sync(kFull, s, o);
             const int ko = __shfl_xor_sync(kFull, k, o), jo = __shfl_xor_sync(kFull, j, o), wo = __shfl_xor_sync(kFull, wb, o);
             if (better(so, ko, jo, s, k, j)) { s = so; k = ko; j = jo; wb = wo; }
         }
+        if (wb >= 0) {
+            uu = __shfl_sync(kFull, uu, wb); rmu = __shfl_sync(kFull, rmu, wb); rsg = __shfl_sync(kFull, rsg, wb);
+            mu_b = __shfl_sync(kFull, mu_b, wb);
+        }
+    }
+    const int Tw = wb >= 0 ? NT - DMAX_TAB[uu] : 0, ww = wb >= 0 ? W_TAB[j] : 1;
+    float *drow = scr0 + ((size_t)px * NWARP + (wb >= 0 ? wb : 0)) * DPITCH;
+    if (part && wb >= 0) {
+        const float *cbw = cb + (px * NWARP + wb) * NBLK;
+        for (int t0 = sl * LB; t0 < Tw; t0 += nsl * LB) {
+            float *dp = drow + t0 + 8 * lane;
+            const float4 a = __ldcg(reinterpret_cast<const float4 *>(dp)), b = __ldcg(reinterpret_cast<const float4 *>(dp) + 1);
+            float p8[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+            float carry = cbw[t0 / LB];
+            if (t0 + LB <= Tw) prefix_block<true>(p8, mu_b, carry, lane, 8);
+            else prefix_block<false>(p8, mu_b, carry, lane, Tw - t0 - 8 * lane);
+            __stcg(reinterpret_cast<float4 *>(dp), make_float4(p8[0], p8[1], p8[2], p8[3]));
+            __stcg(reinterpret_cast<float4 *>(dp) + 1, make_float4(p8[4], p8[5], p8[6], p8[7]));
+        }
+    }
+    __syncthreads(); // the whole prefix series of every pixel's winner is in its scratch row
+    if (part && wb >= 0) {
+        float bv = -S4_INF;
+        int bi = 0x7fffffff;
+        const int last = Tw - ww; // starts 0..last; B = P[i+w] - P[i], P[i] at drow[i-1] (P[0] = 0)
+        int i = sl * 32 + lane;
+        const int step = nsl * 32;
+        for (; i + 3 * step <= last; i += 4 * step) { // four starts per lane in flight
+            float e[4], st[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                e[q] = __ldcg(drow + i + q * step + ww - 1);
+                st[q] = (i + q * step == 0) ? 0.f : __ldcg(drow + i + q * step - 1);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const float B = e[q] - st[q];
+                if (B > bv) { bv = B; bi = i + q * step; }
+            }
+        }
+        for (; i <= last; i += step) {
+            const float B = __ldcg(drow + i + ww - 1) - (i == 0 ? 0.f : __ldcg(drow + i - 1));
+            if (B > bv) { bv = B; bi = i; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float ov = __shfl_xor_sync(kFull, bv, o);
+            const int oi = __shfl_xor_sync(kFull, bi, o);
+            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+        }
+        if (lane == 0) { tl[(px * NWARP + sl) * 2] = bv; reinterpret_cast<int *>(tl)[(px * NWARP + sl) * 2 + 1] = bi; }
+    }
+    __syncthreads();
+    if (part && sl == 0 && lane == 0) { // one thread per pixel: combine the slices, write the partial, take the ticket
         Partial4 out;
         out.snr = -S4_INF; out.k = -1; out.j = -1; out.t = -1; out.mu = 0.f; out.sigma = 0.f; out.u = -1; out.pad = 0;
         if (wb >= 0) {
-            uu = __shfl_sync(kFull, uu, wb); rmu = __shfl_sync(kFull, rmu, wb); rsg = __shfl_sync(kFull, rsg, wb);
-            out.snr = s; out.k = k; out.j = j; out.mu = rmu; out.sigma = rsg; out.u = uu;
-            // arg-max time: the prefix of the winning series once more, into its scratch row, then the one width
-            const int Tw = NT - DMAX_TAB[uu], w = W_TAB[j];
-            float *drow = scr0 + ((size_t)px * NWARP + wb) * DPITCH;
-            const float mu_b = red[(px * NWARP + wb) * 8 + 7]; // the mean sweep B subtracted
-            float carry = 0.f;
-            for (int t0 = 0; t0 < Tw; t0 += LB) {
-                float *dp = drow + t0 + 8 * lane;
-                const float4 a = __ldcg(reinterpret_cast<const float4 *>(dp)), b = __ldcg(reinterpret_cast<const float4 *>(dp) + 1);
-                float p8[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-                if (t0 + LB <= Tw) prefix_block<true>(p8, mu_b, carry, lane, 8);
-                else prefix_block<false>(p8, mu_b, carry, lane, Tw - t0 - 8 * lane);
-                __stcg(reinterpret_cast<float4 *>(dp), make_float4(p8[0], p8[1], p8[2], p8[3]));
-                __stcg(reinterpret_cast<float4 *>(dp) + 1, make_float4(p8[4], p8[5], p8[6], p8[7]));
-            }
-            __syncwarp();
-            float bv = -S4_INF;
-            int bi = 0x7fffffff;
-            for (int i = lane; i <= Tw - w; i += 32) { // B = P[i+w] - P[i]; P[i] sits at drow[i-1] (P[0] = 0)
-                const float B = __ldcg(drow + i + w - 1) - (i == 0 ? 0.f : __ldcg(drow + i - 1));
-                if (B > bv) { bv = B; bi = i; }
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const float ov = __shfl_xor_sync(kFull, bv, o);
-                const int oi = __shfl_xor_sync(kFull, bi, o);
+            float bv = tl[(px * NWARP) * 2];
+            int bi = reinterpret_cast<int *>(tl)[(px * NWARP) * 2 + 1];
+            for (int q = 1; q < nsl; ++q) {
+                const float ov = tl[(px * NWARP + q) * 2];
+                const int oi = reinterpret_cast<int *>(tl)[(px * NWARP + q) * 2 + 1];
                 if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
             }
-            out.t = bi;
+            out.snr = s; out.k = k; out.j = j; out.t = bi; out.mu = rmu; out.sigma = rsg; out.u = uu;
         }
-        int last = 0;
-        if (lane == 0) {
-            P.partials[(size_t)p * NGRP + g] = out;
-            __threadfence(); // the partial is visible before the ticket is taken
-            const int prev = atomicAdd(P.counter + p, 1);
-            last = (prev == NGRP - 1);
-            if (last) {
-                P.counter[p] = 0; // ready for the next launch
-                __threadfence();
-            }
-        }
-        last = __shfl_sync(kFull, last, 0);
-        if (last && lane == 0) { // the pixel's last group: best partial -> outputs
+        P.partials[(size_t)p * NGRP + g] = out;
+        __threadfence(); // the partial is visible before the ticket is taken
+        const int prev = atomicAdd(P.counter + p, 1);
+        if (prev == NGRP - 1) { // the pixel's last group: best partial -> outputs
+            P.counter[p] = 0;   // ready for the next launch
+            __threadfence();
             Partial4 b;
             b.snr = -S4_INF; b.k = -1; b.j = -1; b.t = -1; b.mu = 0.f; b.sigma = 0.f; b.u = -1; b.pad = 0;
             const int4 *pp = reinterpret_cast<const int4 *>(P.partials + (size_t)p * NGRP);
