@@ -292,6 +292,22 @@ int nsfrb_cluster(nsfrb_plan *plan, const float *snr_map, const int32_t *argmax,
                   int32_t *result, void *stream);
 
 /*
+ * nsfrb_cluster for callers that may not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc).  Same computation and outputs as nsfrb_cluster (readings R25-R28), but
+ * no plan is needed -- nx, ny and the threshold are arguments -- and the kernel's workspace is a fixed array in the
+ * library's device image (38 144 bytes, held by every GPU that loads the library until the process exits).  The call
+ * makes no cudaMalloc / cudaFree and no allocating library call: one 256-byte cudaMemsetAsync and one kernel launch on
+ * `stream`, on the CURRENT device (the first call on a device also looks the array's address up).
+ *   Limits: nx*ny <= 16 777 216 pixels, 1 <= topn <= 32; beyond them NSFRB_EINVAL with a message naming the limit.
+ *   All calls in the process share the workspace: calls on one GPU must be stream-ordered (or otherwise not overlap);
+ *   two that run concurrently race.  The workspace keeps the previous call's contents; the call clears what it needs.
+ *   Arguments and outputs as nsfrb_cluster; snr_map is [ny][nx], argmax [3][nx*ny].
+ */
+int nsfrb_cluster_static(int nx, int ny, float threshold, const float *snr_map, const int32_t *argmax,
+                         const float *psf, const uint8_t *mask, int mh, int mw, int topn, nsfrb_cand *top,
+                         double *wsnr, int32_t *members, int32_t *result, void *stream);
+
+/*
  * Harness access to the plan-specialised real-time kernel: for the plan the first ten
  * arguments describe (as nsfrb_plan_create) and a first chunk of chunk_nt samples, writes either the CUDA
  * source the library compiles at the first nsfrb_stream_push (want_cubin = 0) or its sm_100a cubin

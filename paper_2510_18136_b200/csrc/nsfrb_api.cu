@@ -782,6 +782,28 @@ int nsfrb_cluster(nsfrb_plan *pl, const float *snr_map, const int32_t *argmax, c
     return NSFRB_OK;
 }
 
+int nsfrb_cluster_static(int nx, int ny, float threshold, const float *snr_map, const int32_t *argmax, const float *psf,
+                         const uint8_t *mask, int mh, int mw, int topn, nsfrb_cand *top, double *wsnr, int32_t *members,
+                         int32_t *result, void *stream)
+{
+    if (!snr_map || !argmax || !psf || !mask || !top || !wsnr || !members || !result)
+        return fail(NSFRB_EINVAL, "null pointer");
+    if (nx < 1 || ny < 1) return fail(NSFRB_EINVAL, "non-positive image size");
+    if ((long long)nx * ny > (long long)cluster_static_max_npix()) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "nsfrb_cluster_static: %lld pixels exceed the static workspace's limit of %d (use nsfrb_cluster)",
+                 (long long)nx * ny, cluster_static_max_npix());
+        return fail(NSFRB_EINVAL, buf);
+    }
+    if (mh < 1 || mw < 1) return fail(NSFRB_EINVAL, "non-positive PSF size");
+    if (topn < 1 || topn > cluster_max_top()) return fail(NSFRB_EINVAL, "topn outside 1..32 (the static workspace holds 32 keys per CTA)");
+    if (std::isnan(threshold)) return fail(NSFRB_EINVAL, "threshold is NaN");
+    CU(launch_cluster_static(snr_map, argmax, nx * ny, nx, threshold, psf, mask, mh, mw, topn, top, wsnr, members, result,
+                             static_cast<cudaStream_t>(stream)),
+       "k_cluster launch (static workspace)");
+    return NSFRB_OK;
+}
+
 int nsfrb_peaks_count(void) { return peaks_num_tests(); }
 const char *nsfrb_peaks_name(int test) { return peaks_name(test); }
 int nsfrb_measure_peaks(int iters, double *per_s, double *per_clk_sm, void *stream)

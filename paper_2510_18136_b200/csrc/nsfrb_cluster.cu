@@ -6,6 +6,8 @@
 //   k_cluster   one launch: every CTA selects the N best (S/N, pixel) keys of its slice of the map by N rounds of
 //               "largest key below the previous winner"; the last CTA to finish (ticket) merges the per-CTA lists
 //               the same way, then one thread per centre walks the N candidates in rank order.
+#include <mutex>
+
 #include "nsfrb_internal.h"
 
 namespace nsfrb {
@@ -266,6 +268,67 @@ cudaError_t launch_cluster(const float *snr_map, const int32_t *argmax, int npix
     P.threshold = threshold;
     k_cluster<<<grid, kCluThreads, 0, st>>>(P);
     return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// nsfrb_cluster_static: the same kernel for callers that may not allocate (CUDA graph capture, serving loops, harnesses
+// that forbid cudaMalloc).  Its workspace -- the ticket (first 256 bytes) and the per-CTA key lists,
+// kStaticCtas x kMaxTop keys -- is this file-scope array: 38 144 bytes that every GPU which loads the library holds
+// until exit.  All calls share it, so two calls that overlap on one GPU (different streams) race; it keeps the last
+// call's contents: the key lists are fully rewritten by every launch before they are read, the ticket is cleared on the
+// caller's stream before every launch.
+// In host code `g_cluster_scratch` is only a stand-in for the symbol, not a device address: the address comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticCtas = 148;                 // cluster_grid never launches more CTAs
+constexpr int kStaticMaxNpix = 1 << 24;          // stated limit of the entry point (a 4096 x 4096 map)
+constexpr int kStaticWords = 32 + kStaticCtas * kMaxTop; // 64-bit words: 256-byte header + keys
+static __device__ __align__(256) unsigned long long g_cluster_scratch[kStaticWords];
+
+constexpr int kMaxDevices = 64;
+unsigned long long *g_scratch_addr[kMaxDevices] = {nullptr};
+std::mutex g_scratch_mutex;
+
+// device address of the scratch on the current device (looked up once per device)
+cudaError_t cluster_static_scratch(unsigned long long **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_scratch_mutex);
+    if (!g_scratch_addr[dev]) {
+        unsigned long long *ptr = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void **>(&ptr), g_cluster_scratch);
+        if (e != cudaSuccess) return e;
+        if (!ptr) return cudaErrorInvalidSymbol;
+        g_scratch_addr[dev] = ptr;
+    }
+    *out = g_scratch_addr[dev];
+    return cudaSuccess;
+}
+
+} // namespace
+
+int cluster_static_max_npix() { return kStaticMaxNpix; }
+
+// No cudaMalloc/cudaFree and no allocating library call on this path: symbol lookup (first call per device), one
+// 256-byte cudaMemsetAsync, one kernel launch.
+cudaError_t launch_cluster_static(const float *snr_map, const int32_t *argmax, int npix, int nx, float threshold,
+                                  const float *psf, const uint8_t *mask, int mh, int mw, int topn, nsfrb_cand *top,
+                                  double *wsnr, int32_t *members, int32_t *result, cudaStream_t st)
+{
+    if (npix < 1 || npix > kStaticMaxNpix || topn < 1 || topn > kMaxTop || cluster_grid(npix) > kStaticCtas)
+        return cudaErrorInvalidValue; // (the C entry point reports these with their own messages first)
+    unsigned long long *scratch = nullptr;
+    cudaError_t e = cluster_static_scratch(&scratch);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(scratch, 0, 256, st); // the ticket must start at zero whatever an earlier call left behind
+    if (e != cudaSuccess) return e;
+    return launch_cluster(snr_map, argmax, npix, nx, threshold, psf, mask, mh, mw, topn, scratch + 32,
+                          reinterpret_cast<unsigned int *>(scratch), top, wsnr, members, result, st);
 }
 
 } // namespace nsfrb

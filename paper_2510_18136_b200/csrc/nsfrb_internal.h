@@ -199,6 +199,11 @@ cudaError_t launch_cluster(const float *snr_map, const int32_t *argmax, int npix
                            const float *psf, const uint8_t *mask, int mh, int mw, int topn, void *ws,
                            unsigned int *ticket, nsfrb_cand *top, double *wsnr, int32_t *members, int32_t *result,
                            cudaStream_t st);
+// the same kernel with its workspace in a file-scope __device__ array (nsfrb_cluster.cu): allocates nothing
+int cluster_static_max_npix();
+cudaError_t launch_cluster_static(const float *snr_map, const int32_t *argmax, int npix, int nx, float threshold,
+                                  const float *psf, const uint8_t *mask, int mh, int mw, int topn, nsfrb_cand *top,
+                                  double *wsnr, int32_t *members, int32_t *result, cudaStream_t st);
 size_t search_smem_bytes(int nchan, int RS, int H, int tab_cap);
 // on-chip ceilings (nsfrb_peaks.cu)
 int peaks_num_tests();

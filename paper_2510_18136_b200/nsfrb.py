@@ -47,7 +47,7 @@ EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stre
            "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes",
            "nsfrb_psf_mask", "nsfrb_cluster", "nsfrb_median_subtract",
            "nsfrb_stream_push_host_async", "nsfrb_stream_wait", "nsfrb_stream_set_running_sigma",
-           "nsfrb_peaks_count", "nsfrb_peaks_name", "nsfrb_measure_peaks", "nsfrb_plan_prepare")
+           "nsfrb_peaks_count", "nsfrb_peaks_name", "nsfrb_measure_peaks", "nsfrb_plan_prepare", "nsfrb_cluster_static")
 
 _lib = None
 
@@ -111,6 +111,9 @@ def lib() -> ctypes.CDLL:
         L.nsfrb_psf_mask.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_double, vp, vp, vp]
         L.nsfrb_cluster.restype = ctypes.c_int
         L.nsfrb_cluster.argtypes = [vp, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, vp, vp, vp, vp, vp]
+        L.nsfrb_cluster_static.restype = ctypes.c_int
+        L.nsfrb_cluster_static.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_float, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
+                                           ctypes.c_int, vp, vp, vp, vp, vp]
         L.nsfrb_plan_prepare.restype = ctypes.c_int
         L.nsfrb_plan_prepare.argtypes = [vp, ctypes.c_int, ctypes.c_int]
         L.nsfrb_peaks_count.restype = ctypes.c_int
@@ -248,6 +251,28 @@ class ClusterResult:
         cands = self.top.cpu().numpy().view(CAND_DTYPE)[:n].copy()
         return dict(cands=cands, pixels=[int(p) for p in cands["pixel"]], wsnr=self.wsnr.cpu().numpy()[:n].tolist(),
                     members=self.members.cpu().numpy()[:n].tolist(), best=best)
+
+
+def alloc_cluster_result(topn: int, device="cuda") -> ClusterResult:
+    """Output buffers of nsfrb_cluster / nsfrb_cluster_static for `topn` candidates (reusable from call to call)."""
+    n = max(int(topn), 1)
+    return ClusterResult(torch.empty(n * CAND_DTYPE.itemsize, dtype=torch.uint8, device=device),
+                         torch.empty(n, dtype=torch.float64, device=device),
+                         torch.empty(n, dtype=torch.int32, device=device), torch.empty(2, dtype=torch.int32, device=device))
+
+
+def cluster_static(snr_map: torch.Tensor, argmax: torch.Tensor, nx: int, ny: int, threshold: float, psf: torch.Tensor,
+                   mask: torch.Tensor, topn: int = 10, out: ClusterResult | None = None, stream=None) -> ClusterResult:
+    """nsfrb_cluster_static: nsfrb_cluster without a plan and without any device allocation inside the library (its
+    workspace is a fixed array in the library's device image).  Pass `out` (alloc_cluster_result) to reuse the output
+    buffers; calls must not overlap on the GPU (they share the workspace)."""
+    res = out if out is not None else alloc_cluster_result(topn, snr_map.device)
+    s = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().nsfrb_cluster_static(int(nx), int(ny), float(threshold), snr_map.data_ptr(), argmax.data_ptr(),
+                                      psf.data_ptr(), mask.data_ptr(), psf.shape[0], psf.shape[1], int(topn),
+                                      res.top.data_ptr(), res.wsnr.data_ptr(), res.members.data_ptr(), res.result.data_ptr(),
+                                      int(s.cuda_stream)))
+    return res
 
 
 class Plan:
