@@ -1,13 +1,16 @@
 #!/usr/bin/env python
 """bench.py -- headline benchmark of the B200-native NSFRB search (contract: task prompt, section 4).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4|c5|c1] [--extra c3,c5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2|c3|c4|c5|c1] [--no-extra] [--impl reference]
 
 A step is one pass of the whole hot path over one batch of synthetic input:
   c2 (default; BASELINE.json configs[1], the real-time config the chunk-latency metric is quoted on):
        one nsfrb_stream_push of a 25-sample chunk into the full 1536-sample ring (steady state);
   c3/c4/c5/c1: one nsfrb_search of the whole cube.
 metric = Gcells/s, a cell being one (pixel, DM, width, start-sample) S/N evaluation, counted exactly.
+The default line (c2, one GPU) also carries a `workloads` object: c3, c4 and c5 timed in the same run (3 steps each), with
+their per-kernel split and both roofline fractions (BASELINE.json's contract formula and the full FP32 count), against
+on-chip peaks measured in the same run (nsfrb_measure_peaks).  --no-extra skips them.
 N > 1 (torchrun): the path does not shard below a pixel and BASELINE.json fixes the build at one GPU,
 so every rank runs an independent replica of the same workload ("replicas only", weak scaling).
 """
@@ -30,8 +33,9 @@ sys.path.insert(0, ROOT)
 from paper_2510_18136_b200 import workloads as W  # noqa: E402
 
 CHUNK_DURATION_MS = 25 * W.TSAMP_S * 1e3  # 3355 ms (25 samples x 134 ms)
-# DRAM bytes (read + write) of one launch of the dominant kernel, from `ncu --set full`
-NCU_TRAFFIC_BYTES = {"c2": 5.58e9}  # 5.40 GB read + 0.18 GB written by one k_stream launch (profiles/r01_v6.md)
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed `ncu --set full`
+# capture named beside it (a constant of that capture, not measured in this run)
+NCU_TRAFFIC = {"c2": (5.58e9, "profiles/r01_v6_k_stream_c2_details.csv (k_stream as of round 1, commit 0abfa95)")}
 
 
 # ---------------------------------------------------------------------------- helpers
@@ -243,6 +247,78 @@ def time_steps(fn, steps, warmup, flush=None):
     return [a.elapsed_time(b) for a, b in ev]
 
 
+def offline_roofline(wl, bench, search_ms, ms_per_step, hbm_peak, peak_src, onchip, sm_max_mhz):
+    """BASELINE.json's contract roofline -- the slower of (cube bytes once / HBM) and (shift-adds + prefix adds) / FP32 issue
+    rate -- and, beside it, the full FP32 count of SURVEY.md 8(d) (nchan + 3 + 2 nW lane-ops per (pixel, DM, sample)).
+    The FP32 issue rate is the FADD rate nsfrb_measure_peaks achieved in this run; the theoretical 148 x 128 x clock is
+    reported next to it."""
+    info = bench.info
+    alu_theory = 148 * 128 * sm_max_mhz * 1e6 / 1e12          # T lane-ops/s
+    alu_peak = onchip["fadd"]["per_s"] / 1e12 if onchip else alu_theory
+    alu_src = "measured FADD issue rate (nsfrb_measure_peaks, this run)" if onchip else "148 SMs x 128 lanes x sm_max_mhz (not measured)"
+    T_sum = sum(wl.nt - int(x) for x in bench.delays.max(axis=1))        # valid samples over all DM trials
+    contract_ops = (info["shift_adds_per_pixel"] + T_sum) * wl.npix
+    full_ops = (wl.nchan + 3 + 2 * len(wl.width_list)) * T_sum * wl.npix
+    t_hbm = bench.kernel_bytes() / (hbm_peak * 1e9)
+    t_alu = contract_ops / (alu_peak * 1e12)
+    t_full = full_ops / (alu_peak * 1e12)
+    if t_alu > t_hbm:
+        ach = contract_ops / (search_ms * 1e-3) / 1e12
+        roof = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "T lane-ops/s", "frac": ach / alu_peak,
+                "peak_source": alu_src, "algorithmic_ops": contract_ops}
+    else:
+        ach = bench.kernel_bytes() / (search_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak,
+                "peak_source": peak_src}
+    contract_ms = max(t_hbm, t_alu) * 1e3
+    roof.update({"traffic": None, "kernel": "k_search4", "kernel_ms": search_ms, "share_of_step": search_ms / ms_per_step,
+                 "algorithmic_bytes": bench.kernel_bytes(), "contract_roofline_ms": contract_ms,
+                 "step_frac": contract_ms / ms_per_step,
+                 "full_count_ops": full_ops, "full_count_roofline_ms": t_full * 1e3,
+                 "full_count_frac": t_full * 1e3 / search_ms, "full_count_step_frac": t_full * 1e3 / ms_per_step,
+                 "alu_peak_theoretical": alu_theory})
+    return roof
+
+
+def measure_offline_workload(name, nsfrb, hbm_peak, peak_src, onchip, sm_max_mhz, local, steps=3, warmup=3):
+    """One entry of the `workloads` object: c3 / c4 / c5 at BASELINE size, `steps` timed nsfrb_search calls."""
+    wl = W.config(name)
+    need = wl.nchan * wl.nt * wl.npix * 4 + (6 << 30)
+    if torch.cuda.mem_get_info()[0] < need:
+        return {"skipped": f"needs {need >> 30} GiB of free device memory"}
+    bench = OfflineBench(wl, nsfrb)
+    bench.plan.prepare()
+    sampler = ClockSampler(local)
+    sampler.start()
+    t0 = time.perf_counter()
+    per_step = time_steps(bench.step, steps, warmup)
+    while time.perf_counter() - t0 < 1.0:            # keep the load up until nvidia-smi has sampled it
+        bench.step()
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = float(np.mean(per_step))
+    bench.plan.set_profiling(True)
+    kms = []
+    for _ in range(3):
+        bench.step()
+        kms.append(bench.plan.kernel_ms())
+    bench.plan.set_profiling(False)
+    kernel_ms = {k: float(np.mean([m[k] for m in kms])) for k in kms[0]}
+    launches = bench.plan.last_launches()
+    roof = offline_roofline(wl, bench, kernel_ms["search"], ms, hbm_peak, peak_src, onchip, sm_max_mhz)
+    out = {"workload": f"{wl.name}: {wl.note}", "nchan": wl.nchan, "nt": wl.nt, "nx": wl.nx, "ny": wl.ny, "ndm": len(wl.dm_list),
+           "ndm_unique": bench.info["ndm_unique"], "nwidth": len(wl.width_list), "cells_per_step": bench.cells_per_step,
+           "steps": steps, "warmup": warmup, "ms_per_step": ms, "ms_per_step_all": per_step,
+           "value": bench.cells_per_step / (ms * 1e-3) / 1e9, "unit": "Gcells/s", "kernel_ms": kernel_ms,
+           "gpu_launches_per_step": launches, "workspace_bytes": bench.plan.info()["workspace_bytes"],
+           "contract_roofline_ms": roof["contract_roofline_ms"], "contract_frac": roof["step_frac"],
+           "full_count_roofline_ms": roof["full_count_roofline_ms"], "full_count_frac": roof["full_count_step_frac"],
+           "roofline": roof, "clocks": clocks, "l2": "inputs larger than L2"}
+    del bench
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_cuda_arm(args, rank, world, local):
     from paper_2510_18136_b200 import nsfrb
     torch.cuda.set_device(local)
@@ -329,33 +405,31 @@ def run_cuda_arm(args, rank, world, local):
 
     if rank != 0:
         return
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    try:
+        onchip = measure_onchip_peaks(nsfrb)
+    except Exception as exc:  # the roofline then falls back to the theoretical issue rate, and says so
+        onchip = None
+        print(f"nsfrb_measure_peaks failed: {exc}", file=sys.stderr)
     alg_bytes = bench.algorithmic_bytes()
     kern_bytes = bench.kernel_bytes()
-    achieved = kern_bytes / (dominant_ms * 1e-3) / 1e9
-    dom_name = "k_stream" if wl.streaming else "k_search"
-    # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu capture (profiles/)
-    traffic = NCU_TRAFFIC_BYTES.get(wl.name)
     info = bench.info
-    roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-            "traffic": traffic, "peak_source": peak_src, "kernel": dom_name, "kernel_ms": dominant_ms,
-            "share_of_step": dominant_ms / ms_per_step, "algorithmic_bytes": kern_bytes,
-            "step_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / hbm_peak}
-    if not wl.streaming:
-        # BASELINE.json's roofline: the slower of (cube bytes once / HBM) and (shift-adds + prefix adds) / FP32 issue
-        # rate.  FP32 issue peak = 148 SMs x 128 lanes x SM clock (measured 123-134 lane-ops/clk/SM).
-        sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
-        alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e12  # T lane-ops/s
-        prefix_adds = sum(wl.nt - int(x) for x in bench.delays.max(axis=1))
-        alu_ops = (info["shift_adds_per_pixel"] + prefix_adds) * wl.npix
-        t_hbm, t_alu = kern_bytes / (hbm_peak * 1e9), alu_ops / (alu_peak * 1e12)
-        if t_alu > t_hbm:
-            ach = alu_ops / (dominant_ms * 1e-3) / 1e12
-            roof.update({"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "T lane-ops/s", "frac": ach / alu_peak,
-                         "peak_source": "148 SMs x 128 FP32 lanes x sm_max_mhz (DESIGN.md sec. 7)",
-                         "algorithmic_ops": alu_ops, "contract_roofline_ms": t_alu * 1e3,
-                         "step_frac": alu_ops / (ms_per_step * 1e-3) / 1e12 / alu_peak})
-        else:
-            roof["contract_roofline_ms"] = t_hbm * 1e3
+    if wl.streaming:
+        achieved = kern_bytes / (dominant_ms * 1e-3) / 1e9
+        # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu capture named in traffic_source
+        traffic, traffic_src = NCU_TRAFFIC.get(wl.name, (None, None))
+        # what the march really reads: with the incremental statistics it stops after the widest window
+        rows_read = min(wl.nt, int(info["wmax"]) + wl.chunk_nt)
+        read_bytes = rows_read * wl.nchan * wl.npix * 4
+        roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src, "kernel": "k_stream",
+                "kernel_ms": dominant_ms, "share_of_step": dominant_ms / ms_per_step, "algorithmic_bytes": kern_bytes,
+                "step_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / hbm_peak,
+                "note": "achieved/frac use the contract numerator (the ring once, SURVEY.md 8(d)); the kernel reads less: see achieved_read",
+                "read_bytes": read_bytes, "achieved_read": read_bytes / (dominant_ms * 1e-3) / 1e9,
+                "frac_read": read_bytes / (dominant_ms * 1e-3) / 1e9 / hbm_peak}
+    else:
+        roof = offline_roofline(wl, bench, dominant_ms, ms_per_step, hbm_peak, peak_src, onchip, sm_max)
     line = {
         "metric": "Gcells/s (pixel*DM*width*sample)", "value": value, "unit": "Gcells/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -377,7 +451,19 @@ def run_cuda_arm(args, rank, world, local):
         line["chunk_latency_ms"] = ms_per_step
         line["chunk_duration_ms"] = CHUNK_DURATION_MS
         line["chunk_latency_frac"] = ms_per_step / CHUNK_DURATION_MS
+    line["onchip_peaks"] = onchip
     line["cpu_baseline"] = cpu_baseline(wl, bench, budget_s=args.cpu_budget) if world == 1 and not args.no_cpu else None
+    if wl.name == "c2" and world == 1 and not args.no_extra and not args.cubes and not args.running:
+        # the three offline configs in the same run (BASELINE.json: "on all five configs"); c2 stays the headline value
+        del bench
+        torch.cuda.empty_cache()
+        line["workloads"] = {}
+        for name in ("c3", "c4", "c5"):
+            try:
+                line["workloads"][name] = measure_offline_workload(name, nsfrb, hbm_peak, peak_src, onchip, sm_max, local)
+            except Exception as exc:
+                line["workloads"][name] = {"error": f"{type(exc).__name__}: {exc}"}
+                torch.cuda.empty_cache()
     print(json.dumps(line))
 
 
@@ -455,7 +541,9 @@ def run_reference_arm(args, rank, world):
         "impl": "reference", "metric": "Gcells/s (pixel*DM*width*sample)", "value": value, "unit": "Gcells/s",
         "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": s_per_step * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"{wl.name}: {wl.note}", "sample": sample},
+        "config": {"workload": f"{wl.name}: {wl.note}", "nchan": wl.nchan, "nt": wl.nt, "nx": wl.nx, "ny": wl.ny,
+                   "ndm": len(wl.dm_list), "nwidth": len(wl.width_list),
+                   "cells_per_step": int(wl.npix * per_pixel_cells), "sample": sample},
         "cpu_baseline": {"value": value, "unit": "Gcells/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": "Gcells/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -602,6 +690,7 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="c2: do not also time c3, c4, c5 (the `workloads` object)")
     ap.add_argument("--cubes", action="store_true", help="c2: also write the S/N and TOA cubes every push (NEXT 3)")
     ap.add_argument("--running", action="store_true", help="c2: also the running-sigma maps every push (NEXT 1)")
     ap.add_argument("--op", default="search", choices=["search", "bin", "cluster", "median", "peaks"],
