@@ -88,7 +88,18 @@ size_t search4_smem(int H, int nwarp, int pxi, int nt)
 
 bool search4_geo(const nsfrb_plan *pl, Geo &g)
 {
-    g.nwarp = env_int("NSFRB_SEARCH_WARPS", 16) == 8 ? 8 : 16; // trials per CTA; 8: two CTAs per SM
+    // trials (= warps) per CTA: 16 by default; 24 (80 registers per thread, more latency hidden) where a power-of-two ring
+    // still fits 24 warps and the last group is no emptier than with 16 -- short series with few channels (C4: 141 -> 122 ms;
+    // C3 and C5 are slower with 24: 32 trials split 24 + 8, 64 channels want the registers).  NSFRB_SEARCH_WARPS overrides.
+    g.nwarp = env_int("NSFRB_SEARCH_WARPS", 0);
+    if (g.nwarp != 8 && g.nwarp != 16 && g.nwarp != 24 && g.nwarp != 32) {
+        const int hmin0 = round_up(std::max(pl->wmax_used, 1) + kBlockLen + 32, 64);
+        int hp = 64;
+        while (hp < hmin0) hp <<= 1;
+        const int pad16 = (pl->nuniq + 15) / 16 * 16 - pl->nuniq, pad24 = (pl->nuniq + 23) / 24 * 24 - pl->nuniq;
+        const bool fits24 = search4_smem(hp, 24, 16, pl->nt) <= kSmemLimit;
+        g.nwarp = (fits24 && pl->nchan <= 24 && pad24 <= pad16) ? 24 : 16;
+    }
     g.ngroups = (pl->nuniq + g.nwarp - 1) / g.nwarp;
     // pixel batches: about NSFRB_SEARCH_BATCH_MB (default 1024) of workspace each, at least ~8192 items per launch
     const size_t bpp = (size_t)pl->nchan * pl->pitch * sizeof(float);
@@ -111,7 +122,7 @@ bool search4_geo(const nsfrb_plan *pl, Geo &g)
     g.pxi = std::min(g.pxi, g.nwarp);
     // ring: wmax + one block + the rows the bounds read, a multiple of 64; a power of two (every wrap one AND) when shared
     // memory allows
-    const size_t limit = kSmemLimit / (16 / g.nwarp) - (g.nwarp == 8 ? 1024 : 0);
+    const size_t limit = kSmemLimit / std::max(1, 16 / g.nwarp) - (g.nwarp == 8 ? 1024 : 0);
     const int hmin = round_up(std::max(pl->wmax_used, 1) + kBlockLen + 32, 64);
     int h2 = 64;
     while (h2 < hmin) h2 <<= 1;
@@ -229,7 +240,7 @@ int search4_prepare(nsfrb_plan *pl, std::string &err)
     if (e == cudaSuccess) { // one CTA per SM, each with the dedispersed series of its item in flight
         int nsm = 0;
         e = cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, pl->device);
-        s4->grid = std::max(1, nsm) * (16 / g.nwarp);
+        s4->grid = std::max(1, nsm) * std::max(1, 16 / g.nwarp);
         s4->dpitch = g.dpitch;
         const size_t sb = (size_t)s4->grid * g.pxi * g.nwarp * g.dpitch * sizeof(float);
         if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&s4->scratch), sb);

@@ -688,7 +688,7 @@ __device__ __forceinline__ void run_item(const Search4Params &P, float *smem, in
 
 } // namespace s4
 
-extern "C" __global__ void __launch_bounds__(s4::NTHR, 16 / NWARP) k_search4(const Search4Params P)
+extern "C" __global__ void __launch_bounds__(s4::NTHR, (NWARP < 16 ? 16 / NWARP : 1)) k_search4(const Search4Params P)
 {
     extern __shared__ __align__(16) float smem[];
     const int noct = (P.npb + PXI - 1) / PXI;

@@ -323,6 +323,28 @@ struct StreamState {
 
 namespace {
 
+// base[c][p] = the lower median of the first min(chunk_nt, 32) samples of the first chunk (reading R32): the stored level every
+// ring value is taken relative to.  It cancels in D - mu; it only has to be NEAR the data so that float32 storage keeps
+// its resolution -- a single outlier (the very first sample, say) must not become the reference.
+__global__ void __launch_bounds__(256) k_stream_base(const float *__restrict__ chunk, float *__restrict__ base, int npix, int chunk_nt)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.y;
+    if (p >= npix) return;
+    const int m = chunk_nt < 32 ? chunk_nt : 32;
+    const float *src = chunk + (size_t)c * chunk_nt * npix + p;
+    float v[32];
+    for (int i = 0; i < m; ++i) v[i] = src[(size_t)i * npix];
+    float med = v[0];
+    for (int i = 0; i < m; ++i) { // the element with exactly (m - 1) / 2 elements before it in (value, index) order
+        int rank = 0;
+        for (int j = 0; j < m; ++j) rank += (v[j] < v[i]) || (v[j] == v[i] && j < i);
+        if (rank == (m - 1) / 2) med = v[i];
+    }
+    if (!(med == med) || fabsf(med) > 3.0e38f) med = 0.f; // non-finite data: no reference level
+    base[(size_t)c * npix + p] = med;
+}
+
 // a8: chunk[c][i][p] - base[c][p] -> ring[p/32][guard + slot (and + L)][c][p%32], slot = (slot0 + i) mod L
 template <typename V>
 __global__ void __launch_bounds__(256) k_stream_push(const V *__restrict__ chunk, V *__restrict__ ring, V *__restrict__ base,
@@ -705,6 +727,12 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         ++*launches;
     }
     // ---- a8: ring update
+    if (n_prev == 0) { // the reference level of every (channel, pixel), from the first chunk
+        dim3 grid((pl->npix + 255) / 256, pl->nchan);
+        k_stream_base<<<grid, 256, 0, st>>>(chunk, ss->base, pl->npix, chunk_nt);
+        SCU(cudaGetLastError(), "k_stream_base launch");
+        ++*launches;
+    }
     {
         const bool v4 = (pl->npix % 4 == 0) && ((reinterpret_cast<uintptr_t>(chunk) & 15u) == 0);
         const int npv = v4 ? pl->npix / 4 : pl->npix;
@@ -713,10 +741,10 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         if (v4)
             k_stream_push<float4><<<grid, 256, 0, st>>>(reinterpret_cast<const float4 *>(chunk), reinterpret_cast<float4 *>(ss->ring),
                                                         reinterpret_cast<float4 *>(ss->base), npv, pl->nchan, chunk_nt, L, ss->guard, rows,
-                                                        (int)(n_prev % L), n_prev == 0 ? 1 : 0);
+                                                        (int)(n_prev % L), 0);
         else
             k_stream_push<float><<<grid, 256, 0, st>>>(chunk, ss->ring, ss->base, npv, pl->nchan, chunk_nt, L, ss->guard, rows,
-                                                       (int)(n_prev % L), n_prev == 0 ? 1 : 0);
+                                                       (int)(n_prev % L), 0);
         SCU(cudaGetLastError(), "k_stream_push launch");
         ++*launches;
     }

@@ -667,22 +667,11 @@ struct StatsParams {
 
 namespace sk {
 
-template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &P, int lane, int pix, bool live)
+// S1 += sum D, S2 += sum D^2 over cnt consecutive samples of trial U starting at ring pointer rp (lane = pixel).
+// (A sample's D is the same expression wherever it falls in a range: entering, leaving and rebuilding must agree bit for bit.)
+template <int U> __device__ __forceinline__ void stats_range(const float *rp, int cnt, double &a1, double &a2)
 {
-    constexpr long long dm = DMAX_TAB[U];
-    const long long b_prev = P.lo_prev > P.n_prev - dm ? P.lo_prev : P.n_prev - dm; // end of the previous valid set
-    long long ta, tb;
-    if (P.add) {
-        ta = b_prev > P.lo ? b_prev : P.lo;
-        tb = P.lo > P.n - dm ? P.lo : P.n - dm;
-    } else {
-        ta = P.lo_prev;
-        tb = P.lo < b_prev ? P.lo : b_prev;
-    }
-    const float *rp = P.ring + ((long long)blockIdx.x * ROWS + P.row_lo + (ta - P.ring_lo)) * (NCHAN * 32) + lane;
-    double a1 = 0.0, a2 = 0.0;
-    int i = (int)(tb - ta);
-    // (a sample's D is the same expression in both loops: it must not depend on where the sample falls in a range)
+    int i = cnt;
     for (; i >= 4; i -= 4, rp += 4 * NCHAN * 32) { // four samples per round: 4*NCHAN loads in flight
         float e[4][4] = {};
         sfor<0, 4>([&](auto q) {
@@ -701,27 +690,86 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
         a1 += D;
         a2 = fma(D, D, a2);
     }
-    if (!live) return;
+}
+// sum (D - centre)^2 over the same samples: the second pass of an exact two-pass variance
+template <int U> __device__ __forceinline__ double stats_centred(const float *rp, int cnt, double centre)
+{
+    double c2 = 0.0;
+    for (int i = cnt; i > 0; --i, rp += NCHAN * 32) {
+        float e[4] = {0.f, 0.f, 0.f, 0.f};
+        sfor<0, NCHAN>([&](auto c) { e[V(c) & 3] += __ldg(rp + (D_TAB[U][V(c)] * NCHAN + V(c)) * 32); });
+        const double x = (double)((e[0] + e[1]) + (e[2] + e[3])) - centre;
+        c2 = fma(x, x, c2);
+    }
+    return c2;
+}
+
+template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &P, int lane, int pix, bool live)
+{
+    constexpr long long dm = DMAX_TAB[U];
+    const long long b_prev = P.lo_prev > P.n_prev - dm ? P.lo_prev : P.n_prev - dm; // end of the previous valid set
+    long long ta, tb;
+    if (P.add) {
+        ta = b_prev > P.lo ? b_prev : P.lo;
+        tb = P.lo > P.n - dm ? P.lo : P.n - dm;
+    } else {
+        ta = P.lo_prev;
+        tb = P.lo < b_prev ? P.lo : b_prev;
+    }
+    const float *rbase = P.ring + ((long long)blockIdx.x * ROWS + P.row_lo) * (NCHAN * 32) + lane; // sample ring_lo
+    double a1 = 0.0, a2 = 0.0;
+    stats_range<U>(rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2);
     const long long o = (long long)U * NPIX + pix;
+    const double kNaN = __longlong_as_double(0x7ff8000000000000LL);
     if (!P.add) {
-        if (tb > ta) { P.s1[o] -= a1; P.s2[o] -= a2; }
+        if (live && tb > ta) {
+            // A leaving sample that dwarfs what stays behind (|D| beyond ~10^3 sigma sqrt(T)) has eaten the low bits of S2 when it
+            // entered, and a non-finite one has destroyed the sums: mark the series (NaN); the add pass rebuilds it from the ring.
+            const double r1 = P.s1[o] - a1, r2 = P.s2[o] - a2;
+            const bool bad = !(a2 <= 1048576.0 * fabs(r2)) || !(fabs(r1) <= 1.7e308);
+            P.s1[o] = bad ? kNaN : r1;
+            P.s2[o] = bad ? kNaN : r2;
+        }
         return;
     }
-    if (!P.first) { a1 += P.s1[o]; a2 += P.s2[o]; }
-    P.s1[o] = a1;
-    P.s2[o] = a2;
     const long long Tk = tb - P.lo; // tb = max(lo, n - dmax_u)
+    bool rebuild = false;
+    if (!P.first) {
+        a1 += P.s1[o];
+        a2 += P.s2[o];
+        rebuild = !(fabs(a1) <= 1.7e308) || !(fabs(a2) <= 1.7e308); // marked, or poisoned by a non-finite sample
+    }
+    if (__any_sync(0xffffffffu, rebuild)) { // warp = one trial, lanes = pixels: the whole valid set once more (rare)
+        double b1 = 0.0, b2 = 0.0;
+        stats_range<U>(rbase + (P.lo - P.ring_lo) * (NCHAN * 32), (int)Tk, b1, b2);
+        if (rebuild) { a1 = b1; a2 = b2; }
+    }
     float m = 0.f, dl = 0.f, rs = 0.f, sg = __int_as_float(0x7fc00000); // NaN sigma = "no valid sample yet"
+    double mean = 0.0, var = 0.0;
+    bool cancel = false;
     if (Tk >= 1) {
-        const double mean = a1 / (double)Tk, msq = a2 / (double)Tk;
-        double var = msq - mean * mean;
-        if (!(var > msq * 1e-13)) var = 0.0; // below the cancellation floor of the float64 sums: a constant series
+        const double msq = a2 / (double)Tk;
+        mean = a1 / (double)Tk;
+        var = msq - mean * mean;
+        cancel = msq > 0.0 && !(var >= 1e-8 * msq); // over half of float64's digits cancelled: |mean| > 10^4 sigma
+    }
+    if (__any_sync(0xffffffffu, cancel)) { // exact two-pass variance about the mean (reading R31)
+        const double c2 = stats_centred<U>(rbase + (P.lo - P.ring_lo) * (NCHAN * 32), (int)Tk, mean);
+        if (cancel) var = c2 / (double)Tk;
+    }
+    if (live) {
+        P.s1[o] = a1;
+        P.s2[o] = a2;
+    }
+    if (Tk >= 1) {
+        if (!(var > 0.0) && var == var) var = 0.0; // (a NaN stays a NaN: non-finite data in the ring)
         const double sigma = sqrt(var);
         m = (float)mean;
         dl = (float)(mean - (double)m);
-        rs = sigma > 0.0 ? (float)(1.0 / sigma) : 0.f;
+        rs = sigma > 0.0 ? (float)(1.0 / sigma) : (sigma == sigma ? 0.f : __int_as_float(0x7fc00000));
         sg = (float)sigma;
     }
+    if (!live) return;
     P.mu[o] = m;
     P.dlt[o] = dl;
     P.rsig[o] = rs;

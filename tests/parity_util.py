@@ -20,7 +20,7 @@ def tol(s):
 
 
 def check(cube_sel: np.ndarray, delays: np.ndarray, widths, gpu_snr: np.ndarray, gpu_arg: np.ndarray,
-          threshold: float, *, raw_end_min=0, t_offset=0, nthreads=8, max_adjudicated_frac=0.25, label=""):
+          threshold: float, *, raw_end_min=0, t_offset=0, nthreads=8, max_adjudicated_frac=0.10, label=""):
     """cube_sel: [nchan][nt][n] float32 (the pixels compared); gpu_snr [n]; gpu_arg [n][3].
     Returns a dict of counts; raises AssertionError with a readable message on any violation."""
     cube_sel = np.ascontiguousarray(cube_sel, dtype=np.float32)

@@ -32,6 +32,8 @@ def _offline(wl, cube, *, pixels=None, capacity=4096, label=None):
     pix = np.arange(wl.npix) if pixels is None else np.asarray(pixels)
     sub = cube[:, :, torch.as_tensor(pix, device=cube.device)].cpu().numpy()
     st = PU.check(sub, d_orc, wl.width_list, snr[pix], arg[pix], wl.threshold, label=label or wl.name)
+    print(f"[parity] {label or wl.name}: n={st['n']} exact={st['exact']} adjudicated={st['adjudicated']} "
+          f"undefined={st['undefined']} worst |d|/tol={st['worst_tol_frac']:.3f}")
     cs = PU.check_candidates(st["oracle"], pix, cands, nfound, wl.threshold, capacity, all_pixels_checked=pixels is None)
     # stored candidate records repeat the maps exactly
     for c in cands:
@@ -97,7 +99,7 @@ def test_scaled_configs(name, nx, ny, nt):
     cube = W.make_cube(wl, "cuda")
     pulses = _inject_all(wl, cube, d)
     st, cs, snr, arg = _offline(wl, cube)
-    assert st["exact"] >= 0.75 * st["n"], st
+    assert st["exact"] >= 0.9 * st["n"], st
     _check_recovery(wl, d, pulses, snr)
 
 
@@ -198,7 +200,7 @@ def test_stream_c2_scaled():
     wl = W.config("c2").scaled(12, 8)
     # first pushes (ring nearly empty), mid fill, the pushes around the ring wrap (1536/25 = 61.44), steady state
     stats = _stream_case(wl, 68, eval_at={0, 1, 2, 7, 30, 48, 60, 61, 62, 63, 67})
-    assert sum(s["exact"] for s in stats) >= 0.75 * sum(s["n"] - s["undefined"] for s in stats)
+    assert sum(s["exact"] for s in stats) >= 0.9 * sum(s["n"] - s["undefined"] for s in stats)
 
 
 def test_stream_small_ring_variable_chunks():
@@ -279,6 +281,152 @@ def test_stream_incremental_statistics_offsets_many_laps_and_reset(monkeypatch):
         if i >= 1:
             assert np.all(np.abs(snr - incr[(rep, i)]) <= 2 * PU.tol(snr)), (rep, i)
 
+def _scripted_stream(wl, chunks, eval_at, label, pixels=None, **check_kw):
+    """Push `chunks` (device tensors [nchan][c][npix]) through one plan; at the pushes in eval_at compare with the oracle on
+    the chronological ring contents (P-rule).  Returns {push: (snr, arg, oracle result)}."""
+    nsfrb = _nsfrb()
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    out_maps = {}
+    with nsfrb.Plan.for_workload(wl, cand_capacity=64) as plan:
+        out = plan.alloc_outputs()
+        hist, n = np.zeros((wl.nchan, 0, wl.npix), np.float32), 0
+        for i, ch in enumerate(chunks):
+            plan.stream_push(ch, out)
+            n_prev, n = n, n + ch.shape[1]
+            hist = np.concatenate([hist, ch.cpu().numpy()], axis=1)[:, -wl.nt:, :]
+            if i in eval_at:
+                torch.cuda.synchronize()
+                lo = max(0, n - wl.nt)
+                snr = out.snr_map.cpu().numpy()
+                arg = out.argmax.cpu().numpy().T.copy()
+                pix = np.arange(wl.npix) if pixels is None else np.asarray(pixels)
+                st = PU.check(hist[:, :, pix], d, wl.width_list, snr[pix], arg[pix], wl.threshold, raw_end_min=n_prev - lo,
+                              t_offset=lo, label=f"{label} push {i}", **check_kw)
+                out_maps[i] = (snr, arg, st["oracle"])
+    return out_maps
+
+
+def _small_stream_plan():
+    from dataclasses import replace
+    return replace(W.config("c2").scaled(7, 5, nt=200), width_list=np.asarray([1, 3, 9, 30, 100, 180], np.int32))
+
+
+def test_stream_statistics_survive_a_huge_sample_entering_and_leaving():
+    """one 1e8 sample in one channel enters Sum D^2 (~1e16) and, a ring length later, leaves.  The
+    float64 residue it would leave in the carried sums is removed: a leaving sample that dwarfs what stays marks the series
+    and the sums are rebuilt from the ring (R31).  Pushes before, while it is inside every trial's valid set, and
+    from the push at which it has left the ring must match the oracle.  (Push 10 is not compared: the sample has then left the
+    valid sets of the high-DM trials but is still in the ring, and differential dedispersion -- each trial formed from its
+    neighbour -- carries float32 rounding of the outlier, 6e-8 x 1e8, into them for that one push; R32.)"""
+    wl = _small_stream_plan()
+    g = torch.Generator(device="cuda").manual_seed(101)
+    chunks = [torch.randn((wl.nchan, 25, wl.npix), device="cuda", generator=g) for _ in range(24)]
+    chunks[3][2, 7, 5] = 1.0e8            # pixel 5, channel 2
+    chunks[3][4, 9, 11] = -3.0e7          # and a negative one elsewhere
+    # the sample entered at push 3 (absolute 82) leaves the 200-sample ring at push 11 (n = 300 > 82 + 200)
+    _scripted_stream(wl, chunks, {2, 3, 4, 9, 11, 12, 13, 20, 23}, "huge sample")
+
+
+def test_stream_first_sample_outlier_does_not_poison_the_baseline():
+    """(ii): the very first sample is a 1e4 outlier in every channel of some pixels.  The stored reference level is the
+    median of the first chunk (reading R32), not its first sample, so later ring values keep their float32 resolution."""
+    wl = _small_stream_plan()
+    g = torch.Generator(device="cuda").manual_seed(102)
+    chunks = [torch.randn((wl.nchan, 25, wl.npix), device="cuda", generator=g) for _ in range(14)]
+    chunks[0][:, 0, 3] = 1.0e4
+    chunks[0][:, 0, 20] = -1.0e4
+    chunks[0][1, 0, 8] = 5.0e3
+    _scripted_stream(wl, chunks, {0, 1, 2, 7, 8, 9, 13}, "first-sample outlier")
+
+
+def test_stream_non_finite_sample_stops_poisoning_once_it_has_left():
+    """a NaN sample must not kill its (pixel, trial) series until nsfrb_stream_reset: once it has left the ring
+    the sums are rebuilt and the pixel matches the oracle again (while it is inside, results are unspecified)."""
+    wl = _small_stream_plan()
+    g = torch.Generator(device="cuda").manual_seed(103)
+    chunks = [torch.randn((wl.nchan, 25, wl.npix), device="cuda", generator=g) for _ in range(16)]
+    chunks[2][3, 4, 9] = float("nan")     # absolute sample 54: gone once n > 254 + dmax, i.e. from push 10 on
+    chunks[2][0, 5, 17] = float("inf")
+    clean = [p for p in range(wl.npix) if p not in (9, 17)]
+    _scripted_stream(wl, chunks, {3, 6}, "NaN inside (other pixels)", pixels=clean)
+    _scripted_stream(wl, chunks, {11, 12, 15}, "NaN gone")
+
+
+def test_stream_levels_far_from_the_baseline():
+    """(iii): after the first chunk the level of every channel moves away from the stored baseline by `off` with unit
+    noise.  off = 300 (noise 3e-3 of the level): full parity.  off = 1e5: the float32 ring and sums cannot carry 1e-4
+    (documented limit, R32), but sigma must still be right -- the variance comes from the exact two-pass when
+    Sum D^2 - (Sum D)^2 / T cancels (R31) -- so the S/N stays within a few per cent, far from the sigma = 0 of a floor."""
+    wl = _small_stream_plan()
+    g = torch.Generator(device="cuda").manual_seed(104)
+
+    def make(off):
+        out = []
+        for i in range(13):
+            x = torch.randn((wl.nchan, 25, wl.npix), device="cuda", generator=g)
+            out.append(x + (off if i >= 1 else 0.0))
+        return out
+    _scripted_stream(wl, make(300.0), {1, 2, 8, 9, 12}, "level 300")
+    nsfrb = _nsfrb()
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    chunks = make(1.0e5)
+    with nsfrb.Plan.for_workload(wl, cand_capacity=64) as plan:
+        out = plan.alloc_outputs()
+        for ch in chunks:
+            plan.stream_push(ch, out)
+        torch.cuda.synchronize()
+        snr = out.snr_map.cpu().numpy()
+    hist = torch.cat(chunks, dim=1)[:, -wl.nt:, :].cpu().numpy()       # the level-0 chunk has left the ring
+    r = oracle.search(hist, d, wl.width_list, raw_end_min=wl.nt - 25, t_offset=len(chunks) * 25 - wl.nt)
+    assert np.all(np.isfinite(snr)) and np.all(snr > 1.0)
+    assert np.all(np.abs(snr - r.snr) <= 0.08 * np.abs(r.snr)), float(np.max(np.abs(snr - r.snr) / np.abs(r.snr)))
+
+
+def test_stream_five_thousand_pushes():
+    """(iv): 5 000 pushes (625 laps of the ring) of irregular sizes on the 7 x 5 plan: the carried float64 sums do not drift."""
+    wl = _small_stream_plan()
+    g = torch.Generator(device="cuda").manual_seed(105)
+    sizes = [25, 3, 25, 11, 40, 1]
+    big = torch.randn((wl.nchan, 4096, wl.npix), device="cuda", generator=g)
+    chunks, pos = [], 0
+    for i in range(5000):
+        c = sizes[i % len(sizes)]
+        if pos + c > big.shape[1]:
+            pos = (pos + 7) % 64
+        chunks.append((big[:, pos:pos + c, :] + 0.01 * (i % 13)).contiguous())
+        pos += c
+    _scripted_stream(wl, chunks, {0, 1, 50, 999, 2500, 4998, 4999}, "5000 pushes")
+
+
+def test_stream_running_sigma_trials_without_a_sample_on_the_first_pushes():
+    """with chunks shorter than the largest delay some trials have no valid sample on the first pushes; their
+    running variance must start at their first valid push (not from uninitialised memory), also after a reset."""
+    nsfrb = _nsfrb()
+    wl = W.config("c1")
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    assert int(d.max()) >= 6
+    g = torch.Generator(device="cuda").manual_seed(106)
+    alpha = 0.05
+    with nsfrb.Plan.for_workload(wl, cand_capacity=64) as plan:
+        out = plan.alloc_outputs()
+        run = (torch.full((wl.npix,), 7.0, device="cuda"), torch.zeros((3, wl.npix), dtype=torch.int32, device="cuda"))
+        plan.stream_set_running_sigma(alpha, *run)
+        for rep in range(2):
+            if rep:
+                plan.stream_reset()
+            ro = oracle.RunningStreamOracle(wl.nchan, wl.npix, wl.nt, d, wl.width_list, alpha)
+            for i in range(12):
+                chunk = torch.randn((wl.nchan, 3, wl.npix), device="cuda", generator=g) * (1.0 + i)
+                plan.stream_push(chunk, out)
+                torch.cuda.synchronize()
+                res_run = ro.push(chunk.cpu().numpy())
+                got = run[0].cpu().numpy()
+                want = res_run.snr
+                both = np.isfinite(want)
+                assert np.array_equal(np.isneginf(got), np.isneginf(want)), (rep, i)
+                assert np.all(np.abs(got[both] - want[both]) <= 2 * PU.tol(want[both])), (rep, i, float(np.max(np.abs(got[both] - want[both]))))
+
+
 # ----------------------------------------------------------------------------- edge and degenerate cases
 def test_degenerate_pixels_and_duplicate_unsorted_dms():
     from dataclasses import replace
@@ -345,49 +493,82 @@ def test_host_buffer_variants_match_device_path():
 
 
 # ----------------------------------------------------------------------------- BASELINE sizes, sampled pixels
-def _sample_pixels(wl, pulses, n_random, seed=7):
+def _sample_pixels(wl, pulses, n_random, seed=7, extra=()):
     rng = np.random.default_rng(seed)
     pix = set(int(pu.pixel) for pu in pulses)
     pix |= {0, 1, 31, 32, wl.nx - 1, wl.nx, wl.npix - 1, wl.npix - wl.nx}          # image corners / row edges
+    pix |= set(int(v) for v in extra if 0 <= int(v) < wl.npix)
     pix |= set(int(v) for v in rng.choice(wl.npix, n_random, replace=False))
     return np.asarray(sorted(pix))
 
 
-@pytest.mark.parametrize("name,n_random", [("c3", 40), ("c4", 300), ("c5", 10)])
+def _report(label, st):
+    """The P-rule's buckets ('report how many pixels fell into each bucket -- it should be a few %')."""
+    defined = max(st["n"] - st["undefined"], 1)
+    print(f"[parity] {label}: n={st['n']} exact={st['exact']} adjudicated={st['adjudicated']} "
+          f"({100.0 * st['adjudicated'] / defined:.2f} %) undefined={st['undefined']} worst |d|/tol={st['worst_tol_frac']:.3f}")
+
+
+@pytest.mark.parametrize("name,n_random", [("c3", 4096), ("c4", 4096), ("c5", 512)])
 def test_full_size_sampled(name, n_random):
-    """BASELINE.json sizes in the launch configuration bench.py times; the oracle checks a pixel sample
-    (every injected pixel + image edges + random pixels)."""
+    """BASELINE.json sizes in the launch configuration bench.py times; the oracle checks every injected pixel, the image
+    edges, the pixels on both sides of the layout kernel's 64-pixel tile edges and of the pixel-batch boundaries of the
+    search, and n_random random pixels (>= 4096; C5 at 0.25 core-s per pixel: 512)."""
+    import os
+    nsfrb = _nsfrb()
     wl = W.config(name)
-    need = 2.2 * wl.nchan * wl.nt * wl.npix * 4
+    need = wl.nchan * wl.nt * wl.npix * 4 + (8 << 30)
     if torch.cuda.mem_get_info()[0] < need:
         pytest.skip("not enough free device memory")
     d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
     cube = W.make_cube(wl, "cuda")
     pulses = _inject_all(wl, cube, d)
-    keep = pulses if name != "c5" else pulses[:12]
-    pix = _sample_pixels(wl, keep, n_random)
-    st, cs, snr, arg = _offline(wl, cube, pixels=pix, label=f"{name} full")
-    assert st["exact"] >= 0.75 * st["n"], st
+    # pixels around tile and batch edges: the batch holds about 1 GiB of [pixel][chan][time] workspace
+    batch = max(8, ((1 << 30) // (wl.nchan * ((wl.nt + 3) // 4 * 4) * 4)) & ~7)
+    edges = []
+    for b in (64, batch):
+        for k in (1, 2, 3, max(1, wl.npix // b - 1), wl.npix // b):
+            edges += [k * b - 2, k * b - 1, k * b, k * b + 1]
+    pix = _sample_pixels(wl, pulses, n_random, extra=edges)
+    d_orc = d
+    with nsfrb.Plan.for_workload(wl, cand_capacity=4096) as plan:
+        assert np.array_equal(plan.delays(), d_orc)
+        res = plan.search(cube)
+        torch.cuda.synchronize()
+        snr = res.snr_map.cpu().numpy()
+        arg = res.argmax.cpu().numpy().T.copy()
+        cands = res.candidates()
+        nfound = res.n_found()
+    sub = cube[:, :, torch.as_tensor(pix, device=cube.device)].cpu().numpy()
+    del cube
+    torch.cuda.empty_cache()
+    st = PU.check(sub, d_orc, wl.width_list, snr[pix], arg[pix], wl.threshold, label=f"{name} full",
+                  nthreads=os.cpu_count() or 8, max_adjudicated_frac=0.05)
+    _report(f"{name} full size, {len(pix)} of {wl.npix} pixels ({len(pulses)} injected)", st)
+    cs = PU.check_candidates(st["oracle"], pix, cands, nfound, wl.threshold, 4096, all_pixels_checked=False)
+    for c in cands:
+        p = int(c["pixel"])
+        assert c["snr"] == snr[p] and (c["dm_idx"], c["width_idx"], c["t"]) == tuple(arg[p]) and c["snr"] > wl.threshold
     _check_recovery(wl, d, [pu for pu in pulses if pu.s0 >= 12], snr)
     # properties that hold at any size: finite map, indices in range, candidates = thresholded map
     assert np.all(np.isfinite(snr)) and arg[:, 0].min() >= 0 and arg[:, 0].max() < len(wl.dm_list)
     assert arg[:, 1].max() < len(wl.width_list) and arg[:, 2].min() >= 0 and arg[:, 2].max() < wl.nt
     assert cs["found"] == int((snr > wl.threshold).sum())
-    del cube
-    torch.cuda.empty_cache()
 
 
 def test_full_size_stream_c2_sampled():
-    """C2 at full size (256x256 px, 1536-sample ring): fill the ring, then compare steady-state pushes
-    on a pixel sample."""
+    """C2 at full size (256x256 px, 1536-sample ring): >= 256 pixels (every injected one, edges, random) on 11 pushes:
+    the first ones, mid fill, the four around the ring wrap (1536 / 25 = 61.44) and steady state."""
+    import os
     nsfrb = _nsfrb()
     wl = W.config("c2")
     d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
-    n_push = 66
+    n_push = 70
     src = W.ChunkSource(wl, d, n_push, "cuda")
-    pix = _sample_pixels(wl, src.pulses, 60)
+    pix = _sample_pixels(wl, src.pulses, 256)
     tp = torch.as_tensor(pix, device="cuda")
     so = oracle.StreamOracle(wl.nchan, len(pix), wl.nt, d, wl.width_list)
+    tot = {"n": 0, "exact": 0, "adjudicated": 0, "undefined": 0, "worst_tol_frac": 0.0}
     with nsfrb.Plan.for_workload(wl) as plan:
         out = plan.alloc_outputs()
         for i in range(n_push):
@@ -397,16 +578,22 @@ def test_full_size_stream_c2_sampled():
             n_prev = so.n
             so.n += ch.shape[1]
             so.hist = np.concatenate([so.hist, ch], axis=1)[:, -so.L:, :]
-            if i in (0, 40, 61, 62, 65):
+            if i in (0, 1, 20, 40, 60, 61, 62, 63, 65, 68, 69):
                 torch.cuda.synchronize()
                 lo = max(0, so.n - so.L)
                 snr = out.snr_map.cpu().numpy()
                 arg = out.argmax.cpu().numpy().T.copy()
                 st = PU.check(so.hist, d, wl.width_list, snr[pix], arg[pix], wl.threshold, raw_end_min=n_prev - lo,
-                              t_offset=lo, label=f"c2 full push {i}")
+                              t_offset=lo, label=f"c2 full push {i}", nthreads=os.cpu_count() or 8,
+                              max_adjudicated_frac=0.05 if i >= 20 else 0.25)
+                for k in ("n", "exact", "adjudicated", "undefined"):
+                    tot[k] += st[k]
+                tot["worst_tol_frac"] = max(tot["worst_tol_frac"], st["worst_tol_frac"])
                 PU.check_candidates(st["oracle"], pix, out.candidates(), out.n_found(), wl.threshold, 4096,
                                     all_pixels_checked=False)
                 assert out.n_found() == int((snr > wl.threshold).sum())
+    _report(f"c2 full size, {len(pix)} pixels x 11 pushes", tot)
+    assert tot["adjudicated"] <= 0.05 * max(tot["n"] - tot["undefined"], 1)
 
 
 def test_stream_unsorted_duplicate_dms_and_flat_pixels():
