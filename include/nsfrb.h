@@ -181,6 +181,9 @@ int nsfrb_stream_reset(nsfrb_plan *plan);
  * Same calls with HOST buffers (pinned memory recommended): the library copies the input
  * host->device, runs the search, copies snr_map/argmax/cands/ncands device->host on
  * `stream` and synchronises it before returning.  Staging buffers belong to the plan.
+ * nsfrb_search_host never holds a device copy of the whole cube: it walks the image in pixel batches,
+ * copying batch i+1 (a strided block of cube_host: nchan*nt rows of `batch` pixels) on an internal copy stream while batch
+ * i is searched; with pinned memory the call is bound by the host link (23.75 GB of C3 at ~55 GB/s: 0.43 s).
  */
 int nsfrb_search_host(nsfrb_plan *plan, const float *cube_host, void *stream,
                       float *snr_map_host, int32_t *argmax_host,

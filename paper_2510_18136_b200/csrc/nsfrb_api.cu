@@ -199,7 +199,7 @@ int check_outputs(const void *snr_map, const void *argmax, const void *cands, ui
 
 int ensure_host_staging(nsfrb_plan *pl, size_t in_bytes, uint32_t cap)
 {
-    if (pl->d_in_bytes < in_bytes) {
+    if (in_bytes > 0 && pl->d_in_bytes < in_bytes) {
         cudaFree(pl->d_in); pl->d_in = nullptr; pl->d_in_bytes = 0;
         CU(cudaMalloc(reinterpret_cast<void **>(&pl->d_in), in_bytes), "staging input alloc");
         pl->d_in_bytes = in_bytes;
@@ -572,10 +572,22 @@ int nsfrb_search_host(nsfrb_plan *pl, const float *cube_host, void *stream, floa
     if (!pl) return fail(NSFRB_EINVAL, "plan is null");
     if (!cube_host) return fail(NSFRB_EINVAL, "cube is null");
     if (int rc = check_outputs(snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host)) return rc;
+    if (pl->n_received != 0) return fail(NSFRB_ESTATE, "plan holds streamed samples; call nsfrb_stream_reset first");
     ON_PLAN_DEVICE(pl);
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (search4_usable(pl)) {
+        // pixel batches straight from the host cube: no cube-sized staging buffer, copies overlap the search
+        if (int rc = ensure_host_staging(pl, 0, cand_capacity)) return rc;
+        int launches = 0;
+        std::string err;
+        if (int rc = search4_launch_host(pl, cube_host, st, pl->d_snr, pl->d_arg, &launches, err)) return fail(rc, err);
+        CU(cudaMemsetAsync(pl->d_ncands, 0, sizeof(uint32_t), st), "memset ncands");
+        CU(launch_compact(pl->d_snr, pl->d_arg, pl->npix, pl->threshold, pl->d_cands, cand_capacity, pl->d_ncands, st), "k_compact launch");
+        pl->last_launches = launches + 1;
+        return copy_back(pl, st, snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host);
+    }
     const size_t bytes = (size_t)pl->nchan * pl->nt * (size_t)pl->npix * sizeof(float);
     if (int rc = ensure_host_staging(pl, bytes, cand_capacity)) return rc;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
     CU(cudaMemcpyAsync(pl->d_in, cube_host, bytes, cudaMemcpyHostToDevice, st), "H2D cube");
     if (int rc = nsfrb_search(pl, pl->d_in, stream, pl->d_snr, pl->d_arg, pl->d_cands, cand_capacity, pl->d_ncands)) return rc;
     return copy_back(pl, st, snr_map_host, argmax_host, cands_host, cand_capacity, ncands_host);

@@ -158,6 +158,9 @@ int search4_prepare(nsfrb_plan *pl, std::string &err); // compile + workspaces; 
 // recorded after the first batch's layout kernel.
 int search4_launch(nsfrb_plan *pl, const float *cube, cudaStream_t st, float *snr_map, int32_t *argmax, int *launches,
                    cudaEvent_t ev_layout, std::string &err);
+// the same from a host cube: strided H2D copies of one batch at a time on a copy stream, overlapped with the search
+int search4_launch_host(nsfrb_plan *pl, const float *cube_host, cudaStream_t st, float *snr_map, int32_t *argmax, int *launches,
+                        std::string &err);
 void search4_free(nsfrb_plan *p);
 size_t search4_bytes(const nsfrb_plan *p);
 int search4_ring_len(const nsfrb_plan *pl);

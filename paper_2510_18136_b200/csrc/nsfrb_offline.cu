@@ -68,6 +68,10 @@ struct Search4State {
     float *scratch = nullptr;   // [grid][16][dpitch] dedispersed series of the items in flight (L2-resident)
     int grid = 0, dpitch = 0, nwarp = 16; // persistent CTAs (16 / nwarp per SM)
     int32_t *counter = nullptr; // [npix] tickets of the per-pixel reduction
+    // host-cube variant (nsfrb_search_host): two device slabs [nchan][nt][batch] filled by strided copies on a copy stream
+    float *slab[2] = {nullptr, nullptr};
+    cudaStream_t s_copy = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_copied[2] = {nullptr, nullptr}, ev_free[2] = {nullptr, nullptr};
     size_t bytes = 0;
 };
 
@@ -200,6 +204,14 @@ void search4_free(nsfrb_plan *p)
     cudaFree(p->search4->scratch);
     cudaFree(p->search4->W[0]);
     cudaFree(p->search4->W[1]);
+    cudaFree(p->search4->slab[0]);
+    cudaFree(p->search4->slab[1]);
+    if (p->search4->s_copy) cudaStreamDestroy(p->search4->s_copy);
+    if (p->search4->ev_fork) cudaEventDestroy(p->search4->ev_fork);
+    for (int b = 0; b < 2; ++b) {
+        if (p->search4->ev_copied[b]) cudaEventDestroy(p->search4->ev_copied[b]);
+        if (p->search4->ev_free[b]) cudaEventDestroy(p->search4->ev_free[b]);
+    }
     cudaGetLastError();
     delete p->search4;
     p->search4 = nullptr;
@@ -283,6 +295,57 @@ int search4_launch(nsfrb_plan *pl, const float *cube, cudaStream_t st, float *sn
         void *args[] = {&sp};
         const long long items = (long long)((sp.npb + s4->pxi - 1) / s4->pxi) * s4->ngroups;
         if (items <= 0 || items > 0x7fffffffLL) { err = "too many work items for one launch"; return NSFRB_EINVAL; }
+        OCU(cudaLaunchKernel((const void *)s4->fn, dim3((unsigned)std::min<long long>(items, s4->grid)), dim3(32 * s4->nwarp), args, s4->smem, st),
+            "k_search4 launch");
+        ++*launches;
+    }
+    return NSFRB_OK;
+}
+
+// The same pipeline fed from a HOST cube (pinned memory for real overlap): batch i+1 travels host -> device slab on the copy
+// stream (one strided copy: nchan*nt rows of `batch` pixels) while batch i is searched; the layout kernel reads the slab.
+// No cube-sized device buffer: two slabs of one batch each.  Outputs are device buffers; the caller copies them back.
+int search4_launch_host(nsfrb_plan *pl, const float *cube_host, cudaStream_t st, float *snr_map, int32_t *argmax, int *launches,
+                        std::string &err)
+{
+    if (int rc = search4_prepare(pl, err)) return rc;
+    Search4State *s4 = pl->search4;
+    const int nb = s4->batch;
+    auto count = [&](int i) { return std::min(nb, pl->npix - i * nb); };
+    const size_t rows = (size_t)pl->nchan * pl->nt;
+    if (!s4->s_copy) {
+        OCU(cudaStreamCreateWithFlags(&s4->s_copy, cudaStreamNonBlocking), "copy stream");
+        OCU(cudaEventCreateWithFlags(&s4->ev_fork, cudaEventDisableTiming), "event");
+        for (int b = 0; b < 2; ++b) {
+            OCU(cudaEventCreateWithFlags(&s4->ev_copied[b], cudaEventDisableTiming), "event");
+            OCU(cudaEventCreateWithFlags(&s4->ev_free[b], cudaEventDisableTiming), "event");
+        }
+    }
+    for (int b = 0; b < (s4->nbatch > 1 ? 2 : 1); ++b)
+        if (!s4->slab[b]) {
+            const size_t sb = rows * (size_t)nb * sizeof(float);
+            OCU(cudaMalloc(reinterpret_cast<void **>(&s4->slab[b]), sb), "slab alloc");
+            s4->bytes += sb;
+        }
+    OCU(cudaEventRecord(s4->ev_fork, st), "event record"); // the copies start where the caller's stream stands
+    OCU(cudaStreamWaitEvent(s4->s_copy, s4->ev_fork, 0), "stream wait");
+    for (int i = 0; i < s4->nbatch; ++i) {
+        const int b = i & 1, n = count(i);
+        if (i >= 2) OCU(cudaStreamWaitEvent(s4->s_copy, s4->ev_free[b], 0), "stream wait"); // the layout kernel of batch i-2 has read the slab
+        OCU(cudaMemcpy2DAsync(s4->slab[b], (size_t)n * sizeof(float), cube_host + (size_t)i * nb, (size_t)pl->npix * sizeof(float),
+                              (size_t)n * sizeof(float), rows, cudaMemcpyHostToDevice, s4->s_copy),
+            "H2D batch");
+        OCU(cudaEventRecord(s4->ev_copied[b], s4->s_copy), "event record");
+        OCU(cudaStreamWaitEvent(st, s4->ev_copied[b], 0), "stream wait");
+        // (W[b] was last read by the search of batch i-2: stream order on st)
+        OCU(launch_transpose(s4->slab[b], s4->W[b], n, pl->nchan, pl->nt, pl->pitch, 0, n, st), "k_transpose launch");
+        OCU(cudaEventRecord(s4->ev_free[b], st), "event record");
+        ++*launches;
+        Search4Params sp;
+        sp.W = s4->W[b]; sp.partials = pl->d_partials; sp.npix = pl->npix; sp.p0 = i * nb; sp.npb = n;
+        sp.counter = s4->counter; sp.snr_map = snr_map; sp.argmax = argmax; sp.scratch = s4->scratch;
+        void *args[] = {&sp};
+        const long long items = (long long)((sp.npb + s4->pxi - 1) / s4->pxi) * s4->ngroups;
         OCU(cudaLaunchKernel((const void *)s4->fn, dim3((unsigned)std::min<long long>(items, s4->grid)), dim3(32 * s4->nwarp), args, s4->smem, st),
             "k_search4 launch");
         ++*launches;

@@ -130,6 +130,25 @@ def test_offline_pixel_batches(monkeypatch, name, nx, ny, nt, batch, side):
     assert np.array_equal(snr, snr1) and np.array_equal(arg, arg1)
 
 
+def test_search_host_stages_pixel_batches_from_the_host_cube(monkeypatch):
+    """nsfrb_search_host on a plan that needs several pixel batches: strided host -> device copies of one batch at a time
+    on a copy stream, overlapped with the search; the result must equal nsfrb_search on the device cube bit for bit."""
+    nsfrb = _nsfrb()
+    monkeypatch.setenv("NSFRB_SEARCH_BATCH_PIX", "16")
+    wl = W.config("c3").scaled(9, 7, 900, n_pulses=3)            # 63 pixels: three full batches and a ragged one
+    d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
+    cube = W.make_cube(wl, "cuda")
+    _inject_all(wl, cube, d)
+    host = cube.cpu().pin_memory()
+    with nsfrb.Plan.for_workload(wl) as plan:
+        for _ in range(2):                                       # twice: the slabs and events are reused
+            h = plan.search_host(host)
+            dres = plan.search(cube)
+            torch.cuda.synchronize()
+            assert torch.equal(h[0], dres.snr_map.cpu()) and torch.equal(h[1], dres.argmax.cpu())
+            assert int(h[3].numpy().view(np.uint32)[0]) == dres.n_found()
+
+
 def _check_recovery(wl, d, pulses, snr, frac=0.7):
     """Injected single pulses come back at >= frac of the closed form S0 q / sqrt(1 + S0^2 q / T_k)
     (SURVEY 8(c) 'Injected pulse in noise'; the max over cells can only be higher)."""
