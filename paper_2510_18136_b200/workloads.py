@@ -321,3 +321,49 @@ def synthetic_snr_map(nx: int, ny: int, psf: np.ndarray, seed: int = 0, *, peak:
     for _ in range(n_spurious):
         m[int(rng.integers(ny)), int(rng.integers(nx))] = np.float32(rng.uniform(7.0, 12.0))
     return m, (x0, y0)
+
+
+# ----------------------------------------------------------------------------- NEXT 4: synthetic visibilities (imaging)
+IMG_N = 175                                   # 175 x 175-pixel UV grid / image
+IMG_PIXEL_RAD = 10.3 / 206264.80624709636     # L55: 10.3 arcsec pixels
+IMG_NANT, IMG_NCORE = 97, 82                  # Fig. 1 (L65): 97 antennas -> 4656 baselines (L48); L55: 82-antenna core
+
+
+def imaging_array(seed: int = 0) -> np.ndarray:
+    """Seeded stand-in for the DSA-110 layout (the real antenna positions are not in the paper): 82 core antennas on a
+    mostly east-west line about 400 m long with a short north-south arm and metre-scale jitter (all core baselines < 485 m),
+    plus 15 outriggers 0.6-2.5 km away (their baselines are cut by b_max).  Returns uv_m [4656][2] float64 = (east, north)
+    separations in metres of every antenna pair i < j (W-term neglected, L55)."""
+    rng = np.random.default_rng(9000 + seed)
+    ew = np.stack([np.linspace(-200.0, 200.0, 62) + rng.uniform(-2.0, 2.0, 62), rng.uniform(-3.0, 3.0, 62)], axis=1)
+    ns = np.stack([rng.uniform(-3.0, 3.0, 20) + 40.0, np.linspace(15.0, 230.0, 20) + rng.uniform(-2.0, 2.0, 20)], axis=1)
+    ang = rng.uniform(0.0, 2.0 * np.pi, IMG_NANT - IMG_NCORE)
+    rad = rng.uniform(600.0, 2500.0, IMG_NANT - IMG_NCORE)
+    out = np.stack([rad * np.cos(ang), rad * np.sin(ang)], axis=1)
+    pos = np.concatenate([ew, ns, out], axis=0)
+    i, j = np.triu_indices(IMG_NANT, k=1)
+    return (pos[j] - pos[i]).astype(np.float64)
+
+
+def imaging_freqs(subband: int = 8, nchan: int = 8) -> np.ndarray:
+    """Centres of the 8 x 1.46 MHz channels of one 11.7 MHz sub-band of the 187.5 MHz band centred on 1.4 GHz (L48)."""
+    lo = 1.4 - 0.09375 + subband * 0.01171875
+    return lo + (np.arange(nchan) + 0.5) * (0.01171875 / nchan)
+
+
+def imaging_visibilities(uv_m: np.ndarray, freqs_GHz, nt: int, sources, noise: float = 0.0, seed: int = 0) -> np.ndarray:
+    """vis [nt][nchan][nbase][2 pol] complex64: point sources (l_rad, m_rad, flux[, t_on, t_off]) with half the flux in each
+    polarisation, V = S exp(-2 pi i (u l + v m)) with u, v in wavelengths, plus complex Gaussian noise of rms `noise` per
+    polarisation.  (The paper images fringe-stopped, calibrated visibilities, L48-L55; these stand in for them.)"""
+    rng = np.random.default_rng(9100 + seed)
+    f = np.asarray(freqs_GHz, dtype=np.float64)
+    uvl = uv_m[None, :, :] * (f[:, None, None] * 1.0e9 / 299792458.0)          # [nchan][nbase][2] wavelengths
+    vis = np.zeros((nt, len(f), uv_m.shape[0], 2), dtype=np.complex128)
+    for src in sources:
+        l, m, flux = src[0], src[1], src[2]
+        t_on, t_off = (src[3], src[4]) if len(src) >= 5 else (0, nt)
+        ph = np.exp(-2j * np.pi * (uvl[:, :, 0] * l + uvl[:, :, 1] * m)) * (0.5 * flux)
+        vis[t_on:t_off] += ph[None, :, :, None]
+    if noise > 0.0:
+        vis += noise * (rng.standard_normal(vis.shape) + 1j * rng.standard_normal(vis.shape)) / np.sqrt(2.0)
+    return vis.astype(np.complex64)
