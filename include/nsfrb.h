@@ -330,6 +330,37 @@ int nsfrb_jit_search_kernel(int nx, int ny, int nchan, int nt, const double *fre
                             int want_cubin, char *out, size_t capacity, size_t *needed);
 
 /*
+ * Upstream imaging (PAPER.md:L55, L61 fn. 10, L67; readings I1-I6 in DESIGN.md): fringe-stopped
+ * visibilities of one sub-band -> one n x n image per time sample, ready to be a channel plane of a search chunk.
+ *   "grids visibilities with baseline lengths b > b_min = 20 m from the dense 82-antenna 'core' (b < b_max = 485 m) to a
+ *    175 x 175-pixel UV-grid ... The two visibility polarizations are summed, then approximately uniform weighting (Briggs
+ *    robustness parameter R = -2) is applied to accumulate visibilities, and a 2-dimensional inverse-FFT is applied" (L55);
+ *   "ifftshift ... np.fft.ifft2 ... ifftshift" (L61); "Each of the 8 channels are imaged individually, then summed" (L67).
+ * Definition.  For channel c and baseline b with bmin < |uv_m[b]| < bmax:  (fu, fv) = floor(uv_m[b] * f_c / c_light * n *
+ * pixel_rad + 0.5) (nearest UV cell, offsets from grid index n/2; baselines whose cell or its mirror image falls off the grid
+ * are dropped); natural weight 1; W_k = number of visibilities in cell k counting every visibility at (fu, fv) and (-fu, -fv);
+ * Briggs weight w = 1 / (1 + W_k f^2), f^2 = (5 * 10^-robust)^2 / (sum_k W_k^2 / sum_i 1).  The channel's grid holds
+ * w (V0 + V1) at (fu, fv) and its conjugate at (-fu, -fv); channel image = Re(ifftshift(ifft2(ifftshift(grid)))) * n^2 /
+ * (2 sum w) (a unit point source at the phase centre has value 1 at pixel (x0, x0), x0 = n - n/2: the pixel the final
+ * ifftshift moves index 0 to); out = the sum of the channel images.  x runs with u (l), y with v (m); out[t][y][x].
+ *
+ * nsfrb_imager_create: all of the above that does not depend on the data, in float64 on the host; small tables go to the
+ *   current device.  uv_m host [nbase][2] metres (east, north); freqs_GHz host [nchan].  2 <= n <= 2048.
+ * nsfrb_imager_image:  vis device, [nt][nchan][nbase][2 pol] complex64 as (re, im) float32 pairs (the paper's 14.9 MB
+ *   buffer for nt = 25), 16-byte aligned, read only;  out device, [nt][n*n] float32, written.  One launch on `stream`,
+ *   asynchronous.  With out = chunk + subband * nt * n * n the result is one channel plane of an nsfrb_stream_push chunk.
+ * nsfrb_imager_get_table: cells host [nchan][nbase][2] int32 and weights host [nchan][nbase] float64 (0 = not gridded), for
+ *   bit-exact parity of the integer part.
+ * Errors: NSFRB_EINVAL (null, sizes, non-finite parameters, misaligned vis), NSFRB_ENOMEM, NSFRB_ECUDA.
+ */
+typedef struct nsfrb_imager nsfrb_imager;
+int nsfrb_imager_create(nsfrb_imager **out, int n, double pixel_rad, const double *uv_m, int nbase,
+                        const double *freqs_GHz, int nchan, double bmin_m, double bmax_m, double robust);
+int nsfrb_imager_image(nsfrb_imager *imager, const float *vis, int nt, float *out, void *stream);
+int nsfrb_imager_get_table(const nsfrb_imager *imager, int32_t *cells, double *weights);
+int nsfrb_imager_destroy(nsfrb_imager *imager);
+
+/*
  * Measured on-chip ceilings of the current device, for the offline roofline ("the builder writes two
  * microbenchmarks (FADD/FMNMX chain; conflict-free LDS stream) and uses the achieved numbers").  Runs one short
  * kernel per instruction mix on every SM (about 0.1 s in all with iters = 2000); synchronises `stream`.

@@ -1,7 +1,7 @@
 """Oracle for the upstream imaging step -- TEST INFRASTRUCTURE, not product code.
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline leg may import this module; it shares nothing with
-paper_2510_18136_b200/csrc (no tables, no helpers).  Plain numpy, float64 / complex128, written in the order of the paper:
+the CUDA path (no tables, no helpers, no imports either way).  Plain numpy, float64 / complex128, written in the order of the paper:
 
   PAPER.md:L55  "grids visibilities with baseline lengths b > b_min = 20 m from the dense 82-antenna 'core'
                  (b < b_max = 485 m) to a 175 x 175-pixel UV-grid.  The core is assumed to be coplanar, so the W-term is

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnsfrb.so")
-SOURCES = ["nsfrb_api.cu", "nsfrb_kernels.cu", "nsfrb_search.cu", "nsfrb_stream.cu", "nsfrb_offline.cu", "nsfrb_cluster.cu", "nsfrb_median.cu", "nsfrb_peaks.cu"]
+SOURCES = ["nsfrb_api.cu", "nsfrb_kernels.cu", "nsfrb_search.cu", "nsfrb_stream.cu", "nsfrb_offline.cu", "nsfrb_cluster.cu", "nsfrb_median.cu", "nsfrb_peaks.cu", "nsfrb_imaging.cu"]
 JIT_SRCS = [os.path.join(CSRC, "nsfrb_stream_kernel.cuh"),   # compiled at plan time (NVRTC); embedded as text
             os.path.join(CSRC, "nsfrb_search_kernel.cuh")]
 HEADERS = JIT_SRCS + [os.path.join(CSRC, "nsfrb_internal.h"), os.path.join(os.path.dirname(HERE), "include", "nsfrb.h")]

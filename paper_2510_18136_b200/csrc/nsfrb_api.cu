@@ -41,6 +41,8 @@ constexpr size_t kMaxSmem = 227 * 1024; // opt-in dynamic shared memory per CTA 
 
 } // namespace
 
+int nsfrb::api_fail(int code, const std::string &msg) { return fail(code, msg); }
+
 void nsfrb::free_plan(nsfrb_plan *p)
 {
     if (!p) return;

@@ -144,6 +144,8 @@ struct nsfrb_plan {
 
 namespace nsfrb {
 
+// sets the thread-local error text of nsfrb_last_error and returns `code` (for entry points outside nsfrb_api.cu)
+int api_fail(int code, const std::string &msg);
 int plan_host_init(nsfrb_plan **out, int nx, int ny, int nchan, int nt, const double *freqs_GHz, double tsamp_s,
                    const double *dm_list, int ndm, const int32_t *width_list, int nwidth, float threshold);
 void free_plan(nsfrb_plan *p);

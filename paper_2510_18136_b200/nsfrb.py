@@ -47,7 +47,8 @@ EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stre
            "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes",
            "nsfrb_psf_mask", "nsfrb_cluster", "nsfrb_median_subtract",
            "nsfrb_stream_push_host_async", "nsfrb_stream_wait", "nsfrb_stream_set_running_sigma",
-           "nsfrb_peaks_count", "nsfrb_peaks_name", "nsfrb_measure_peaks", "nsfrb_plan_prepare", "nsfrb_cluster_static")
+           "nsfrb_peaks_count", "nsfrb_peaks_name", "nsfrb_measure_peaks", "nsfrb_plan_prepare", "nsfrb_cluster_static",
+           "nsfrb_imager_create", "nsfrb_imager_image", "nsfrb_imager_get_table", "nsfrb_imager_destroy")
 
 _lib = None
 
@@ -114,6 +115,15 @@ def lib() -> ctypes.CDLL:
         L.nsfrb_cluster_static.restype = ctypes.c_int
         L.nsfrb_cluster_static.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_float, vp, vp, vp, vp, ctypes.c_int, ctypes.c_int,
                                            ctypes.c_int, vp, vp, vp, vp, vp]
+        L.nsfrb_imager_create.restype = ctypes.c_int
+        L.nsfrb_imager_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, ctypes.c_double, f64p, ctypes.c_int, f64p, ctypes.c_int,
+                                          ctypes.c_double, ctypes.c_double, ctypes.c_double]
+        L.nsfrb_imager_image.restype = ctypes.c_int
+        L.nsfrb_imager_image.argtypes = [vp, vp, ctypes.c_int, vp, vp]
+        L.nsfrb_imager_get_table.restype = ctypes.c_int
+        L.nsfrb_imager_get_table.argtypes = [vp, i32p, f64p]
+        L.nsfrb_imager_destroy.restype = ctypes.c_int
+        L.nsfrb_imager_destroy.argtypes = [vp]
         L.nsfrb_plan_prepare.restype = ctypes.c_int
         L.nsfrb_plan_prepare.argtypes = [vp, ctypes.c_int, ctypes.c_int]
         L.nsfrb_peaks_count.restype = ctypes.c_int
@@ -273,6 +283,49 @@ def cluster_static(snr_map: torch.Tensor, argmax: torch.Tensor, nx: int, ny: int
                                       res.top.data_ptr(), res.wsnr.data_ptr(), res.members.data_ptr(), res.result.data_ptr(),
                                       int(s.cuda_stream)))
     return res
+
+
+class Imager:
+    """nsfrb_imager_create / nsfrb_imager_image / nsfrb_imager_destroy (NEXT 4: visibilities -> images)."""
+
+    def __init__(self, n, pixel_rad, uv_m, freqs_GHz, bmin_m=20.0, bmax_m=485.0, robust=-2.0):
+        uv = np.ascontiguousarray(uv_m, dtype=np.float64)
+        f = np.ascontiguousarray(freqs_GHz, dtype=np.float64)
+        self.n, self.nbase, self.nchan = int(n), uv.shape[0], f.size
+        self._h = ctypes.c_void_p()
+        f64p = ctypes.POINTER(ctypes.c_double)
+        _check(lib().nsfrb_imager_create(ctypes.byref(self._h), self.n, float(pixel_rad), uv.ctypes.data_as(f64p), self.nbase,
+                                         f.ctypes.data_as(f64p), self.nchan, float(bmin_m), float(bmax_m), float(robust)))
+
+    def table(self):
+        cells = np.zeros((self.nchan, self.nbase, 2), dtype=np.int32)
+        w = np.zeros((self.nchan, self.nbase), dtype=np.float64)
+        _check(lib().nsfrb_imager_get_table(self._h, cells.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+                                            w.ctypes.data_as(ctypes.POINTER(ctypes.c_double))))
+        return cells, w
+
+    def image(self, vis: torch.Tensor, out: torch.Tensor | None = None, stream=None) -> torch.Tensor:
+        """vis: CUDA complex64 [nt][nchan][nbase][2] -> float32 [nt][n*n] (asynchronous)."""
+        if not (vis.is_cuda and vis.dtype == torch.complex64 and vis.is_contiguous() and vis.dim() == 4
+                and tuple(vis.shape[1:]) == (self.nchan, self.nbase, 2)):
+            raise ValueError("vis must be a contiguous complex64 CUDA tensor [nt][nchan][nbase][2]")
+        nt = vis.shape[0]
+        if out is None:
+            out = torch.empty((nt, self.n * self.n), dtype=torch.float32, device=vis.device)
+        s = torch.cuda.current_stream() if stream is None else stream
+        _check(lib().nsfrb_imager_image(self._h, vis.data_ptr(), nt, out.data_ptr(), int(s.cuda_stream)))
+        return out
+
+    def close(self):
+        if self._h:
+            lib().nsfrb_imager_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
 
 
 class Plan:
