@@ -678,6 +678,55 @@ def run_cluster_arm(args):
                                    "note": "latency-bound: one launch, three dependent phases"}}))
 
 
+def run_image_arm(args):
+    """--op image: NEXT 4, the paper's imaging block (25 samples x 8 channels x 4656 baselines x 2 pols = 14.9 MB -> 25 images
+    of 175 x 175) for 16 sub-bands back to back = one 3.35 s chunk of the array.  ALU-bound by its own count: 4 FMA per
+    (gridded visibility, image column) in the row transform + 2 per (row, pixel) in the column transform."""
+    from paper_2510_18136_b200 import nsfrb
+    torch.cuda.set_device(0)
+    hbm_peak, peak_src, _ = measured_peaks()
+    onchip = measure_onchip_peaks(nsfrb)
+    uv = W.imaging_array(0)
+    n, nt, nsub = W.IMG_N, 25, 16
+    imagers = [nsfrb.Imager(n, W.IMG_PIXEL_RAD, uv, W.imaging_freqs(sb)) for sb in range(nsub)]
+    g = torch.Generator(device="cuda").manual_seed(7)
+    vis = [torch.view_as_complex(torch.randn((nt, 8, len(uv), 2, 2), device="cuda", generator=g)) for _ in range(nsub)]
+    chunk = torch.empty((nsub, nt, n * n), device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def step():
+        for sb in range(nsub):
+            imagers[sb].image(vis[sb], out=chunk[sb])
+
+    per_step = time_steps(step, args.steps, args.warmup, lambda: flush.zero_())
+    ms = float(np.mean(per_step))
+    nent = sum(int((im.table()[1] > 0).sum()) for im in imagers)
+    ops = (nent * n * 4 + nsub * (n // 2 + 1) * n * n * 2) * nt          # FMA lane-ops per chunk
+    peak = onchip["ffma"]["per_s"] / 1e12
+    nbytes = sum(v.numel() * 8 for v in vis) + chunk.numel() * 4
+    # the oracle on one time sample of one sub-band, scaled
+    from oracle import imaging as OI
+    v1 = vis[0][:1].cpu().numpy()
+    t0 = time.perf_counter()
+    OI.image(v1, uv, W.imaging_freqs(0))
+    cpu_s = time.perf_counter() - t0
+    for im in imagers:
+        im.close()
+    print(json.dumps({"metric": "images/s (NEXT 4: grid + inverse DFT, 175 x 175, 8 channels summed)", "value": nsub * nt / (ms * 1e-3),
+                      "unit": "images/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
+                      "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": "one 3.35 s chunk of the array: 16 sub-bands x 25 samples x 8 channels x 4656 baselines x 2 pols",
+                                 "l2": "flushed between steps", "chunk_latency_frac": ms / CHUNK_DURATION_MS},
+                      "gpu_launches": nsub * args.steps,
+                      "roofline": {"bound": "alu", "achieved": ops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "T lane-ops/s",
+                                   "frac": ops / (ms * 1e-3) / 1e12 / peak, "traffic": None,
+                                   "peak_source": "measured FFMA issue rate (nsfrb_measure_peaks, this run)", "kernel": "k_image",
+                                   "algorithmic_ops": ops, "algorithmic_bytes": nbytes,
+                                   "hbm_frac": nbytes / (ms * 1e-3) / 1e9 / hbm_peak},
+                      "cpu_baseline": {"value": 1.0 / cpu_s, "unit": "images/s", "cores": 1, "kind": "oracle",
+                                       "sample": "one time sample of one sub-band (numpy ifft2 route)"}}))
+
+
 def measure_onchip_peaks(nsfrb_mod, iters=2000):
     """The achieved on-chip ceilings of this GPU (nsfrb_measure_peaks: FADD/FMNMX/FMNMX3 issue, the search's
     2 FADD + 1 FMNMX3 cell pair, conflict-free shared-memory streams), with the SM clock derived from the two timings."""
@@ -718,7 +767,7 @@ def main():
     ap.add_argument("--no-extra", action="store_true", help="c2: do not also time c3, c4, c5 (the `workloads` object)")
     ap.add_argument("--cubes", action="store_true", help="c2: also write the S/N and TOA cubes every push (NEXT 3)")
     ap.add_argument("--running", action="store_true", help="c2: also the running-sigma maps every push (NEXT 1)")
-    ap.add_argument("--op", default="search", choices=["search", "bin", "cluster", "median", "peaks"],
+    ap.add_argument("--op", default="search", choices=["search", "bin", "cluster", "median", "peaks", "image"],
                     help="bin: time the binning kernel (NEXT 2); cluster: top-10 + PSF clustering (NEXT 3); "
                          "median: per-pixel median subtraction (NEXT 1)")
     ap.add_argument("--bin-factor", type=int, default=5)
@@ -731,6 +780,9 @@ def main():
     elif args.op == "median" and args.impl == "cuda":
         if rank == 0:
             run_median_arm(args)
+    elif args.op == "image" and args.impl == "cuda":
+        if rank == 0:
+            run_image_arm(args)
     elif args.op == "peaks" and args.impl == "cuda":
         if rank == 0:
             run_peaks_arm(args)

@@ -9,7 +9,8 @@
 // inverse DFT over the SPARSE visibility list, all channels at once, in the half plane fv >= 0:
 //   phase 1  R[r][x] = sum over the entries of row r = |fv| of  a_i Vc_i tw[fu_i (x - x0) mod n]     (Vc = V for fv >= 0, conj V and
 //            -fu for fv < 0; V = the two polarisations summed; a_i = Briggs weight / sum of the channel's weights)
-//            warps take rows, lanes take columns, the visibility is a broadcast load, the twiddle a shared-memory table
+//            warps take rows, lanes take columns; 32 visibilities at a time are loaded coalesced and broadcast by shuffles;
+//            the twiddle is a shared-memory table
 //   phase 2  I[y][x] = 2 sum_r Re(R[r][x] tw[r (y - x0) mod n])                                    (the other half plane is the conjugate)
 // with x0 = n - n / 2 the pixel the paper's final ifftshift puts the phase centre on.  Same result as the oracle's route up
 // to float32 rounding; shares no code with oracle/imaging.py.
@@ -30,23 +31,24 @@ struct nsfrb_imager {
     // device
     int2 *d_entry = nullptr;      // [nentries] (visibility index | conj << 31, fu), sorted by row
     float *d_coeff = nullptr;     // [nentries]
-    int *d_row = nullptr;         // [n/2 + 2] CSR offsets by row |fv|
+    int *d_row = nullptr;         // [nunit][3] work units (row |fv|, first entry, one past the last): <= 256 entries of one row each
+    int nunit = 0;
     float2 *d_tw = nullptr;       // [n] exp(2 pi i k / n)
 };
 
 namespace nsfrb {
 namespace {
 
-constexpr int kImgThreads = 256;
+constexpr int kImgThreads = 512;
 
 struct ImageParams {
     const float4 *vis;  // [nt][nchan*nbase] (re0, im0, re1, im1)
     const int2 *entry;
     const float *coeff;
-    const int *row;
+    const int *unit;    // [nunit][3]
     const float2 *tw;
     float *out;         // [nt][n][n]
-    int n, nvis, nrow;  // nvis = nchan*nbase; nrow = n/2 + 1
+    int n, nvis, nrow, nunit;  // nvis = nchan*nbase; nrow = n/2 + 1
 };
 
 __global__ void __launch_bounds__(kImgThreads) k_image(const ImageParams P)
@@ -57,28 +59,52 @@ __global__ void __launch_bounds__(kImgThreads) k_image(const ImageParams P)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = kImgThreads / 32;
     const int t = blockIdx.y, x = blockIdx.x * 32 + lane;
     const int n = P.n, x0 = n - n / 2;
+    __shared__ int next_unit;
+    if (threadIdx.x == 0) next_unit = 0;
     for (int i = threadIdx.x; i < n; i += kImgThreads) tw[i] = P.tw[i];
+    for (int i = threadIdx.x; i < P.nrow * 32; i += kImgThreads) R[i] = make_float2(0.f, 0.f);
     __syncthreads();
-    const float rn = 1.0f / (float)n;
     const int dx = x - x0;
     const float4 *vt = P.vis + (size_t)t * P.nvis;
-    // ---- phase 1: rows of the half plane
-    for (int r = warp; r < P.nrow; r += nwarp) {
+    // ---- phase 1: rows of the half plane, in work units of <= 256 entries of one row (an east-west array puts most of its
+    // visibilities into the rows next to fv = 0: a row per warp would leave one warp with half the work).  Warps take units
+    // from a shared counter; per 32 entries every lane loads one (coalesced, independent loads) and forms its weighted,
+    // polarisation-summed, possibly conjugated visibility; the 32 are then broadcast one by one; a unit's partial sums are
+    // added to the row with shared-memory atomics (the order of those additions is the only run-to-run freedom: ~1e-7).
+    const unsigned M = 0xffffffffu / (unsigned)n + 1u; // ceil(2^32 / n): umulhi(p, M) = floor(p / n), or that + 1 for large p
+    const int bias = n * (n + 1);                       // > |fu dx|: makes the product non-negative, and is 0 mod n
+    for (;;) {
+        int ui = 0;
+        if (lane == 0) ui = atomicAdd(&next_unit, 1);
+        ui = __shfl_sync(0xffffffffu, ui, 0);
+        if (ui >= P.nunit) break;
         float re = 0.f, im = 0.f;
-        const int e0 = P.row[r], e1 = P.row[r + 1];
-        for (int e = e0; e < e1; ++e) {
-            const int2 en = __ldg(P.entry + e);
-            const float a = __ldg(P.coeff + e);
-            const float4 v = __ldg(vt + (en.x & 0x7fffffff));
-            const float vr = a * (v.x + v.z), vi = (en.x < 0 ? -a : a) * (v.y + v.w); // pols summed; conjugate for fv < 0
-            const int p = en.y * dx;                                                   // |p| < 2^24: exact in float
-            int k = p - n * (int)floorf((float)p * rn);
-            k = k < 0 ? k + n : (k >= n ? k - n : k);
-            const float2 w = tw[k];
-            re = fmaf(vr, w.x, fmaf(-vi, w.y, re));
-            im = fmaf(vr, w.y, fmaf(vi, w.x, im));
+        const int r = P.unit[3 * ui], e0 = P.unit[3 * ui + 1], e1 = P.unit[3 * ui + 2];
+        for (int eb = e0; eb < e1; eb += 32) {
+            const int e = eb + lane;
+            float vr = 0.f, vi = 0.f;
+            int fu = 0;
+            if (e < e1) {
+                const int2 en = __ldg(P.entry + e);
+                const float a = __ldg(P.coeff + e);
+                const float4 v = __ldg(vt + (en.x & 0x7fffffff));
+                vr = a * (v.x + v.z);                          // pols summed (L55)
+                vi = (en.x < 0 ? -a : a) * (v.y + v.w);        // conjugate for fv < 0
+                fu = en.y;
+            }
+            const int cnt = e1 - eb < 32 ? e1 - eb : 32;
+            for (int j = 0; j < cnt; ++j) {
+                const float br = __shfl_sync(0xffffffffu, vr, j), bi = __shfl_sync(0xffffffffu, vi, j);
+                const unsigned p = (unsigned)(__shfl_sync(0xffffffffu, fu, j) * dx + bias);
+                int k = (int)(p - (unsigned)n * __umulhi(p, M)); // the quotient may be one too large (never too small)
+                k = k < 0 ? k + n : k;
+                const float2 w = tw[k];
+                re = fmaf(br, w.x, fmaf(-bi, w.y, re));
+                im = fmaf(br, w.y, fmaf(bi, w.x, im));
+            }
         }
-        R[r * 32 + lane] = make_float2(re, im);
+        atomicAdd(&R[r * 32 + lane].x, re);
+        atomicAdd(&R[r * 32 + lane].y, im);
     }
     __syncthreads();
     // ---- phase 2: columns
@@ -168,16 +194,21 @@ int nsfrb_imager_create(nsfrb_imager **out, int n, double pixel_rad, const doubl
         }
     }
     std::stable_sort(entries.begin(), entries.end(), [](const Entry &a, const Entry &b) { return a.row < b.row; });
-    const int nrow = n / 2 + 1;
     std::vector<int2> h_entry(std::max<size_t>(entries.size(), 1));
     std::vector<float> h_coeff(std::max<size_t>(entries.size(), 1), 0.f);
-    std::vector<int> h_row(nrow + 1, 0);
+    std::vector<int> h_row; // work units (row, e0, e1), heaviest rows first in the list order of the sort (row 0 upwards)
     for (size_t i = 0; i < entries.size(); ++i) {
         h_entry[i] = make_int2(entries[i].idx | (entries[i].conj ? (int)0x80000000u : 0), entries[i].fu);
         h_coeff[i] = (float)entries[i].a;
-        if (entries[i].row < nrow) ++h_row[entries[i].row + 1];
     }
-    for (int r = 0; r < nrow; ++r) h_row[r + 1] += h_row[r];
+    for (size_t i = 0; i < entries.size();) {
+        size_t j = i;
+        while (j < entries.size() && entries[j].row == entries[i].row && j - i < 256) ++j;
+        h_row.push_back(entries[i].row); h_row.push_back((int)i); h_row.push_back((int)j);
+        i = j;
+    }
+    im->nunit = (int)(h_row.size() / 3);
+    if (h_row.empty()) h_row.assign(3, 0);
     std::vector<float2> h_tw(n);
     for (int k = 0; k < n; ++k) h_tw[k] = make_float2((float)std::cos(2.0 * M_PI * k / n), (float)std::sin(2.0 * M_PI * k / n));
     im->nentries = (int)entries.size();
@@ -208,8 +239,8 @@ int nsfrb_imager_image(nsfrb_imager *im, const float *vis, int nt, float *out, v
     if ((reinterpret_cast<uintptr_t>(vis) & 15u) != 0) return api_fail(NSFRB_EINVAL, "vis is not 16-byte aligned");
     if (nt < 1 || nt > 65535) return api_fail(NSFRB_EINVAL, "nt out of range (1..65535)");
     nsfrb::ImageParams P;
-    P.vis = reinterpret_cast<const float4 *>(vis); P.entry = im->d_entry; P.coeff = im->d_coeff; P.row = im->d_row; P.tw = im->d_tw;
-    P.out = out; P.n = im->n; P.nvis = im->nchan * im->nbase; P.nrow = im->n / 2 + 1;
+    P.vis = reinterpret_cast<const float4 *>(vis); P.entry = im->d_entry; P.coeff = im->d_coeff; P.unit = im->d_row; P.tw = im->d_tw;
+    P.out = out; P.n = im->n; P.nvis = im->nchan * im->nbase; P.nrow = im->n / 2 + 1; P.nunit = im->nunit;
     const size_t smem = ((size_t)im->n + (size_t)P.nrow * 32) * sizeof(float2);
     static size_t granted[64] = {0};
     int dev = 0;
