@@ -81,10 +81,11 @@ typedef struct {
  *   for nsfrb_stream_push.  freqs_GHz: host [nchan], finite, > 0, any order.  tsamp_s > 0.
  *   dm_list: host [ndm], finite, >= 0.  width_list: host [nwidth], each >= 1, distinct.
  *   Every trial must keep at least one sample: nt > max_c d[k][c] for all k.
- * All host arrays are copied.  Device memory is allocated on the current CUDA device when first needed: small
- * tables at creation; nchan*nt*npix*4 B (the time-contiguous copy of the cube) at the first nsfrb_search; the
- * ring, 2*(nt + guard)*nchan*npix*4 B, plus a workspace of ~10 B per (pixel, trial, width) at the first
- * nsfrb_stream_push.
+ * All host arrays are copied.  Device memory is allocated on the CUDA device current at creation: small tables at creation;
+ * at nsfrb_plan_prepare or the first nsfrb_search two pixel-batch workspaces of about 1 GiB each (the search walks the image
+ * in batches: no cube-sized buffer) plus ~2 MB of scratch per SM; at nsfrb_plan_prepare or the first nsfrb_stream_push the
+ * ring, 2*(nt + guard)*nchan*npix*4 B, plus a workspace of ~10 B per (pixel, trial, width).  Plans with more than 32 usable
+ * widths use a generic kernel with a cube-sized workspace (nchan*nt*npix*4 B).
  */
 int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt,
                       const double *freqs_GHz, double tsamp_s,
@@ -138,7 +139,13 @@ int nsfrb_search(nsfrb_plan *plan, const float *cube, void *stream,
  * The first push of a plan compiles the plan-specialised kernel with NVRTC (seconds to a minute, growing with
  * ndm*nchan) and allocates the ring (2*(nt + guard)*nchan*npix*4 B); a compile failure returns NSFRB_ECUDA with
  * the compiler log.  Compiled kernels are cached on disk (NSFRB_JIT_CACHE=<dir>, default /tmp/nsfrb_jit_cache_<uid>, private to the user;
- * NSFRB_JIT_CACHE=0 disables).  Chunks longer than the plan's first chunk are searched in several passes.
+ * NSFRB_JIT_CACHE=0 disables).  nsfrb_plan_prepare(plan, NSFRB_PREPARE_STREAM, chunk_nt) does both ahead of time.  A chunk longer
+ * than any before it recompiles the kernel for that length (a stream synchronisation; prepare with the longest chunk to avoid it).
+ * Stored samples are kept relative to a per-(channel, pixel) reference level, the median of the first chunk after a reset; the
+ * float32 path holds its 1e-4 tolerance while data stay within ~1e3 sigma of it (R32).
+ * Non-finite samples: results of the (pixel, trial) series that contain one are unspecified while it is in the ring; once it has
+ * left, the carried sums are rebuilt from the ring and the series is exact again (no nsfrb_stream_reset needed).  The same holds
+ * for a finite sample of enormous magnitude (R31).
  */
 int nsfrb_stream_push(nsfrb_plan *plan, const float *chunk, int chunk_nt, void *stream,
                       float *snr_map, int32_t *argmax,
