@@ -9,10 +9,10 @@
 //   W_TAB[NW]         the usable widths, caller's order (NW <= 32)    J_OF_W[NW]     original width index
 //
 // Persistent CTAs; a work item = PXI pixels x NWARP trials, in three phases with one CTA barrier between them:
-//   sweep A (thread = sample)  differential dedispersion along the DM axis straight from the time-contiguous batch workspace
-//            (coalesced, L1/L2-served loads with immediate offsets): the first trial is the plain channel sum, every next
-//            one adds (new - current) for the channels whose delay changed, the current value of every channel living in a
-//            register.  D goes to a per-CTA scratch (L2-resident).
+//   sweep A (thread = 4 consecutive samples)  differential dedispersion along the DM axis straight from the time-contiguous batch
+//            workspace: per channel one aligned window of vector loads (immediate offsets) covers every delay of the group; the
+//            first trial is the plain channel sum, every next one adds (new - previous trial's) for the channels whose delay
+//            changed.  D goes to a per-CTA scratch (L2-resident) as float4.
 //   sweep B (warp = trial, pixel after pixel; no barrier)  first one pass over the series for its exact mean and sigma
 //            (a1, a3), then blocks of 256 samples, 8 consecutive samples per lane: x = D - mu, prefix by 8 serial adds + one
 //            warp scan, P into the trial's ring (two interleaved planes of float4: every 128-bit access of a warp is
@@ -121,38 +121,60 @@ __device__ __forceinline__ bool better(float s, int k, int j, float bs, int bk, 
     return j < bj;
 }
 
-// ---- sweep A: differential dedispersion of sample t for the NWARP trials of group G.  wp = W[p] + t; dst = scratch + t.
+// ---- sweep A: differential dedispersion of SPT consecutive samples t .. t + SPT - 1 (t a multiple of SPT) for the NWARP trials
+// of group G.  wp = W[p] + t; dst = scratch + t.  Channel by channel the thread loads ONE aligned window that covers every
+// delay of the group (2-4 vector loads instead of one scalar load per (trial, changed channel)) and adds, for each trial,
+// window[new delay] - window[previous trial's delay] to that trial's difference; the first trial takes the plain sum.  The
+// dedispersed values are the running sum of the differences over the trials.
+constexpr int SPT = NWARP <= 16 ? 4 : 2; // samples per thread (the differences of all trials live in registers)
+
+template <int G, int C> struct ChanSpan { // delays of channel C over the trials of group G
+    static __host__ __device__ constexpr int lo() { int m = 1 << 30; for (int s = 0; s < NWARP; ++s) { const int u = G * NWARP + s; if (u < NU && D_TAB[u][C] < m) m = D_TAB[u][C]; } return m; }
+    static __host__ __device__ constexpr int hi() { int m = 0; for (int s = 0; s < NWARP; ++s) { const int u = G * NWARP + s; if (u < NU && D_TAB[u][C] > m) m = D_TAB[u][C]; } return m; }
+};
+
 template <int G> __device__ __forceinline__ void dedisperse(const float *__restrict__ wp, float *__restrict__ dst)
 {
-    float cur[NCHAN];
-    float acc = 0.f;
-    sfor<0, NWARP>([&](auto s) {
-        constexpr int u = G * NWARP + V(s);
-        if constexpr (u < NU) {
-            if constexpr (V(s) == 0) {
-                float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
-                sfor<0, NCHAN>([&](auto c) {
-                    const float v = __ldg(wp + V(c) * PITCH + D_TAB[u][V(c)]);
-                    cur[V(c)] = v;
-                    if constexpr ((V(c) & 3) == 0) a0 += v;
-                    else if constexpr ((V(c) & 3) == 1) a1 += v;
-                    else if constexpr ((V(c) & 3) == 2) a2 += v;
-                    else a3 += v;
-                });
-                acc = (a0 + a1) + (a2 + a3);
+    float diff[NWARP][SPT];
+#pragma unroll
+    for (int s = 0; s < NWARP; ++s)
+#pragma unroll
+        for (int i = 0; i < SPT; ++i) diff[s][i] = 0.f;
+    sfor<0, NCHAN>([&](auto c) {
+        constexpr int a = ChanSpan<G, V(c)>::lo() / SPT * SPT;                 // aligned start of the window
+        constexpr int nq = (ChanSpan<G, V(c)>::hi() + SPT - 1 - a) / SPT + 1;   // vectors that cover [lo, hi + SPT - 1]
+        float win[nq * SPT];
+        sfor<0, nq>([&](auto q) {
+            if constexpr (SPT == 4) {
+                const float4 v = __ldg(reinterpret_cast<const float4 *>(wp + V(c) * PITCH + a) + V(q));
+                win[4 * V(q)] = v.x; win[4 * V(q) + 1] = v.y; win[4 * V(q) + 2] = v.z; win[4 * V(q) + 3] = v.w;
             } else {
-                float a0 = 0.f, a1 = 0.f;
-                sfor<0, NCHAN>([&](auto c) {
-                    if constexpr (D_TAB[u][V(c)] != D_TAB[u - 1][V(c)]) {
-                        const float nv = __ldg(wp + V(c) * PITCH + D_TAB[u][V(c)]);
-                        const float v = nv - cur[V(c)];
-                        cur[V(c)] = nv;
-                        if constexpr ((V(c) & 1) == 0) a0 += v; else a1 += v;
-                    }
-                });
-                acc += a0 + a1;
+                const float2 v = __ldg(reinterpret_cast<const float2 *>(wp + V(c) * PITCH + a) + V(q));
+                win[2 * V(q)] = v.x; win[2 * V(q) + 1] = v.y;
             }
-            dst[V(s) * DPITCH] = acc;
+        });
+        sfor<0, NWARP>([&](auto s) {
+            constexpr int u = G * NWARP + V(s);
+            if constexpr (u < NU) {
+                if constexpr (V(s) == 0) {
+#pragma unroll
+                    for (int i = 0; i < SPT; ++i) diff[0][i] += win[D_TAB[u][V(c)] - a + i];
+                } else if constexpr (D_TAB[u][V(c)] != D_TAB[u - 1][V(c)]) {
+#pragma unroll
+                    for (int i = 0; i < SPT; ++i) diff[V(s)][i] += win[D_TAB[u][V(c)] - a + i] - win[D_TAB[u - 1][V(c)] - a + i];
+                }
+            }
+        });
+    });
+    float acc[SPT];
+#pragma unroll
+    for (int i = 0; i < SPT; ++i) acc[i] = 0.f;
+    sfor<0, NWARP>([&](auto s) {
+        if constexpr (G * NWARP + V(s) < NU) {
+#pragma unroll
+            for (int i = 0; i < SPT; ++i) acc[i] += diff[V(s)][i];
+            if constexpr (SPT == 4) *reinterpret_cast<float4 *>(dst + V(s) * DPITCH) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+            else *reinterpret_cast<float2 *>(dst + V(s) * DPITCH) = make_float2(acc[0], acc[1]);
         }
     });
 }
@@ -410,7 +432,7 @@ template <int G> __device__ __forceinline__ void sweep_a(const float *Wp, float 
 {
     constexpr int T_g = NT - DMAX_TAB[G * NWARP];      // longest series of the group (trials are sorted by dmax)
     constexpr int TA = (T_g + LB - 1) / LB * LB;       // sweep B reads whole blocks
-    for (int t = tid; t < TA; t += NTHR) dedisperse<G>(Wp + t, scr + t); // (reads past NT stay inside the padded workspace)
+    for (int t = SPT * tid; t < TA; t += SPT * NTHR) dedisperse<G>(Wp + t, scr + t); // (reads past NT stay inside the padded workspace)
 }
 
 template <int G0, int N> __device__ __forceinline__ void dispatch_a(int g, const float *Wp, float *scr, int tid)
