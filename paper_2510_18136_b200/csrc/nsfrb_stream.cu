@@ -47,6 +47,8 @@ struct StreamParams {
     int32_t t_offset;
     const float *dlt;  // INCR: exact mean minus its float rounding, and 1/sigma, per (unique trial, pixel)
     const float *rsig;
+    const float *dh;   // DHIST: dedispersed history [pixel block][rows][nuniq][32]
+    const float *dh8;  // COARSE: its 8-row block sums [pixel block][2 * L / 8][nuniq][32]
 };
 
 // host mirror of k_stream_stats's parameter block (nsfrb_stream_kernel.cuh)
@@ -56,6 +58,8 @@ struct StatsParams {
     float *mu, *dlt, *rsig, *sig_out;
     int32_t row_lo, add, first, pad;
     long long ring_lo, lo_prev, n_prev, lo, n;
+    float *dh;
+    float *dh8;
 };
 
 struct StreamCfg {
@@ -66,6 +70,8 @@ struct StreamCfg {
     float light_cost = 1.0f;                        // time of a light tile relative to a plain dedispersion tile (segment balance): it waits on memory; 1.0 measured best on C2 with SEG=2 (profiles/r01_v5.md)
     int LIGHT = 1;                                  // INCR only: plain runs are summed once for all trials of a thread (light tiles)
     int INCR = 1;                                   // 1: mean/sigma kept incrementally by k_stream_stats (the march stops at the last start range)
+    int COARSE = 1;                                 // DHIST only, ring length a multiple of 8: 8-row block sums of the history serve the plain runs
+    int DHIST = 1;                                  // INCR only: k_stream_stats also keeps every trial's dedispersed samples (a second ring); the march reads those
     size_t smem = 0;
     int threads() const { return 32 * GPC * SEG; }
 };
@@ -81,7 +87,8 @@ size_t cfg_smem(const StreamCfg &c)
 }
 
 // Tile shape for a plan: KK trials per thread, GPC groups x SEG segments of warps per CTA.
-bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamCfg &c, std::string &err)
+// dhist: 1/0 = with/without the dedispersed history, -1 = the default (NSFRB_STREAM_DHIST, else on)
+bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamCfg &c, std::string &err, int dhist = -1)
 {
     c = StreamCfg();
     c.NW = std::max(pl->nw_used, 1);
@@ -91,9 +98,20 @@ bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamC
         c.INCR = (e && std::strcmp(e, "march") == 0) ? 0 : 1;
         if (const char *lt = getenv("NSFRB_STREAM_LIGHT")) c.LIGHT = atoi(lt) != 0;
         if (!c.INCR) c.LIGHT = 0;
+        if (dhist < 0) {
+            const char *dh = getenv("NSFRB_STREAM_DHIST");
+            dhist = dh ? (atoi(dh) != 0) : 1;
+        }
+        c.DHIST = (c.INCR && dhist) ? 1 : 0;
+        const char *co = getenv("NSFRB_STREAM_COARSE");
+        c.COARSE = (c.DHIST && c.LIGHT && pl->nt % 8 == 0 && !(co && atoi(co) == 0)) ? 1 : 0;
         if (const char *lc = getenv("NSFRB_STREAM_LIGHT_COST")) c.light_cost = (float)atof(lc);
     }
-    if (pl->nchan > 24) { // the thread holds nchan*TT raw rows in registers: one time step per tile, more registers
+    if (c.DHIST) {
+        // a thread holds KK*TT history values and no raw rows: the trials of a thread share nothing, so fewer trials per
+        // thread and more warps per CTA (the shared-memory Qe block of a CTA is per trial either way)
+        kk = 8; gpc = 2; seg = 1; tt = 4; minb = 4; pfd = 2;
+    } else if (pl->nchan > 24) { // the thread holds nchan*TT raw rows in registers: one time step per tile, more registers
         tt = 1;
         minb = 2;
     } else if (c.LIGHT) {
@@ -135,7 +153,7 @@ bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamC
             carry = std::max(carry, s);
         }
         // fewer CTAs per SM while the estimate exceeds the registers a thread may have at that residency
-        const int est = pl->nchan * tt + carry + kk * (tt + 4) + 36;
+        const int est = c.DHIST ? 2 * kk * tt + 6 * kk + 40 : pl->nchan * tt + carry + kk * (tt + 4) + 36;
         const int threads = 32 * std::min(gpc, ngroups) * seg;
         while (minb > 1 && est > std::min(255, 65536 / (minb * threads)) - 5) --minb;
     }
@@ -171,6 +189,7 @@ std::string make_prologue(const nsfrb_plan *pl, const StreamCfg &c)
     auto def = [&](const char *n, long long v) { s += "#define " + std::string(n) + " " + std::to_string(v) + "\n"; };
     def("NPIX", pl->npix); def("NCHAN", pl->nchan); def("NU", pl->nuniq); def("KK", c.KK); def("GPC", c.GPC);
     def("SEG", c.SEG); def("TT", c.TT); def("NW", c.NW); def("CMAX", c.CMAX); def("NSUPER", c.NSUPER); def("MINB", c.MINB); def("PFD", c.PFD); def("INCR", c.INCR); def("LIGHT", c.LIGHT); def("NW_ALL", pl->nw); def("ROWS", 2 * (pl->dmax_all + 40) + 2 * pl->nt);
+    def("COARSE", c.COARSE); def("DHIST", c.DHIST); def("LRING", pl->nt); def("GUARD", pl->dmax_all + 40);
     s += "static __device__ constexpr short D_TAB[NU][NCHAN] = {";
     for (int u = 0; u < pl->nuniq; ++u) {
         s += u ? ",{" : "{";
@@ -298,6 +317,8 @@ struct StreamState {
     cudaKernel_t fn[2] = {nullptr, nullptr};
     cudaKernel_t fn_stats[2] = {nullptr, nullptr}; // k_stream_stats of the same module (INCR)
     float *ring = nullptr; // [pixel block][G + 2L + G][nchan][32]
+    float *dhist = nullptr; // [pixel block][G + 2L + G][nuniq][32]  dedispersed history (cfg.DHIST)
+    float *dh8 = nullptr;   // [pixel block][2L/8][nuniq][32]  its 8-row block sums (cfg.COARSE)
     float *base = nullptr; // [nchan][npix]  first sample ever, removed from every stored sample
     float *mu0 = nullptr;  // [nuniq][npix]
     // incremental statistics (k_stream_stats): float64 sums of D and D^2 over the valid samples of every (unique trial,
@@ -570,6 +591,26 @@ int stream_init(nsfrb_plan *pl, int chunk_nt, std::string &err)
     const size_t ring_b = (size_t)((pl->npix + 31) / 32) * (2 * ss->guard + 2 * pl->nt) * pl->nchan * 32 * sizeof(float);
     SCU(cudaMalloc(reinterpret_cast<void **>(&ss->ring), ring_b), "ring alloc");
     SCU(cudaMemset(ss->ring, 0, ring_b), "ring clear");
+    size_t dh_b = 0;
+    if (ss->cfg.DHIST) {
+        dh_b = ring_b / pl->nchan * pl->nuniq;
+        size_t fr = 0, tot = 0;
+        // the history is a second ring, nuniq / nchan times the first: where it does not fit comfortably the march dedisperses
+        if (cudaMemGetInfo(&fr, &tot) != cudaSuccess || dh_b > fr / 2) {
+            cudaGetLastError();
+            dh_b = 0;
+            if (!choose_cfg(pl, chunk_nt, getenv("NSFRB_STREAM_VARIANT"), ss->cfg, err, 0)) return NSFRB_ENOMEM;
+        } else {
+            SCU(cudaMalloc(reinterpret_cast<void **>(&ss->dhist), dh_b), "dedispersed-history alloc");
+            SCU(cudaMemset(ss->dhist, 0, dh_b), "dedispersed-history clear");
+            if (ss->cfg.COARSE) {
+                const size_t d8 = (size_t)((pl->npix + 31) / 32) * (2 * pl->nt / 8) * pl->nuniq * 32 * sizeof(float);
+                SCU(cudaMalloc(reinterpret_cast<void **>(&ss->dh8), d8), "history block-sum alloc");
+                SCU(cudaMemset(ss->dh8, 0, d8), "history block-sum clear");
+                dh_b += d8;
+            }
+        }
+    }
     SCU(cudaMalloc(reinterpret_cast<void **>(&ss->base), row * sizeof(float)), "base alloc");
     const size_t mu_b = (size_t)pl->nuniq * pl->npix * sizeof(float);
     SCU(cudaMalloc(reinterpret_cast<void **>(&ss->mu0), mu_b), "mu0 alloc");
@@ -602,7 +643,7 @@ int stream_init(nsfrb_plan *pl, int chunk_nt, std::string &err)
     }
     ss->snr_cube = pl->cube_snr;
     ss->toa_cube = pl->cube_toa;
-    ss->bytes = ring_b + row * sizeof(float) + mu_b + 2 * m_b + s_b + st_b;
+    ss->bytes = ring_b + dh_b + row * sizeof(float) + mu_b + 2 * m_b + s_b + st_b;
     return NSFRB_OK;
 }
 
@@ -612,7 +653,7 @@ void stream_free(nsfrb_plan *p)
 {
     if (!p || !p->stream) return;
     StreamState *ss = p->stream;
-    cudaFree(ss->ring); cudaFree(ss->base); cudaFree(ss->mu0); cudaFree(ss->partials); cudaFree(ss->mws); cudaFree(ss->aws); cudaFree(ss->sws); cudaFree(ss->d_canon);
+    cudaFree(ss->ring); cudaFree(ss->dhist); cudaFree(ss->dh8); cudaFree(ss->base); cudaFree(ss->mu0); cudaFree(ss->partials); cudaFree(ss->mws); cudaFree(ss->aws); cudaFree(ss->sws); cudaFree(ss->d_canon);
     cudaFree(ss->st1); cudaFree(ss->st2); cudaFree(ss->dlt); cudaFree(ss->rsig);
     cudaFree(ss->sig); cudaFree(ss->var); cudaFree(ss->own_cs); cudaFree(ss->own_ct);
     for (auto &l : ss->lib) if (l) cudaLibraryUnload(l);
@@ -679,7 +720,7 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         // the longer one instead (CMAX is the only shape parameter that depends on the chunk; the workspaces do not)
         StreamCfg c2;
         std::string e2;
-        if (choose_cfg(pl, chunk_nt, getenv("NSFRB_STREAM_VARIANT"), c2, e2) && c2.CMAX > ss->cfg.CMAX) {
+        if (choose_cfg(pl, chunk_nt, getenv("NSFRB_STREAM_VARIANT"), c2, e2, ss->cfg.DHIST) && c2.CMAX > ss->cfg.CMAX) {
             SCU(cudaStreamSynchronize(st), "stream sync before the kernel is replaced");
             for (int v = 0; v < 2; ++v) {
                 if (ss->lib[v]) cudaLibraryUnload(ss->lib[v]);
@@ -718,7 +759,7 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
     const int64_t lo_prev = std::max<int64_t>(0, n_prev - L);
     StatsParams tp;
     tp.ring = ss->ring; tp.s1 = ss->st1; tp.s2 = ss->st2; tp.mu = ss->mu0; tp.dlt = ss->dlt; tp.rsig = ss->rsig; tp.sig_out = nullptr;
-    tp.pad = 0; tp.lo_prev = lo_prev; tp.n_prev = n_prev; tp.lo = lo; tp.n = n;
+    tp.dh = ss->dhist; tp.dh8 = ss->dh8; tp.pad = 0; tp.lo_prev = lo_prev; tp.n_prev = n_prev; tp.lo = lo; tp.n = n;
     const dim3 stat_grid((pl->npix + 31) / 32, (pl->nuniq + 7) / 8);
     if (c.INCR && lo > lo_prev && n_prev > 0) {
         tp.row_lo = ss->guard + (int)(lo_prev % L); tp.ring_lo = lo_prev; tp.add = 0; tp.first = 0;
@@ -792,7 +833,7 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         sp.mws = ss->mws; sp.aws = ss->aws; sp.sws = ss->sws;
         sp.snr_cube = cs; sp.toa_cube = ct; sp.t_offset = (int32_t)(lo & 0x7fffffff);
         sp.sig_out = (running && !c.INCR) ? ss->sig : nullptr;
-        sp.dlt = ss->dlt; sp.rsig = ss->rsig;
+        sp.dlt = ss->dlt; sp.rsig = ss->rsig; sp.dh = ss->dhist; sp.dh8 = ss->dh8;
         segment_bounds(pl, c, len, sp.i0, sp.C, sp.bound);
         void *args[] = {&sp};
         dim3 grid((pl->npix + 31) / 32, c.NSUPER);

@@ -69,7 +69,23 @@ struct StreamParams {
     // the march stops after the last start range and accumulates no sum of squares
     const float *dlt;
     const float *rsig;
+    // DHIST = 1: the dedispersed history dh[pixel block][ROWS][NU][32] -- D_u(t) of every unique trial at the row of raw sample
+    // t + dmax_u (same slots and double mapping as the ring), written once per sample by k_stream_stats when the sample enters
+    // the valid set.  The march then reads one value per (trial, step) instead of dedispersing NCHAN channels, and the r-th
+    // sample from the end of every series sits in row top_row - (r - 1): all trials march in their own frames, in step.
+    const float *dh;
+    // COARSE = 1 (needs LRING % 8 == 0): dh8[pixel block][2 * LRING / 8][NU][32], the sums of the 8-row aligned blocks of dh (block
+    // b = rows 8b .. 8b+7 of the ring's slot space, stored at b and b + LRING/8), written when a block's last row arrives.
+    // A plain run of the march adds whole blocks and only the ragged rows at its two ends one by one.
+    const float *dh8;
 };
+
+#ifndef DHIST
+#define DHIST 0
+#endif
+#ifndef COARSE
+#define COARSE 0
+#endif
 
 namespace sk {
 
@@ -100,7 +116,9 @@ template <int G> struct GT {
         return m;
     }
     static __host__ __device__ constexpr int e(int kk, int c) { return dmaxg() - D_TAB[u(kk)][c]; }
-    static __host__ __device__ constexpr int delta(int kk) { return dmaxg() - DMAX_TAB[u(kk)]; } // own step = group step + delta
+    // own step = group step + delta.  (DHIST: the history stores D_u(t) at the row of raw sample t + dmax_u, so the r-th
+    // sample from the end of EVERY series sits in row top - (r - 1): each trial marches in its own frame, delta = 0)
+    static __host__ __device__ constexpr int delta(int kk) { return DHIST ? 0 : dmaxg() - DMAX_TAB[u(kk)]; }
     static __host__ __device__ constexpr int dspread()
     {
         int m = 0;
@@ -131,6 +149,7 @@ template <int G> struct GT {
 };
 
 constexpr int kThreads = 32 * GPC * SEG;
+constexpr int CURN = DHIST ? KK * TT : NCHAN * TT; // values a thread holds for one tile: D of its trials, or the raw rows
 constexpr int kTrialsPerCta = GPC * KK;
 
 // shared memory: Qe[kTrialsPerCta][CMAX][32], the cross-group reduction scratch, and per (group, segment)
@@ -148,11 +167,14 @@ template <int G> struct Worker {
     using T = GT<G>;
     const float *rp;  // &ring[block][top_row][0][lane]
     const float *rp0; // the same for lane 0
+#if DHIST
+    const float *dp, *dp0; // &dh[block][top_row][0][lane], and the same for lane 0
+#endif
     float *qe;       // &Qe[gl*KK][0][lane]
     float *mg;       // &mws[block][gl*KK][0][lane]
     int *ag;         // &aws[block][gl*KK][0][lane]
     int i0, C, len;
-    float carry[T::CARRY];
+    float carry[DHIST ? 1 : T::CARRY];
     float mu[KK], dmu[KK], Q[KK], S2[KK]; // mu: provisional means (mu[0] and the differences dmu are live in the loop)
     int ja, jb; // widths [ja, jb) can have cells in the current tile
     // register cache of one width's running maxima (the rest live in mws/aws)
@@ -193,8 +215,15 @@ template <int G> struct Worker {
         jc = j;
     }
 
-    __device__ __forceinline__ void load_new(float (&buf)[NCHAN * TT], int rb) const
+    __device__ __forceinline__ void load_new(float (&buf)[CURN], int rb) const
     {
+#if DHIST
+        // steps rb+1 .. rb+TT  <=>  history rows top - (rb + tt), one 128-byte segment per (trial, step)
+        const float *d = dp - (long long)rb * (NU * 32);
+        sfor<0, KK>([&](auto kk) {
+            sfor<0, TT>([&](auto tt) { buf[V(kk) * TT + V(tt)] = ldrow(d + (T::u(V(kk)) - V(tt) * NU) * 32); });
+        });
+#else
         const float *b = rp - (long long)rb * (NCHAN * 32);
         sfor<0, NCHAN>([&](auto c) {
             sfor<0, TT>([&](auto tt) {
@@ -202,17 +231,24 @@ template <int G> struct Worker {
                 buf[V(c) * TT + V(tt)] = ldrow(b + off);
             });
         });
+#endif
     }
     // ask L2 for the TT raw rows (all channels: TT*NCHAN*128 contiguous bytes in the blocked ring) that the tile
     // PFD tiles ahead will need first -- one bulk prefetch, no registers held; the later loads hit L2
     __device__ __forceinline__ void prefetch_l2(int rb) const
     {
+#if DHIST
+        const float *dlo = dp0 - (long long)(rb + TT - 1) * (NU * 32); // oldest of the TT rows, trial 0, lane 0
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(dlo), "r"(TT * NU * 128) : "memory");
+#else
         constexpr int emax_all = []() { int m = 0; for (int c = 0; c < NCHAN; ++c) m = T::emax(c) > m ? T::emax(c) : m; return m; }();
         const float *lo = rp0 - (long long)(rb + emax_all + TT - 1) * (NCHAN * 32); // oldest of the TT rows, channel 0, lane 0
         asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(lo), "r"(TT * NCHAN * 128) : "memory");
+#endif
     }
     __device__ __forceinline__ void load_carry(int rb)
     {
+#if !DHIST // (the history holds finished samples: no halo)
         const float *b = rp - (long long)rb * (NCHAN * 32);
         sfor<0, NCHAN>([&](auto c) {
             sfor<0, T::span(V(c))>([&](auto m) {
@@ -220,10 +256,77 @@ template <int G> struct Worker {
                 carry[T::coff(V(c)) + V(m)] = ldrow(b + off);
             });
         });
+#endif
     }
 
 
-#if LIGHT
+#if LIGHT && DHIST && COARSE
+    const float *dv0; // &dh[block][GUARD][0][lane]: virtual row v (0 .. 2*LRING-1; v mod LRING = ring slot) is dv0 + v*NU*32
+    const float *dq0; // &dh8[block][0][0][lane]: block row v >> 3
+    int vtop;         // virtual row of the newest sample
+    // acc[kk] += sum over rows v in [va, vb] of base[(v * NU + u(kk)) * 32]   (warp-uniform bounds; four rows in flight)
+    __device__ __forceinline__ void sum_rows(const float *base, int va, int vb, float (&acc)[KK]) const
+    {
+        for (int v = va; v <= vb; v += 4) {
+            const float *p = base + (long long)v * (NU * 32);
+            float x[4][KK];
+            sfor<0, 4>([&](auto q) {
+                const bool ok = v + V(q) <= vb;
+                sfor<0, KK>([&](auto kk) { x[V(q)][V(kk)] = ok ? ldrow(p + (V(q) * NU + T::u(V(kk))) * 32) : 0.f; });
+            });
+            sfor<0, KK>([&](auto kk) { acc[V(kk)] += (x[0][V(kk)] + x[1][V(kk)]) + (x[2][V(kk)] + x[3][V(kk)]); });
+        }
+    }
+    // ---- a plain run (no end stored, no start range met), steps rb0+1 .. rb_end: only the suffix sums move.  The first tile is
+    // already in `cur`; of the rest, whole 8-row blocks come from dh8, the ragged rows at the two ends from dh.
+    __device__ __forceinline__ void coarse_run(float (&cur)[CURN], int rb0, int rb_end, bool more, bool pf)
+    {
+        float acc[KK];
+        sfor<0, KK>([&](auto kk) {
+            float a0 = 0.f, a1 = 0.f;
+            sfor<0, TT>([&](auto tt) {
+                if constexpr ((V(tt) & 1) == 0) a0 += cur[V(kk) * TT + V(tt)]; else a1 += cur[V(kk) * TT + V(tt)];
+            });
+            acc[V(kk)] = a0 + a1;
+        });
+        if (more) load_new(cur, rb_end); // the tile after the run
+        if (PFD > 0 && pf && more) {      // ... and the rows behind it, which a start range will want
+            const float *plo = dp0 - (long long)(rb_end + 2 * TT + 8 - 1) * (NU * 32);
+            asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(plo), "r"((TT + 8) * NU * 128) : "memory");
+        }
+        const int top = vtop - rb0 - TT, v_lo = vtop - (rb_end - 1); // rows [v_lo, top] remain (step r <-> row vtop - (r - 1))
+        if (top >= v_lo) {
+            const int bfirst = (v_lo + 7) >> 3, blast = ((top + 1) >> 3) - 1;
+            if (blast >= bfirst) {
+                sum_rows(dv0, 8 * (blast + 1), top, acc);
+                sum_rows(dq0, bfirst, blast, acc);
+                sum_rows(dv0, v_lo, 8 * bfirst - 1, acc);
+            } else {
+                sum_rows(dv0, v_lo, top, acc);
+            }
+        }
+        const float fn = (float)(rb_end - rb0);
+        sfor<0, KK>([&](auto kk) { Q[V(kk)] += fmaf(-fn, mu[V(kk)], acc[V(kk)]); });
+    }
+#elif LIGHT && DHIST
+    // ---- plain runs (no end stored, no start range met): only the suffix sums move, one history value per (trial, step)
+    __device__ __forceinline__ void run_begin() {}
+    __device__ __forceinline__ void run_end(float, int) {}
+    __device__ __forceinline__ void light(float (&cur)[CURN], int rb, bool more, bool pf, float &)
+    {
+        float part[KK];
+        sfor<0, KK>([&](auto kk) {
+            float a0 = -(float)TT * mu[V(kk)], a1 = 0.f;
+            sfor<0, TT>([&](auto tt) {
+                if constexpr ((V(tt) & 1) == 0) a0 += cur[V(kk) * TT + V(tt)]; else a1 += cur[V(kk) * TT + V(tt)];
+            });
+            part[V(kk)] = a0 + a1;
+        });
+        if (more) load_new(cur, rb + TT);
+        if (PFD > 0 && pf) prefetch_l2(rb + PFD * TT);
+        sfor<0, KK>([&](auto kk) { Q[V(kk)] += part[V(kk)]; });
+    }
+#elif LIGHT
     // ---- plain runs (no end stored, no start range met): only the suffix sums move.  Over a run of n steps trial kk adds
     //   sum_c sum_{m = o(kk,c)}^{n-1+o(kk,c)} W_c[m]  =  sum_c sum_{m<n} W_c[m]  +  edge(kk) at the exit  -  edge(kk) at the entry,
     // W_c[m] the raw window of channel c counted from the run's first row and edge(kk) = sum_c sum_{m<o(kk,c)} W_c[m], the
@@ -254,7 +357,7 @@ template <int G> struct Worker {
             Q[V(kk)] += (g + edge_of<V(kk)>()) + fn * cd;
         });
     }
-    __device__ __forceinline__ void light(float (&cur)[NCHAN * TT], int rb, bool more, bool pf, float &g)
+    __device__ __forceinline__ void light(float (&cur)[CURN], int rb, bool more, bool pf, float &g)
     {
         auto Wn = [&](auto c, auto m) -> float {
             if constexpr (V(m) < T::span(V(c))) return carry[T::coff(V(c)) + V(m)];
@@ -280,14 +383,19 @@ template <int G> struct Worker {
     // (if `more`) the rows of the next tile have been requested into the same registers.
     // `cells`: the tile stores ends or meets a start range (one code body serves plain and cell tiles: the
     // hot instruction footprint of an SM has to stay within the ~32 KB the instruction cache streams well)
-    template <bool MASKED> __device__ __forceinline__ void tile(float (&cur)[NCHAN * TT], int rb, bool more, bool pf, bool cells)
+    template <bool MASKED> __device__ __forceinline__ void tile(float (&cur)[CURN], int rb, bool more, bool pf, bool cells)
     {
+        float Dv[KK][TT];
+#if DHIST
+        sfor<0, KK>([&](auto kk) {
+            sfor<0, TT>([&](auto tt) { Dv[V(kk)][V(tt)] = cur[V(kk) * TT + V(tt)] - mu[V(kk)]; });
+        });
+#else
         auto Wn = [&](auto c, auto m) -> float {
             if constexpr (V(m) < T::span(V(c))) return carry[T::coff(V(c)) + V(m)];
             else return cur[V(c) * TT + (V(m) - T::span(V(c)))];
         };
         // a2: first trial = plain channel sum, every next one differentially
-        float Dv[KK][TT];
         sfor<0, KK>([&](auto kk) {
             if constexpr (V(kk) == 0) {
                 sfor<0, TT>([&](auto tt) {
@@ -314,6 +422,7 @@ template <int G> struct Worker {
         sfor<0, NCHAN>([&](auto c) {
             sfor<0, T::span(V(c))>([&](auto m) { carry[T::coff(V(c)) + V(m)] = Wn(c, IC<V(m) + TT>{}); });
         });
+#endif
         if (more) load_new(cur, rb + TT); // rows of the next tile; their latency overlaps what follows
         if (PFD > 0 && pf) prefetch_l2(rb + PFD * TT);
         // a1, a3, a4: centred sample, suffix sum (left in Dv), sum of squares
@@ -409,6 +518,15 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     w.i0 = P.i0; w.C = P.C; w.len = P.len;
     w.rp0 = P.ring + ((long long)blockIdx.x * ROWS + P.top_row) * (NCHAN * 32);
     w.rp = w.rp0 + lane;
+#if DHIST
+    w.dp0 = P.dh + ((long long)blockIdx.x * ROWS + P.top_row) * (NU * 32);
+    w.dp = w.dp0 + lane;
+#if LIGHT && COARSE
+    w.vtop = P.top_row - GUARD;
+    w.dv0 = P.dh + ((long long)blockIdx.x * ROWS + GUARD) * (NU * 32) + lane;
+    w.dq0 = P.dh8 + (long long)blockIdx.x * (2 * LRING / 8) * (NU * 32) + lane;
+#endif
+#endif
     w.qe = Qe + (gl * KK) * CMAX * 32 + lane;
     {
         const long long blk = ((long long)blockIdx.x * NSUPER + blockIdx.y) * kTrialsPerCta + gl * KK;
@@ -435,7 +553,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     const bool pf = gl == 0 && lane == 0; // the DM groups of a pixel block read the same rows: one thread prefetches
     bool synced = false;
     if (r_begin < r_end) {
-        float cur[NCHAN * TT];
+        float cur[CURN];
         w.load_carry(r_begin);
         w.load_new(cur, r_begin);
         int rb = r_begin;
@@ -481,6 +599,15 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
 #if LIGHT
                 if (!cells) { // a plain run: up to the tile before the next start range (or the end of the unmasked part)
                     const int stop = plain_until < fast_stop ? plain_until : fast_stop;
+#if DHIST && COARSE
+                    {
+                        const int nt = (stop - rb + TT - 1) / TT;
+                        const int rb_end = rb + (nt > 1 ? nt : 1) * TT;
+                        w.coarse_run(cur, rb, rb_end, rb_end < r_end, pf);
+                        rb = rb_end;
+                        continue;
+                    }
+#else
                     const int rb0 = rb;
                     float g = 0.f;
                     w.run_begin();
@@ -490,6 +617,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                     } while (rb < stop);
                     w.run_end(g, rb - rb0);
                     continue;
+#endif
                 }
 #endif
                 w.template tile<false>(cur, rb, rb + TT < r_end, pf, cells);
@@ -663,14 +791,26 @@ struct StatsParams {
     int row_lo;           // ring row that holds the raw sample of absolute index ring_lo
     int add, first, pad;
     long long ring_lo, lo_prev, n_prev, lo, n;
+    float *dh;            // DHIST: the dedispersed history (see StreamParams), written by the add = 1 launch, read by add = 0
+    float *dh8;           // COARSE: its 8-row block sums, written by the add = 1 launch
 };
 
 namespace sk {
 
 // S1 += sum D, S2 += sum D^2 over cnt consecutive samples of trial U starting at ring pointer rp (lane = pixel).
 // (A sample's D is the same expression wherever it falls in a range: entering, leaving and rebuilding must agree bit for bit.)
-template <int U> __device__ __forceinline__ void stats_range(const float *rp, int cnt, double &a1, double &a2)
+// dcol (DHIST, may be null): &dh[block][GUARD][U][lane]; the sample at ring slot `slot` is also stored there (both mappings).
+template <int U> __device__ __forceinline__ void stats_range(const float *rp, int cnt, double &a1, double &a2, float *dcol = nullptr, int slot = 0)
 {
+    auto keep = [&](float Df) {
+#if DHIST
+        if (dcol) {
+            dcol[(long long)slot * (NU * 32)] = Df;
+            dcol[(long long)(slot + LRING) * (NU * 32)] = Df;
+            slot = slot + 1 == LRING ? 0 : slot + 1;
+        }
+#endif
+    };
     int i = cnt;
     for (; i >= 4; i -= 4, rp += 4 * NCHAN * 32) { // four samples per round: 4*NCHAN loads in flight
         float e[4][4] = {};
@@ -678,7 +818,9 @@ template <int U> __device__ __forceinline__ void stats_range(const float *rp, in
             sfor<0, NCHAN>([&](auto c) { e[V(q)][V(c) & 3] += __ldg(rp + ((D_TAB[U][V(c)] + V(q)) * NCHAN + V(c)) * 32); });
         });
         sfor<0, 4>([&](auto q) {
-            const double D = (double)((e[V(q)][0] + e[V(q)][1]) + (e[V(q)][2] + e[V(q)][3]));
+            const float Df = (e[V(q)][0] + e[V(q)][1]) + (e[V(q)][2] + e[V(q)][3]);
+            keep(Df);
+            const double D = (double)Df;
             a1 += D;
             a2 = fma(D, D, a2);
         });
@@ -686,11 +828,27 @@ template <int U> __device__ __forceinline__ void stats_range(const float *rp, in
     for (; i > 0; --i, rp += NCHAN * 32) {
         float e[4] = {0.f, 0.f, 0.f, 0.f};
         sfor<0, NCHAN>([&](auto c) { e[V(c) & 3] += __ldg(rp + (D_TAB[U][V(c)] * NCHAN + V(c)) * 32); });
-        const double D = (double)((e[0] + e[1]) + (e[2] + e[3]));
+        const float Df = (e[0] + e[1]) + (e[2] + e[3]);
+        keep(Df);
+        const double D = (double)Df;
         a1 += D;
         a2 = fma(D, D, a2);
     }
 }
+#if DHIST
+// the same sums over cnt samples read back from the history (the float that was stored is the float that was added)
+__device__ __forceinline__ void stats_history(const float *dcol, int slot, int cnt, double &a1, double &a2)
+{
+    const float *p = dcol + (long long)slot * (NU * 32); // slot < LRING, cnt <= LRING: the double mapping covers the run
+    int i = cnt;
+    for (; i >= 4; i -= 4, p += 4 * NU * 32) {
+        float d[4];
+        sfor<0, 4>([&](auto q) { d[V(q)] = __ldg(p + V(q) * NU * 32); });
+        sfor<0, 4>([&](auto q) { const double D = (double)d[V(q)]; a1 += D; a2 = fma(D, D, a2); });
+    }
+    for (; i > 0; --i, p += NU * 32) { const double D = (double)__ldg(p); a1 += D; a2 = fma(D, D, a2); }
+}
+#endif
 // sum (D - centre)^2 over the same samples: the second pass of an exact two-pass variance
 template <int U> __device__ __forceinline__ double stats_centred(const float *rp, int cnt, double centre)
 {
@@ -718,7 +876,31 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
     }
     const float *rbase = P.ring + ((long long)blockIdx.x * ROWS + P.row_lo) * (NCHAN * 32) + lane; // sample ring_lo
     double a1 = 0.0, a2 = 0.0;
+#if DHIST
+    float *dcol = P.dh + ((long long)blockIdx.x * ROWS + GUARD) * (NU * 32) + U * 32 + lane;
+    if (tb > ta) {
+        const int slot = (int)((ta + DMAX_TAB[U]) % LRING); // D_u(t) lives at the row of raw sample t + dmax_u
+        if (P.add) stats_range<U>(rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2, dcol, slot);
+        else stats_history(dcol, slot, (int)(tb - ta), a1, a2);
+#if COARSE
+        if (P.add) { // the aligned rows [ra, rz) have just been written: every block whose last row is among them is complete
+            const long long ra = ta + DMAX_TAB[U], rz = tb + DMAX_TAB[U];
+            float *dcol8 = P.dh8 + (long long)blockIdx.x * (2 * LRING / 8) * (NU * 32) + U * 32 + lane;
+            for (long long b = ra >> 3; b <= ((rz - 8) >> 3); ++b) {
+                const int s8 = (int)((8 * b) % LRING); // slot of the block's first row (LRING % 8 == 0: the block does not wrap)
+                const float *r8 = dcol + (long long)s8 * (NU * 32);
+                float d[8];
+                sfor<0, 8>([&](auto q) { d[V(q)] = r8[V(q) * NU * 32]; }); // (plain loads: some of these rows were stored above)
+                const float E = ((d[0] + d[1]) + (d[2] + d[3])) + ((d[4] + d[5]) + (d[6] + d[7]));
+                dcol8[(long long)(s8 >> 3) * (NU * 32)] = E;
+                dcol8[(long long)((s8 >> 3) + LRING / 8) * (NU * 32)] = E;
+            }
+        }
+#endif
+    }
+#else
     stats_range<U>(rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2);
+#endif
     const long long o = (long long)U * NPIX + pix;
     const double kNaN = __longlong_as_double(0x7ff8000000000000LL);
     if (!P.add) {
