@@ -105,12 +105,14 @@ bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamC
         c.DHIST = (c.INCR && dhist) ? 1 : 0;
         const char *co = getenv("NSFRB_STREAM_COARSE");
         c.COARSE = (c.DHIST && c.LIGHT && pl->nt % 8 == 0 && !(co && atoi(co) == 0)) ? 1 : 0;
+        if (c.COARSE && !getenv("NSFRB_STREAM_LIGHT_COST")) c.light_cost = 0.15f; // a plain tile costs one block load per 8 rows
         if (const char *lc = getenv("NSFRB_STREAM_LIGHT_COST")) c.light_cost = (float)atof(lc);
     }
     if (c.DHIST) {
-        // a thread holds KK*TT history values and no raw rows: the trials of a thread share nothing, so fewer trials per
-        // thread and more warps per CTA (the shared-memory Qe block of a CTA is per trial either way)
-        kk = 8; gpc = 2; seg = 1; tt = 4; minb = 4; pfd = 2;
+        // a thread holds KK*TT history values and no raw rows, the trials of a thread share nothing and every DM group runs the
+        // same instance of the code: fewer trials per thread and more warps per CTA (the shared-memory Qe block of a CTA is per
+        // trial either way) -- 4 trials x 4 groups measured best on C2 (profiles/r02.md)
+        kk = 4; gpc = 4; seg = 1; tt = 4; minb = 4; pfd = 2;
     } else if (pl->nchan > 24) { // the thread holds nchan*TT raw rows in registers: one time step per tile, more registers
         tt = 1;
         minb = 2;
@@ -761,7 +763,7 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
     tp.ring = ss->ring; tp.s1 = ss->st1; tp.s2 = ss->st2; tp.mu = ss->mu0; tp.dlt = ss->dlt; tp.rsig = ss->rsig; tp.sig_out = nullptr;
     tp.dh = ss->dhist; tp.dh8 = ss->dh8; tp.pad = 0; tp.lo_prev = lo_prev; tp.n_prev = n_prev; tp.lo = lo; tp.n = n;
     const dim3 stat_grid((pl->npix + 31) / 32, (pl->nuniq + 7) / 8);
-    if (c.INCR && lo > lo_prev && n_prev > 0) {
+    if (c.INCR && !c.DHIST && lo > lo_prev && n_prev > 0) { // (DHIST: the leaving samples come from the history, in the launch below)
         tp.row_lo = ss->guard + (int)(lo_prev % L); tp.ring_lo = lo_prev; tp.add = 0; tp.first = 0;
         void *args[] = {&tp};
         SCU(cudaLaunchKernel((const void *)ss->fn_stats[variant], stat_grid, dim3(256), args, 0, st), "k_stream_stats launch");
@@ -791,7 +793,7 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
     }
     pl->n_received = n;
     if (c.INCR) { // second half: the samples that enter; mean, 1/sigma (and sigma itself for the running-sigma mode)
-        tp.row_lo = ss->guard + (int)(lo % L); tp.ring_lo = lo; tp.add = 1; tp.first = n_prev == 0 ? 1 : 0;
+        tp.row_lo = ss->guard + (int)(lo % L); tp.ring_lo = lo; tp.add = c.DHIST ? 2 : 1; tp.first = n_prev == 0 ? 1 : 0;
         tp.sig_out = running ? ss->sig : nullptr;
         void *args[] = {&tp};
         SCU(cudaLaunchKernel((const void *)ss->fn_stats[variant], stat_grid, dim3(256), args, 0, st), "k_stream_stats launch");

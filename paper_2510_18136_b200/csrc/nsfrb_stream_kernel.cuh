@@ -168,7 +168,19 @@ template <int G> struct Worker {
     const float *rp;  // &ring[block][top_row][0][lane]
     const float *rp0; // the same for lane 0
 #if DHIST
-    const float *dp, *dp0; // &dh[block][top_row][0][lane], and the same for lane 0
+    const float *dp, *dp0; // &dh[block][top_row][u0][lane]; the row's first float
+    // One instance of the march serves every DM group: with the history nothing but the trial column depends on the group
+    // (G = 0 is the only instantiation), so the warps of an SM share one copy of the code.
+    int u0; // first trial of the thread
+    static constexpr bool kFull = NSUPER * GPC * KK == NU; // no padding trial anywhere
+    __device__ __forceinline__ int uof(int kk) const { return (kFull || u0 + kk < NU) ? u0 + kk : NU - 1; }
+    __device__ __forceinline__ bool has(int kk) const { return kFull || u0 + kk < NU; }
+    __device__ __forceinline__ int ubase() const { return u0; }
+    __device__ __forceinline__ int col(int kk) const { return uof(kk) - u0; } // column of the trial relative to dp (a padding trial repeats the last one)
+#else
+    static __device__ __forceinline__ constexpr int uof(int kk) { return T::u(kk); }
+    static __device__ __forceinline__ constexpr bool has(int kk) { return G * KK + kk < NU; }
+    static __device__ __forceinline__ constexpr int ubase() { return G * KK; }
 #endif
     float *qe;       // &Qe[gl*KK][0][lane]
     float *mg;       // &mws[block][gl*KK][0][lane]
@@ -188,7 +200,7 @@ template <int G> struct Worker {
             float *mj = mg + jc * 32;
             int *aj = ag + jc * 32;
             sfor<0, KK>([&](auto kk) {
-                if constexpr (G * KK + V(kk) < NU) {
+                if (has(V(kk))) {
                     mj[V(kk) * NW * 32] = mc[V(kk)];
                     aj[V(kk) * NW * 32] = ac[V(kk)];
                 }
@@ -206,7 +218,7 @@ template <int G> struct Worker {
             const float *mj = mg + j * 32;
             const int *aj = ag + j * 32;
             sfor<0, KK>([&](auto kk) {
-                if constexpr (G * KK + V(kk) < NU) {
+                if (has(V(kk))) {
                     mc[V(kk)] = mj[V(kk) * NW * 32];
                     ac[V(kk)] = aj[V(kk) * NW * 32];
                 }
@@ -221,7 +233,7 @@ template <int G> struct Worker {
         // steps rb+1 .. rb+TT  <=>  history rows top - (rb + tt), one 128-byte segment per (trial, step)
         const float *d = dp - (long long)rb * (NU * 32);
         sfor<0, KK>([&](auto kk) {
-            sfor<0, TT>([&](auto tt) { buf[V(kk) * TT + V(tt)] = ldrow(d + (T::u(V(kk)) - V(tt) * NU) * 32); });
+            sfor<0, TT>([&](auto tt) { buf[V(kk) * TT + V(tt)] = ldrow(d + (col(V(kk)) - V(tt) * NU) * 32); });
         });
 #else
         const float *b = rp - (long long)rb * (NCHAN * 32);
@@ -272,7 +284,7 @@ template <int G> struct Worker {
             float x[4][KK];
             sfor<0, 4>([&](auto q) {
                 const bool ok = v + V(q) <= vb;
-                sfor<0, KK>([&](auto kk) { x[V(q)][V(kk)] = ok ? ldrow(p + (V(q) * NU + T::u(V(kk))) * 32) : 0.f; });
+                sfor<0, KK>([&](auto kk) { x[V(q)][V(kk)] = ok ? ldrow(p + (V(q) * NU + col(V(kk))) * 32) : 0.f; });
             });
             sfor<0, KK>([&](auto kk) { acc[V(kk)] += (x[0][V(kk)] + x[1][V(kk)]) + (x[2][V(kk)] + x[3][V(kk)]); });
         }
@@ -431,7 +443,7 @@ template <int G> struct Worker {
                 float x = Dv[V(kk)][V(tt)];
                 if constexpr (MASKED) {
                     const int ro = rb + 1 + V(tt) + T::delta(V(kk)); // step in the trial's own frame
-                    x = (ro >= 1 && ro <= len - DMAX_TAB[T::u(V(kk))]) ? x : 0.f;
+                    x = (ro >= 1 && ro <= len - DMAX_TAB[uof(V(kk))]) ? x : 0.f;
                 }
                 Q[V(kk)] += x;
 #if !INCR
@@ -444,7 +456,7 @@ template <int G> struct Worker {
             // Q at the ends of this pass: Qe[ii] = Q(i0 + ii), own frame
             float *qb = qe + (rb + 1 - i0) * 32;
             sfor<0, KK>([&](auto kk) {
-                if constexpr (G * KK + V(kk) < NU)
+                if (has(V(kk)))
                     sfor<0, TT>([&](auto tt) {
                         const unsigned ii = (unsigned)(rb + 1 - i0 + V(tt) + T::delta(V(kk)));
                         if (ii < (unsigned)C) qb[(V(kk) * CMAX + V(tt) + T::delta(V(kk))) * 32] = Dv[V(kk)][V(tt)];
@@ -463,7 +475,7 @@ template <int G> struct Worker {
                 const bool inside = !MASKED && ib >= 0 && ib + TT - 1 + T::dspread() < C;
                 if (inside) { // every cell of the tile is defined: no range checks
                     sfor<0, KK>([&](auto kk) {
-                        if constexpr (G * KK + V(kk) < NU)
+                        if (has(V(kk)))
                             sfor<0, TT>([&](auto tt) {
                                 const float v = Dv[V(kk)][V(tt)] - qb[(V(kk) * CMAX + V(tt) + T::delta(V(kk))) * 32];
                                 if (v >= mc[V(kk)]) { mc[V(kk)] = v; ac[V(kk)] = ib + V(tt) + T::delta(V(kk)); }
@@ -471,13 +483,13 @@ template <int G> struct Worker {
                     });
                 } else {
                     sfor<0, KK>([&](auto kk) {
-                        if constexpr (G * KK + V(kk) < NU)
+                        if (has(V(kk)))
                             sfor<0, TT>([&](auto tt) {
                                 const int ii = ib + V(tt) + T::delta(V(kk));
                                 bool in = (unsigned)ii < (unsigned)C;
                                 if constexpr (MASKED) {
                                     const int ro = rb + 1 + V(tt) + T::delta(V(kk));
-                                    in = in && ro >= 1 && ro <= len - DMAX_TAB[T::u(V(kk))];
+                                    in = in && ro >= 1 && ro <= len - DMAX_TAB[uof(V(kk))];
                                 }
                                 if (in) {
                                     const float v = Dv[V(kk)][V(tt)] - qb[(V(kk) * CMAX + V(tt) + T::delta(V(kk))) * 32];
@@ -505,7 +517,7 @@ __device__ __forceinline__ bool better(float s, int k, int j, int t, float bs, i
 }
 
 template <int G>
-__device__ __forceinline__ void run_group(const StreamParams &P, float *smem, int gl, int seg, int lane, int pix, bool live)
+__device__ __forceinline__ void run_group(const StreamParams &P, float *smem, int gl, int seg, int lane, int pix, bool live, int u0 = 0)
 {
     using T = GT<G>;
     float *Qe = smem;
@@ -515,16 +527,19 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     int *rng = reinterpret_cast<int *>(red + kRedFloats);
 
     Worker<G> w;
+#if DHIST
+    w.u0 = u0;
+#endif
     w.i0 = P.i0; w.C = P.C; w.len = P.len;
     w.rp0 = P.ring + ((long long)blockIdx.x * ROWS + P.top_row) * (NCHAN * 32);
     w.rp = w.rp0 + lane;
 #if DHIST
     w.dp0 = P.dh + ((long long)blockIdx.x * ROWS + P.top_row) * (NU * 32);
-    w.dp = w.dp0 + lane;
+    w.dp = w.dp0 + u0 * 32 + lane;
 #if LIGHT && COARSE
     w.vtop = P.top_row - GUARD;
-    w.dv0 = P.dh + ((long long)blockIdx.x * ROWS + GUARD) * (NU * 32) + lane;
-    w.dq0 = P.dh8 + (long long)blockIdx.x * (2 * LRING / 8) * (NU * 32) + lane;
+    w.dv0 = P.dh + ((long long)blockIdx.x * ROWS + GUARD) * (NU * 32) + u0 * 32 + lane;
+    w.dq0 = P.dh8 + (long long)blockIdx.x * (2 * LRING / 8) * (NU * 32) + u0 * 32 + lane;
 #endif
 #endif
     w.qe = Qe + (gl * KK) * CMAX * 32 + lane;
@@ -535,7 +550,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     }
     w.ja = 0; w.jb = 0; w.jc = -1; w.jfirst = -1; w.jseen = -1;
     sfor<0, KK>([&](auto kk) {
-        w.mu[V(kk)] = P.mu0[(long long)T::u(V(kk)) * NPIX + pix];
+        w.mu[V(kk)] = P.mu0[(long long)w.uof(V(kk)) * NPIX + pix];
         w.Q[V(kk)] = 0.f;
         w.S2[V(kk)] = 0.f;
         w.dmu[V(kk)] = 0.f;
@@ -548,15 +563,21 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
     // group frame: segment 0 starts with the masked lead-in that covers the newest delta_u samples
     constexpr int kLead = (T::dspread() + TT - 1) / TT * TT;
     const int r_begin = seg == 0 ? -kLead : P.bound[seg], r_end = P.bound[seg + 1];
-    const int r_fast_end = P.len - T::dmaxg(); // last group step (valid for every trial of the group)
+#if DHIST
+    int dmaxg = 0;
+    sfor<0, KK>([&](auto kk) { dmaxg = DMAX_TAB[w.uof(V(kk))] > dmaxg ? DMAX_TAB[w.uof(V(kk))] : dmaxg; });
+#else
+    constexpr int dmaxg = T::dmaxg();
+#endif
+    const int r_fast_end = P.len - dmaxg; // last group step (valid for every trial of the group)
     const int qe_end = P.i0 + P.C;             // group steps < qe_end may store Qe (they lie in segment 0)
     const bool pf = gl == 0 && lane == 0; // the DM groups of a pixel block read the same rows: one thread prefetches
     bool synced = false;
     if (r_begin < r_end) {
         float cur[CURN];
-        w.load_carry(r_begin);
-        w.load_new(cur, r_begin);
         int rb = r_begin;
+        w.load_carry(rb);
+        w.load_new(cur, rb);
         int plain_until = r_begin; // exclusive
         // classify the tile at rb: does it store ends or meet a start range?  (also keeps the Qe barrier protocol)
         auto classify = [&]() -> bool {
@@ -654,7 +675,7 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
         // unrolled over KK trials x NW widths it was 150 KB of instructions fetched for a single pass)
 #pragma unroll 1
         for (int kk = 0; kk < KK; ++kk) {
-            const int u = G * KK + kk;
+            const int u = w.ubase() + kk;
             if (u < NU) {
                 const int Tk = P.len - DMAX_TAB[u];
                 if (Tk >= 1) {
@@ -773,7 +794,11 @@ extern "C" __global__ void __launch_bounds__(sk::kThreads, MINB) k_stream(const 
     const bool live = pix < NPIX;
     if (!live) pix = NPIX - 1;
     const int g = blockIdx.y * GPC + gl; // DM group of this warp; NSUPER*GPC groups exist (the last may be padding)
+#if DHIST
+    sk::run_group<0>(P, smem, gl, seg, lane, pix, live, g * KK);
+#else
     sk::dispatch<0, NSUPER * GPC>(g, P, smem, gl, seg, lane, pix, live);
+#endif
 }
 
 #if INCR
@@ -843,10 +868,10 @@ __device__ __forceinline__ void stats_history(const float *dcol, int slot, int c
     int i = cnt;
     for (; i >= 4; i -= 4, p += 4 * NU * 32) {
         float d[4];
-        sfor<0, 4>([&](auto q) { d[V(q)] = __ldg(p + V(q) * NU * 32); });
+        sfor<0, 4>([&](auto q) { d[V(q)] = p[V(q) * NU * 32]; }); // (plain loads: the fused launch stores to these rows afterwards)
         sfor<0, 4>([&](auto q) { const double D = (double)d[V(q)]; a1 += D; a2 = fma(D, D, a2); });
     }
-    for (; i > 0; --i, p += NU * 32) { const double D = (double)__ldg(p); a1 += D; a2 = fma(D, D, a2); }
+    for (; i > 0; --i, p += NU * 32) { const double D = (double)p[0]; a1 += D; a2 = fma(D, D, a2); }
 }
 #endif
 // sum (D - centre)^2 over the same samples: the second pass of an exact two-pass variance
@@ -864,27 +889,44 @@ template <int U> __device__ __forceinline__ double stats_centred(const float *rp
 
 template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &P, int lane, int pix, bool live)
 {
+    // P.add: 0 = take out the samples that leave V_u, 1 = put in the ones that enter and publish, 2 = both (DHIST: the leaving
+    // samples are read from the history, so nothing has to run before the ring update)
     constexpr long long dm = DMAX_TAB[U];
+    const bool do_rm = P.add != 1, do_add = P.add != 0;
     const long long b_prev = P.lo_prev > P.n_prev - dm ? P.lo_prev : P.n_prev - dm; // end of the previous valid set
-    long long ta, tb;
-    if (P.add) {
-        ta = b_prev > P.lo ? b_prev : P.lo;
-        tb = P.lo > P.n - dm ? P.lo : P.n - dm;
-    } else {
-        ta = P.lo_prev;
-        tb = P.lo < b_prev ? P.lo : b_prev;
-    }
+    const long long la = P.lo_prev, lb = P.lo < b_prev ? P.lo : b_prev;             // leaving:  [la, lb)
+    const long long ta = b_prev > P.lo ? b_prev : P.lo, tb = P.lo > P.n - dm ? P.lo : P.n - dm; // entering: [ta, tb)
     const float *rbase = P.ring + ((long long)blockIdx.x * ROWS + P.row_lo) * (NCHAN * 32) + lane; // sample ring_lo
+    const long long o = (long long)U * NPIX + pix;
+    const double kNaN = __longlong_as_double(0x7ff8000000000000LL);
+#if DHIST
+    float *dcol = P.dh + ((long long)blockIdx.x * ROWS + GUARD) * (NU * 32) + U * 32 + lane; // D_u(t) lives at the row of raw sample t + dmax_u
+#endif
+    double s1 = 0.0, s2 = 0.0; // the carried sums
+    if (!P.first) { s1 = P.s1[o]; s2 = P.s2[o]; }
+    if (do_rm && lb > la) {
+        double a1 = 0.0, a2 = 0.0;
+#if DHIST
+        stats_history(dcol, (int)((la + dm) % LRING), (int)(lb - la), a1, a2);
+#else
+        stats_range<U>(rbase + (la - P.ring_lo) * (NCHAN * 32), (int)(lb - la), a1, a2);
+#endif
+        // A leaving sample that dwarfs what stays behind (|D| beyond ~10^3 sigma sqrt(T)) has eaten the low bits of S2 when it
+        // entered, and a non-finite one has destroyed the sums: mark the series (NaN); the add pass rebuilds it from the ring.
+        const double r1 = s1 - a1, r2 = s2 - a2;
+        const bool bad = !(a2 <= 1048576.0 * fabs(r2)) || !(fabs(r1) <= 1.7e308);
+        s1 = bad ? kNaN : r1;
+        s2 = bad ? kNaN : r2;
+        if (!do_add && live) { P.s1[o] = s1; P.s2[o] = s2; }
+    }
+    if (!do_add) return;
     double a1 = 0.0, a2 = 0.0;
 #if DHIST
-    float *dcol = P.dh + ((long long)blockIdx.x * ROWS + GUARD) * (NU * 32) + U * 32 + lane;
     if (tb > ta) {
-        const int slot = (int)((ta + DMAX_TAB[U]) % LRING); // D_u(t) lives at the row of raw sample t + dmax_u
-        if (P.add) stats_range<U>(rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2, dcol, slot);
-        else stats_history(dcol, slot, (int)(tb - ta), a1, a2);
+        stats_range<U>(rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2, dcol, (int)((ta + dm) % LRING));
 #if COARSE
-        if (P.add) { // the aligned rows [ra, rz) have just been written: every block whose last row is among them is complete
-            const long long ra = ta + DMAX_TAB[U], rz = tb + DMAX_TAB[U];
+        { // the aligned rows [ra, rz) have just been written: every block whose last row is among them is complete
+            const long long ra = ta + dm, rz = tb + dm;
             float *dcol8 = P.dh8 + (long long)blockIdx.x * (2 * LRING / 8) * (NU * 32) + U * 32 + lane;
             for (long long b = ra >> 3; b <= ((rz - 8) >> 3); ++b) {
                 const int s8 = (int)((8 * b) % LRING); // slot of the block's first row (LRING % 8 == 0: the block does not wrap)
@@ -901,24 +943,11 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
 #else
     stats_range<U>(rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2);
 #endif
-    const long long o = (long long)U * NPIX + pix;
-    const double kNaN = __longlong_as_double(0x7ff8000000000000LL);
-    if (!P.add) {
-        if (live && tb > ta) {
-            // A leaving sample that dwarfs what stays behind (|D| beyond ~10^3 sigma sqrt(T)) has eaten the low bits of S2 when it
-            // entered, and a non-finite one has destroyed the sums: mark the series (NaN); the add pass rebuilds it from the ring.
-            const double r1 = P.s1[o] - a1, r2 = P.s2[o] - a2;
-            const bool bad = !(a2 <= 1048576.0 * fabs(r2)) || !(fabs(r1) <= 1.7e308);
-            P.s1[o] = bad ? kNaN : r1;
-            P.s2[o] = bad ? kNaN : r2;
-        }
-        return;
-    }
     const long long Tk = tb - P.lo; // tb = max(lo, n - dmax_u)
     bool rebuild = false;
     if (!P.first) {
-        a1 += P.s1[o];
-        a2 += P.s2[o];
+        a1 += s1;
+        a2 += s2;
         rebuild = !(fabs(a1) <= 1.7e308) || !(fabs(a2) <= 1.7e308); // marked, or poisoned by a non-finite sample
     }
     if (__any_sync(0xffffffffu, rebuild)) { // warp = one trial, lanes = pixels: the whole valid set once more (rare)
