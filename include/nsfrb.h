@@ -230,6 +230,17 @@ int nsfrb_plan_get_info(const nsfrb_plan *plan, nsfrb_plan_info *info);
 int nsfrb_plan_last_launches(const nsfrb_plan *plan);
 
 /*
+ * How the real-time path of this plan holds its data, for harnesses that report traffic:
+ *   0  no streaming state yet (no push, no NSFRB_PREPARE_STREAM)
+ *   1  raw ring only: every push dedisperses the rows it marches over
+ *   2  raw ring + dedispersed history: D_u(t) of every unique trial is formed once, when the sample arrives
+ *   3  as 2, plus the sums of the history's 8-sample blocks (ring length a multiple of 8): the default where it fits
+ * Mode 2/3 take nuniq/nchan times the raw ring's memory again; where that exceeds half of the free device memory at the
+ * first push (or with NSFRB_STREAM_DHIST=0) the plan runs in mode 1.  Results are the same in every mode (S-rules).
+ */
+int nsfrb_stream_mode(const nsfrb_plan *plan);
+
+/*
  * Per-kernel device timing for harnesses.  With profiling on, every call records CUDA events
  * on its stream around each kernel it enqueues.  nsfrb_plan_get_kernel_ms waits for the last
  * call's events and writes the milliseconds of out[0] = layout kernel (transpose or ring push),

@@ -830,6 +830,8 @@ int nsfrb_measure_peaks(int iters, double *per_s, double *per_clk_sm, void *stre
 
 int nsfrb_plan_last_launches(const nsfrb_plan *pl) { return pl ? pl->last_launches : 0; }
 
+int nsfrb_stream_mode(const nsfrb_plan *pl) { return pl ? stream_mode(pl) : 0; }
+
 int nsfrb_plan_set_profiling(nsfrb_plan *pl, int on)
 {
     if (!pl) return fail(NSFRB_EINVAL, "plan is null");

@@ -174,6 +174,7 @@ int stream_prepare(nsfrb_plan *pl, int chunk_nt, std::string &err); // allocate 
 int stream_set_cubes(nsfrb_plan *pl, float *snr_cube, int32_t *toa_cube, std::string &err);
 int stream_set_running(nsfrb_plan *pl, double alpha, float *snr_run, int32_t *arg_run, std::string &err);
 size_t stream_bytes(const nsfrb_plan *p); // device bytes the real-time path holds (0 before the first push)
+int stream_mode(const nsfrb_plan *p);     // 0 none yet, 1 raw ring, 2 + dedispersed history, 3 + its 8-sample block sums
 // a8 + k_stream passes + reduction over slices; outputs as nsfrb_stream_push.  Returns an NSFRB_* code and
 // leaves the message in `err`.
 int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t st, float *snr_map, int32_t *argmax,

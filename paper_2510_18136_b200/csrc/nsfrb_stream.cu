@@ -676,6 +676,13 @@ int stream_set_cubes(nsfrb_plan *pl, float *snr_cube, int32_t *toa_cube, std::st
 
 size_t stream_bytes(const nsfrb_plan *p) { return (p && p->stream) ? p->stream->bytes : 0; }
 
+int stream_mode(const nsfrb_plan *p)
+{
+    if (!p || !p->stream) return 0;
+    const StreamCfg &c = p->stream->cfg;
+    return c.DHIST ? (c.COARSE ? 3 : 2) : 1;
+}
+
 void stream_reset(nsfrb_plan *p)
 {
     if (!p || !p->stream) return;

@@ -276,17 +276,30 @@ template <int G> struct Worker {
     const float *dv0; // &dh[block][GUARD][0][lane]: virtual row v (0 .. 2*LRING-1; v mod LRING = ring slot) is dv0 + v*NU*32
     const float *dq0; // &dh8[block][0][0][lane]: block row v >> 3
     int vtop;         // virtual row of the newest sample
-    // acc[kk] += sum over rows v in [va, vb] of base[(v * NU + u(kk)) * 32]   (warp-uniform bounds; four rows in flight)
-    __device__ __forceinline__ void sum_rows(const float *base, int va, int vb, float (&acc)[KK]) const
+    // acc[kk] += sum over the rows [va, vb] and [vc, vd] of base[(v * NU + u(kk)) * 32]   (warp-uniform bounds, either range may
+    // be empty; RIF rows = 32 loads in flight per thread)
+    static constexpr int RIF = KK >= 8 ? 4 : (KK >= 4 ? 8 : 16);
+    __device__ __forceinline__ void sum_rows(const float *base, int va, int vb, int vc, int vd, float (&acc)[KK]) const
     {
-        for (int v = va; v <= vb; v += 4) {
-            const float *p = base + (long long)v * (NU * 32);
-            float x[4][KK];
-            sfor<0, 4>([&](auto q) {
-                const bool ok = v + V(q) <= vb;
-                sfor<0, KK>([&](auto kk) { x[V(q)][V(kk)] = ok ? ldrow(p + (V(q) * NU + col(V(kk))) * 32) : 0.f; });
+        const int n1 = vb >= va ? vb - va + 1 : 0, n = n1 + (vd >= vc ? vd - vc + 1 : 0);
+        for (int i = 0; i < n; i += RIF) {
+            float x[RIF][KK];
+            sfor<0, RIF>([&](auto q) {
+                const int idx = i + V(q);
+                const bool ok = idx < n;
+                const int v = idx < n1 ? va + idx : vc + (idx - n1);
+                const float *p = base + (long long)v * (NU * 32);
+                sfor<0, KK>([&](auto kk) { x[V(q)][V(kk)] = ok ? ldrow(p + col(V(kk)) * 32) : 0.f; });
             });
-            sfor<0, KK>([&](auto kk) { acc[V(kk)] += (x[0][V(kk)] + x[1][V(kk)]) + (x[2][V(kk)] + x[3][V(kk)]); });
+            sfor<0, KK>([&](auto kk) {
+                float t[RIF];
+                sfor<0, RIF>([&](auto q) { t[V(q)] = x[V(q)][V(kk)]; });
+                sfor<0, RIF / 2>([&](auto q) { t[V(q)] += t[V(q) + RIF / 2]; });
+                if constexpr (RIF >= 4) sfor<0, RIF / 4>([&](auto q) { t[V(q)] += t[V(q) + RIF / 4]; });
+                if constexpr (RIF >= 8) sfor<0, RIF / 8>([&](auto q) { t[V(q)] += t[V(q) + RIF / 8]; });
+                if constexpr (RIF >= 16) t[0] += t[1];
+                acc[V(kk)] += t[0];
+            });
         }
     }
     // ---- a plain run (no end stored, no start range met), steps rb0+1 .. rb_end: only the suffix sums move.  The first tile is
@@ -310,11 +323,10 @@ template <int G> struct Worker {
         if (top >= v_lo) {
             const int bfirst = (v_lo + 7) >> 3, blast = ((top + 1) >> 3) - 1;
             if (blast >= bfirst) {
-                sum_rows(dv0, 8 * (blast + 1), top, acc);
-                sum_rows(dq0, bfirst, blast, acc);
-                sum_rows(dv0, v_lo, 8 * bfirst - 1, acc);
+                sum_rows(dv0, 8 * (blast + 1), top, v_lo, 8 * bfirst - 1, acc); // the ragged rows at both ends, in one go
+                sum_rows(dq0, bfirst, blast, 0, -1, acc);
             } else {
-                sum_rows(dv0, v_lo, top, acc);
+                sum_rows(dv0, v_lo, top, 0, -1, acc);
             }
         }
         const float fn = (float)(rb_end - rb0);

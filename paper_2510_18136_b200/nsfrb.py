@@ -43,7 +43,7 @@ assert CAND_DTYPE.itemsize == ctypes.sizeof(nsfrb_cand) == 20
 # every symbol include/nsfrb.h declares
 EXPORTS = ("nsfrb_plan_create", "nsfrb_search", "nsfrb_stream_push", "nsfrb_stream_reset", "nsfrb_search_host",
            "nsfrb_stream_push_host", "nsfrb_plan_destroy", "nsfrb_plan_get_delays", "nsfrb_plan_get_info",
-           "nsfrb_plan_last_launches", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
+           "nsfrb_plan_last_launches", "nsfrb_stream_mode", "nsfrb_plan_set_profiling", "nsfrb_plan_get_kernel_ms", "nsfrb_last_error",
            "nsfrb_version", "nsfrb_jit_stream_kernel", "nsfrb_bin_time", "nsfrb_jit_search_kernel", "nsfrb_stream_set_cubes",
            "nsfrb_psf_mask", "nsfrb_cluster", "nsfrb_median_subtract",
            "nsfrb_stream_push_host_async", "nsfrb_stream_wait", "nsfrb_stream_set_running_sigma",
@@ -86,6 +86,8 @@ def lib() -> ctypes.CDLL:
         L.nsfrb_plan_get_info.argtypes = [vp, ctypes.POINTER(nsfrb_plan_info)]
         L.nsfrb_plan_last_launches.restype = ctypes.c_int
         L.nsfrb_plan_last_launches.argtypes = [vp]
+        L.nsfrb_stream_mode.restype = ctypes.c_int
+        L.nsfrb_stream_mode.argtypes = [vp]
         L.nsfrb_plan_set_profiling.restype = ctypes.c_int
         L.nsfrb_plan_set_profiling.argtypes = [vp, ctypes.c_int]
         L.nsfrb_plan_get_kernel_ms.restype = ctypes.c_int
@@ -374,6 +376,10 @@ class Plan:
 
     def last_launches(self) -> int:
         return int(lib().nsfrb_plan_last_launches(self._h))
+
+    def stream_mode(self) -> int:
+        """nsfrb_stream_mode: 0 no streaming state yet, 1 raw ring, 2 + dedispersed history, 3 + its block sums."""
+        return int(lib().nsfrb_stream_mode(self._h))
 
     def set_profiling(self, on: bool = True):
         _check(lib().nsfrb_plan_set_profiling(self._h, int(on)))

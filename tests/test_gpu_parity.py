@@ -165,7 +165,7 @@ def _check_recovery(wl, d, pulses, snr, frac=0.7):
 
 
 # ----------------------------------------------------------------------------- streaming (C2)
-def _stream_case(wl, n_push, eval_at, chunk_sizes=None, capacity=1024, cubes=False):
+def _stream_case(wl, n_push, eval_at, chunk_sizes=None, capacity=1024, cubes=False, expect_mode=None):
     nsfrb = _nsfrb()
     d = oracle.delays(wl.freqs_GHz, wl.tsamp_s, wl.dm_list)
     src = W.ChunkSource(wl, d, n_push, "cuda")
@@ -185,6 +185,8 @@ def _stream_case(wl, n_push, eval_at, chunk_sizes=None, capacity=1024, cubes=Fal
                 chunk = torch.randn((wl.nchan, c, wl.npix), device="cuda", generator=src.g)
             plan.stream_push(chunk, out)
             torch.cuda.synchronize()
+            if expect_mode is not None:
+                assert plan.stream_mode() == expect_mode
             ch = chunk.cpu().numpy()
             n_prev = so.n
             so.n += ch.shape[1]
@@ -226,6 +228,29 @@ def test_stream_small_ring_variable_chunks():
     from dataclasses import replace
     wl = replace(W.config("c2").scaled(9, 5, nt=300), width_list=np.asarray([1, 2, 5, 16, 40, 120, 250], np.int32))
     _stream_case(wl, 40, eval_at=set(range(40)), chunk_sizes=[25, 1, 7, 60, 300, 13])
+
+
+@pytest.mark.parametrize("env,nt,mode", [
+    ({}, 256, 3),                                                  # default: dedispersed history + 8-row block sums
+    ({"NSFRB_STREAM_COARSE": "0"}, 256, 2),                        # history, plain runs row by row
+    ({}, 250, 2),                                                  # ring length not a multiple of 8: no block sums
+    ({"NSFRB_STREAM_DHIST": "0"}, 256, 1),                         # raw ring: the march dedisperses
+    ({"NSFRB_STREAM_VARIANT": "8,2,1,4,4,2"}, 256, 3),             # other tile shapes of the history march ...
+    ({"NSFRB_STREAM_VARIANT": "2,8,1,2,4,0"}, 256, 3),
+    ({"NSFRB_STREAM_VARIANT": "3,2,2,4,2,2"}, 256, 3),             # ... padding trials (16 = 5 x 3 + 1) and two time segments
+    ({"NSFRB_STREAM_DHIST": "0", "NSFRB_STREAM_VARIANT": "8,2,2,2,3,6"}, 256, 1),   # ... and of the raw march
+    ({"NSFRB_STREAM_DHIST": "0", "NSFRB_STREAM_LIGHT": "0"}, 256, 1),
+    ({"NSFRB_STREAM_STATS": "march"}, 256, 1),                     # round-1 behaviour: statistics in the march itself
+])
+def test_stream_modes_and_tile_shapes(monkeypatch, env, nt, mode):
+    """Every way the real-time path can hold and march its data (nsfrb_stream_mode, the NSFRB_STREAM_* knobs of DESIGN.md 7.4)
+    gives the oracle's result on every push: eight laps of a short ring, chunk sizes from 1 sample to (nearly) the whole ring,
+    widths up to the ring length (plain runs with ragged ends on both sides of the 8-row blocks, wrap-around of the slots)."""
+    from dataclasses import replace
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
+    wl = replace(W.config("c2").scaled(9, 5, nt=nt), width_list=np.asarray([1, 2, 5, 16, 40, 70, 120, 245], np.int32))
+    _stream_case(wl, 48, eval_at=set(range(48)), chunk_sizes=[25, 1, 7, 60, 250, 13, 25, 25], expect_mode=mode)
 
 
 def test_stream_equals_offline_on_ring_contents():

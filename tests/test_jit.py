@@ -33,18 +33,22 @@ def test_duplicate_trials_and_unused_widths_are_dropped_from_the_kernel():
 
 
 def test_default_shape_and_modes_are_in_the_prologue(monkeypatch):
-    """Default: incremental statistics + light tiles, one time segment, three steps per tile (DESIGN.md 5.2);
-    NSFRB_STREAM_STATS=march restores the whole-ring march with the v4 shape; above 24 channels one step per tile."""
+    """Default: incremental statistics + dedispersed history with 8-row block sums, 4 trials x 4 groups per CTA, one time segment,
+    four steps per tile.  NSFRB_STREAM_DHIST=0 gives the raw-ring march (light tiles, three steps per tile),
+    NSFRB_STREAM_STATS=march the whole-ring march with the v4 shape; the raw march above 24 channels takes one step per tile."""
     wl = W.config("c2")
     src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
-    for d in ("#define INCR 1", "#define LIGHT 1", "#define SEG 1", "#define TT 3", "#define KK 8", "#define GPC 2", "#define PFD 4"):
+    for d in ("#define INCR 1", "#define LIGHT 1", "#define DHIST 1", "#define COARSE 1", "#define SEG 1", "#define TT 4", "#define KK 4",
+              "#define GPC 4", "#define PFD 2", "#define LRING 1536"):
         assert d in src, d
     assert "k_stream_stats" in src
-    monkeypatch.setenv("NSFRB_STREAM_STATS", "march")
+    src = nsfrb.jit_stream_kernel(wl.nx, wl.ny, wl.nchan, 1532, wl.freqs_GHz, wl.tsamp_s, wl.dm_list, wl.width_list, 25).decode()
+    assert "#define DHIST 1" in src and "#define COARSE 0" in src          # block sums need a ring length that is a multiple of 8
+    monkeypatch.setenv("NSFRB_STREAM_DHIST", "0")
     src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
-    for d in ("#define INCR 0", "#define LIGHT 0", "#define SEG 2", "#define TT 2"):
+    for d in ("#define INCR 1", "#define LIGHT 1", "#define DHIST 0", "#define COARSE 0", "#define SEG 1", "#define TT 3", "#define KK 8",
+              "#define GPC 2", "#define PFD 4"):
         assert d in src, d
-    monkeypatch.delenv("NSFRB_STREAM_STATS")
     monkeypatch.setenv("NSFRB_STREAM_LIGHT", "0")
     src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
     assert "#define INCR 1" in src and "#define LIGHT 0" in src and "#define SEG 2" in src
@@ -52,6 +56,11 @@ def test_default_shape_and_modes_are_in_the_prologue(monkeypatch):
     wl5 = W.config("c5")
     src = nsfrb.jit_stream_kernel(wl5.nx, wl5.ny, wl5.nchan, 1536, wl5.freqs_GHz, wl5.tsamp_s, wl5.dm_list[:16], wl5.width_list, 25).decode()
     assert "#define NCHAN 64" in src and "#define TT 1" in src and "#define SEG 2" in src
+    monkeypatch.delenv("NSFRB_STREAM_DHIST")
+    monkeypatch.setenv("NSFRB_STREAM_STATS", "march")
+    src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
+    for d in ("#define INCR 0", "#define LIGHT 0", "#define DHIST 0", "#define SEG 2", "#define TT 2"):
+        assert d in src, d
 
 
 def test_bad_variant_is_rejected():
