@@ -276,12 +276,15 @@ template <int G> struct Worker {
     const float *dv0; // &dh[block][GUARD][0][lane]: virtual row v (0 .. 2*LRING-1; v mod LRING = ring slot) is dv0 + v*NU*32
     const float *dq0; // &dh8[block][0][0][lane]: block row v >> 3
     int vtop;         // virtual row of the newest sample
-    // acc[kk] += sum over the rows [va, vb] and [vc, vd] of base[(v * NU + u(kk)) * 32]   (warp-uniform bounds, either range may
-    // be empty; RIF rows = 32 loads in flight per thread)
+    // acc[kk] += sum over the rows [va, vb] and [vc, vd] of (base[(v * NU + u(kk)) * 32] - cm[kk])   (warp-uniform bounds, either
+    // range may be empty; RIF rows = 32 loads in flight per thread).  cm: the provisional mean (times 8 for block sums) -- every
+    // value is centred BEFORE it is accumulated, as in a tile, so the sums stay small where the level is far from zero.
     static constexpr int RIF = KK >= 8 ? 4 : (KK >= 4 ? 8 : 16);
-    __device__ __forceinline__ void sum_rows(const float *base, int va, int vb, int vc, int vd, float (&acc)[KK]) const
+    __device__ __forceinline__ void sum_rows(const float *base, int va, int vb, int vc, int vd, float scale, float (&acc)[KK]) const
     {
         const int n1 = vb >= va ? vb - va + 1 : 0, n = n1 + (vd >= vc ? vd - vc + 1 : 0);
+        float cm[KK];
+        sfor<0, KK>([&](auto kk) { cm[V(kk)] = scale * mu[V(kk)]; });
         for (int i = 0; i < n; i += RIF) {
             float x[RIF][KK];
             sfor<0, RIF>([&](auto q) {
@@ -289,7 +292,7 @@ template <int G> struct Worker {
                 const bool ok = idx < n;
                 const int v = idx < n1 ? va + idx : vc + (idx - n1);
                 const float *p = base + (long long)v * (NU * 32);
-                sfor<0, KK>([&](auto kk) { x[V(q)][V(kk)] = ok ? ldrow(p + col(V(kk)) * 32) : 0.f; });
+                sfor<0, KK>([&](auto kk) { x[V(q)][V(kk)] = ok ? ldrow(p + col(V(kk)) * 32) - cm[V(kk)] : 0.f; });
             });
             sfor<0, KK>([&](auto kk) {
                 float t[RIF];
@@ -310,7 +313,7 @@ template <int G> struct Worker {
         sfor<0, KK>([&](auto kk) {
             float a0 = 0.f, a1 = 0.f;
             sfor<0, TT>([&](auto tt) {
-                if constexpr ((V(tt) & 1) == 0) a0 += cur[V(kk) * TT + V(tt)]; else a1 += cur[V(kk) * TT + V(tt)];
+                if constexpr ((V(tt) & 1) == 0) a0 += cur[V(kk) * TT + V(tt)] - mu[V(kk)]; else a1 += cur[V(kk) * TT + V(tt)] - mu[V(kk)];
             });
             acc[V(kk)] = a0 + a1;
         });
@@ -323,14 +326,13 @@ template <int G> struct Worker {
         if (top >= v_lo) {
             const int bfirst = (v_lo + 7) >> 3, blast = ((top + 1) >> 3) - 1;
             if (blast >= bfirst) {
-                sum_rows(dv0, 8 * (blast + 1), top, v_lo, 8 * bfirst - 1, acc); // the ragged rows at both ends, in one go
-                sum_rows(dq0, bfirst, blast, 0, -1, acc);
+                sum_rows(dv0, 8 * (blast + 1), top, v_lo, 8 * bfirst - 1, 1.f, acc); // the ragged rows at both ends, in one go
+                sum_rows(dq0, bfirst, blast, 0, -1, 8.f, acc);
             } else {
-                sum_rows(dv0, v_lo, top, 0, -1, acc);
+                sum_rows(dv0, v_lo, top, 0, -1, 1.f, acc);
             }
         }
-        const float fn = (float)(rb_end - rb0);
-        sfor<0, KK>([&](auto kk) { Q[V(kk)] += fmaf(-fn, mu[V(kk)], acc[V(kk)]); });
+        sfor<0, KK>([&](auto kk) { Q[V(kk)] += acc[V(kk)]; });
     }
 #elif LIGHT && DHIST
     // ---- plain runs (no end stored, no start range met): only the suffix sums move, one history value per (trial, step)
@@ -886,24 +888,46 @@ __device__ __forceinline__ void stats_history(const float *dcol, int slot, int c
     for (; i > 0; --i, p += NU * 32) { const double D = (double)p[0]; a1 += D; a2 = fma(D, D, a2); }
 }
 #endif
-// sum (D - centre)^2 over the same samples: the second pass of an exact two-pass variance
-template <int U> __device__ __forceinline__ double stats_centred(const float *rp, int cnt, double centre)
+// The rare paths (rebuild after a marked series, two-pass variance) over the whole valid set of trial u, with the shifts read
+// from the table at run time: like everything in stats_trial but the loop over the entering samples, ONE copy of the code
+// serves all trials (the eight trials of a CTA share the instruction cache).  Same expression and order as stats_range, so
+// the same floats.
+// centred = false: a1 += sum D, a2 += sum D^2;  centred = true: a2 += sum (D - centre)^2
+__device__ __forceinline__ void stats_whole(int u, const float *rp, int cnt, bool centred, double centre, double &a1, double &a2)
 {
-    double c2 = 0.0;
+    int off[NCHAN];
+    sfor<0, NCHAN>([&](auto c) { off[V(c)] = ((int)D_TAB[u][V(c)] * NCHAN + V(c)) * 32; });
     for (int i = cnt; i > 0; --i, rp += NCHAN * 32) {
         float e[4] = {0.f, 0.f, 0.f, 0.f};
-        sfor<0, NCHAN>([&](auto c) { e[V(c) & 3] += __ldg(rp + (D_TAB[U][V(c)] * NCHAN + V(c)) * 32); });
-        const double x = (double)((e[0] + e[1]) + (e[2] + e[3])) - centre;
-        c2 = fma(x, x, c2);
+        sfor<0, NCHAN>([&](auto c) { e[V(c) & 3] += __ldg(rp + off[V(c)]); });
+        const double D = (double)((e[0] + e[1]) + (e[2] + e[3]));
+        if (centred) {
+            const double x = D - centre;
+            a2 = fma(x, x, a2);
+        } else {
+            a1 += D;
+            a2 = fma(D, D, a2);
+        }
     }
-    return c2;
 }
 
-template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &P, int lane, int pix, bool live)
+// the entering (or, without the history, leaving) samples of trial u: the only part compiled per trial (immediate shifts)
+template <int U0, int N>
+__device__ __forceinline__ void stats_range_of(int u, const float *rp, int cnt, double &a1, double &a2, float *dcol = nullptr, int slot = 0)
+{
+    if constexpr (N == 1) {
+        stats_range<U0>(rp, cnt, a1, a2, dcol, slot);
+    } else {
+        if (u < U0 + N / 2) stats_range_of<U0, N / 2>(u, rp, cnt, a1, a2, dcol, slot);
+        else stats_range_of<U0 + N / 2, N - N / 2>(u, rp, cnt, a1, a2, dcol, slot);
+    }
+}
+
+__device__ __forceinline__ void stats_trial(const StatsParams &P, int U, int lane, int pix, bool live)
 {
     // P.add: 0 = take out the samples that leave V_u, 1 = put in the ones that enter and publish, 2 = both (DHIST: the leaving
     // samples are read from the history, so nothing has to run before the ring update)
-    constexpr long long dm = DMAX_TAB[U];
+    const long long dm = DMAX_TAB[U];
     const bool do_rm = P.add != 1, do_add = P.add != 0;
     const long long b_prev = P.lo_prev > P.n_prev - dm ? P.lo_prev : P.n_prev - dm; // end of the previous valid set
     const long long la = P.lo_prev, lb = P.lo < b_prev ? P.lo : b_prev;             // leaving:  [la, lb)
@@ -921,7 +945,7 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
 #if DHIST
         stats_history(dcol, (int)((la + dm) % LRING), (int)(lb - la), a1, a2);
 #else
-        stats_range<U>(rbase + (la - P.ring_lo) * (NCHAN * 32), (int)(lb - la), a1, a2);
+        stats_range_of<0, NU>(U, rbase + (la - P.ring_lo) * (NCHAN * 32), (int)(lb - la), a1, a2);
 #endif
         // A leaving sample that dwarfs what stays behind (|D| beyond ~10^3 sigma sqrt(T)) has eaten the low bits of S2 when it
         // entered, and a non-finite one has destroyed the sums: mark the series (NaN); the add pass rebuilds it from the ring.
@@ -935,7 +959,7 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
     double a1 = 0.0, a2 = 0.0;
 #if DHIST
     if (tb > ta) {
-        stats_range<U>(rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2, dcol, (int)((ta + dm) % LRING));
+        stats_range_of<0, NU>(U, rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2, dcol, (int)((ta + dm) % LRING));
 #if COARSE
         { // the aligned rows [ra, rz) have just been written: every block whose last row is among them is complete
             const long long ra = ta + dm, rz = tb + dm;
@@ -953,7 +977,7 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
 #endif
     }
 #else
-    stats_range<U>(rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2);
+    stats_range_of<0, NU>(U, rbase + (ta - P.ring_lo) * (NCHAN * 32), (int)(tb - ta), a1, a2);
 #endif
     const long long Tk = tb - P.lo; // tb = max(lo, n - dmax_u)
     bool rebuild = false;
@@ -964,7 +988,7 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
     }
     if (__any_sync(0xffffffffu, rebuild)) { // warp = one trial, lanes = pixels: the whole valid set once more (rare)
         double b1 = 0.0, b2 = 0.0;
-        stats_range<U>(rbase + (P.lo - P.ring_lo) * (NCHAN * 32), (int)Tk, b1, b2);
+        stats_whole(U, rbase + (P.lo - P.ring_lo) * (NCHAN * 32), (int)Tk, false, 0.0, b1, b2);
         if (rebuild) { a1 = b1; a2 = b2; }
     }
     float m = 0.f, dl = 0.f, rs = 0.f, sg = __int_as_float(0x7fc00000); // NaN sigma = "no valid sample yet"
@@ -977,7 +1001,8 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
         cancel = msq > 0.0 && !(var >= 1e-8 * msq); // over half of float64's digits cancelled: |mean| > 10^4 sigma
     }
     if (__any_sync(0xffffffffu, cancel)) { // exact two-pass variance about the mean (reading R31)
-        const double c2 = stats_centred<U>(rbase + (P.lo - P.ring_lo) * (NCHAN * 32), (int)Tk, mean);
+        double c1 = 0.0, c2 = 0.0;
+        stats_whole(U, rbase + (P.lo - P.ring_lo) * (NCHAN * 32), (int)Tk, true, mean, c1, c2);
         if (cancel) var = c2 / (double)Tk;
     }
     if (live) {
@@ -999,16 +1024,6 @@ template <int U> __device__ __forceinline__ void stats_trial(const StatsParams &
     if (P.sig_out) P.sig_out[o] = sg;
 }
 
-template <int U0, int N> __device__ __forceinline__ void stats_dispatch(int u, const StatsParams &P, int lane, int pix, bool live)
-{
-    if constexpr (N == 1) {
-        stats_trial<U0>(P, lane, pix, live);
-    } else {
-        if (u < U0 + N / 2) stats_dispatch<U0, N / 2>(u, P, lane, pix, live);
-        else stats_dispatch<U0 + N / 2, N - N / 2>(u, P, lane, pix, live);
-    }
-}
-
 } // namespace sk
 
 extern "C" __global__ void __launch_bounds__(256) k_stream_stats(const StatsParams P)
@@ -1019,7 +1034,7 @@ extern "C" __global__ void __launch_bounds__(256) k_stream_stats(const StatsPara
     int pix = blockIdx.x * 32 + lane;
     const bool live = pix < NPIX;
     if (!live) pix = NPIX - 1;
-    sk::stats_dispatch<0, NU>(u, P, lane, pix, live);
+    sk::stats_trial(P, u, lane, pix, live);
 }
 #endif
 
