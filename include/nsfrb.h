@@ -84,7 +84,9 @@ typedef struct {
  * All host arrays are copied.  Device memory is allocated on the CUDA device current at creation: small tables at creation;
  * at nsfrb_plan_prepare or the first nsfrb_search two pixel-batch workspaces of about 1 GiB each (the search walks the image
  * in batches: no cube-sized buffer) plus ~2 MB of scratch per SM; at nsfrb_plan_prepare or the first nsfrb_stream_push the
- * ring, 2*(nt + guard)*nchan*npix*4 B, plus a workspace of ~10 B per (pixel, trial, width).  Plans with more than 32 usable
+ * ring, 2*(nt + guard)*nchan*npix*4 B, the ring of dedispersed samples, 2.25*(nt + guard)*ndm_unique*npix*4 B (left out where
+ * it would take more than half of the free device memory: nsfrb_stream_mode), plus a workspace of ~10 B per (pixel, trial,
+ * width).  Plans with more than 32 usable
  * widths use a generic kernel with a cube-sized workspace (nchan*nt*npix*4 B).
  */
 int nsfrb_plan_create(nsfrb_plan **out, int nx, int ny, int nchan, int nt,
@@ -135,9 +137,11 @@ int nsfrb_search(nsfrb_plan *plan, const float *cube, void *stream,
  * The sums behind mu_k and sigma_k (sum of D_k and of D_k^2 over the valid samples, float64 per trial and pixel) are
  * plan state carried from push to push: a push adds the samples that enter the valid set and subtracts those that
  * leave it; nsfrb_stream_reset clears them together with the ring.  The memory they take (24 B per trial and pixel) is
- * counted in nsfrb_plan_info's workspace_bytes.
+ * counted in nsfrb_plan_info's workspace_bytes.  So is the dedispersed sample D_k(t) itself: it is formed once, by the push
+ * that brings its last raw sample, and kept in a second ring that later pushes read (nsfrb_stream_mode 2 and 3; DESIGN.md
+ * 5.2) -- state with the lifetime of the raw ring, holding nothing the raw ring does not determine.
  * The first push of a plan compiles the plan-specialised kernel with NVRTC (seconds to a minute, growing with
- * ndm*nchan) and allocates the ring (2*(nt + guard)*nchan*npix*4 B); a compile failure returns NSFRB_ECUDA with
+ * ndm*nchan) and allocates the rings (see nsfrb_plan_create); a compile failure returns NSFRB_ECUDA with
  * the compiler log.  Compiled kernels are cached on disk (NSFRB_JIT_CACHE=<dir>, default /tmp/nsfrb_jit_cache_<uid>, private to the user;
  * NSFRB_JIT_CACHE=0 disables).  nsfrb_plan_prepare(plan, NSFRB_PREPARE_STREAM, chunk_nt) does both ahead of time.  A chunk longer
  * than any before it recompiles the kernel for that length (a stream synchronisation; prepare with the longest chunk to avoid it).
