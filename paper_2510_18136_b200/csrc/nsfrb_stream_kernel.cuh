@@ -879,13 +879,11 @@ template <int U> __device__ __forceinline__ void stats_range(const float *rp, in
 __device__ __forceinline__ void stats_history(const float *dcol, int slot, int cnt, double &a1, double &a2)
 {
     const float *p = dcol + (long long)slot * (NU * 32); // slot < LRING, cnt <= LRING: the double mapping covers the run
-    int i = cnt;
-    for (; i >= 4; i -= 4, p += 4 * NU * 32) {
-        float d[4];
-        sfor<0, 4>([&](auto q) { d[V(q)] = p[V(q) * NU * 32]; }); // (plain loads: the fused launch stores to these rows afterwards)
-        sfor<0, 4>([&](auto q) { const double D = (double)d[V(q)]; a1 += D; a2 = fma(D, D, a2); });
+    for (int i0 = 0; i0 < cnt; i0 += 32, p += 32 * NU * 32) { // one round trip per 32 samples (a push of 25: one)
+        float d[32];
+        sfor<0, 32>([&](auto q) { d[V(q)] = i0 + V(q) < cnt ? p[V(q) * NU * 32] : 0.f; }); // (plain loads: the fused launch stores to these rows afterwards)
+        sfor<0, 32>([&](auto q) { const double D = (double)d[V(q)]; a1 += D; a2 = fma(D, D, a2); }); // (a padding zero adds nothing)
     }
-    for (; i > 0; --i, p += NU * 32) { const double D = (double)p[0]; a1 += D; a2 = fma(D, D, a2); }
 }
 #endif
 // The rare paths (rebuild after a marked series, two-pass variance) over the whole valid set of trial u, with the shifts read
@@ -964,14 +962,23 @@ __device__ __forceinline__ void stats_trial(const StatsParams &P, int U, int lan
         { // the aligned rows [ra, rz) have just been written: every block whose last row is among them is complete
             const long long ra = ta + dm, rz = tb + dm;
             float *dcol8 = P.dh8 + (long long)blockIdx.x * (2 * LRING / 8) * (NU * 32) + U * 32 + lane;
-            for (long long b = ra >> 3; b <= ((rz - 8) >> 3); ++b) {
-                const int s8 = (int)((8 * b) % LRING); // slot of the block's first row (LRING % 8 == 0: the block does not wrap)
-                const float *r8 = dcol + (long long)s8 * (NU * 32);
-                float d[8];
-                sfor<0, 8>([&](auto q) { d[V(q)] = r8[V(q) * NU * 32]; }); // (plain loads: some of these rows were stored above)
-                const float E = ((d[0] + d[1]) + (d[2] + d[3])) + ((d[4] + d[5]) + (d[6] + d[7]));
-                dcol8[(long long)(s8 >> 3) * (NU * 32)] = E;
-                dcol8[(long long)((s8 >> 3) + LRING / 8) * (NU * 32)] = E;
+            const long long b_hi = (rz - 8) >> 3;
+            for (long long b0 = ra >> 3; b0 <= b_hi; b0 += 4) { // four blocks per round trip (a push of 25 samples completes 3 or 4)
+                float d[4][8];
+                int s8[4];
+                sfor<0, 4>([&](auto j) {
+                    const bool ok = b0 + V(j) <= b_hi;
+                    s8[V(j)] = (int)((8 * (b0 + V(j))) % LRING); // slot of the block's first row (LRING % 8 == 0: the block does not wrap)
+                    const float *r8 = dcol + (long long)s8[V(j)] * (NU * 32);
+                    sfor<0, 8>([&](auto q) { d[V(j)][V(q)] = ok ? r8[V(q) * NU * 32] : 0.f; }); // (plain loads: some of these rows were stored above)
+                });
+                sfor<0, 4>([&](auto j) {
+                    if (b0 + V(j) <= b_hi) {
+                        const float E = ((d[V(j)][0] + d[V(j)][1]) + (d[V(j)][2] + d[V(j)][3])) + ((d[V(j)][4] + d[V(j)][5]) + (d[V(j)][6] + d[V(j)][7]));
+                        dcol8[(long long)(s8[V(j)] >> 3) * (NU * 32)] = E;
+                        dcol8[(long long)((s8[V(j)] >> 3) + LRING / 8) * (NU * 32)] = E;
+                    }
+                });
             }
         }
 #endif
