@@ -118,10 +118,12 @@ bool search4_geo(const nsfrb_plan *pl, Geo &g)
     g.prune = env_int("NSFRB_SEARCH_PRUNE", 1) != 0;
     g.dpitch = round_up(pl->nt, 512);
     // pixels per work item: the item's barriers are shared by them and the tail keeps one warp per pixel busy.  The scratch
-    // (pxi x nwarp series per CTA) is about 2 MB per CTA (measured best on C3-C5: 8 / 16 / 4 pixels; it then cycles through
-    // L2 and HBM, one block ahead of the search)
+    // (pxi x nwarp series per CTA) is kept to about 0.6 MB per CTA, so that the scratch of all 148 CTAs (~90 MB) stays in the
+    // 126 MB L2 between sweep A, which writes it, and sweep B, which reads it three times: 2 / 12 / 1 pixels on C3 / C4 / C5
+    // (measured: 2 MB per CTA, which cycles through HBM, costs +3 % / +1 % / +13 %; profiles/r02.md)
     const size_t series = (size_t)g.nwarp * g.dpitch * sizeof(float);
-    g.pxi = (int)std::max<size_t>(1, std::min<size_t>(16, (2048u << 10) / series));
+    g.pxi = (int)std::max<size_t>(1, std::min<size_t>(16, (640u << 10) / series));
+    if (g.pxi >= 4) g.pxi &= ~3; // (whole groups of four: the tail hands a pixel to each of four warp quads)
     if (env_int("NSFRB_SEARCH_PXI", 0) > 0) g.pxi = std::min(16, env_int("NSFRB_SEARCH_PXI", 0));
     g.pxi = std::min(g.pxi, g.nwarp);
     // ring: wmax + one block + the rows the bounds read, a multiple of 64; a power of two (every wrap one AND) when shared
