@@ -1,44 +1,46 @@
-// k_stream: the hot kernel of nsfrb_stream_push (steps a1..a6 of DESIGN.md) for sm_100a.
+// k_stream and k_stream_stats: the kernels of nsfrb_stream_push (steps a1..a6 of DESIGN.md 5.2) for sm_100a.
 //
 // This file is compiled AT PLAN TIME (NVRTC, sm_100a) behind a generated prologue that fixes the
-// plan's constants -- NPIX, NCHAN, the delay table, the width list, the tile shape -- so every
-// dedispersion shift is an immediate and every register array is statically indexed (PAPER.md:L75:
-// "shift indices for each frequency channel [are] pre-computed and loaded onto the GPU to minimize
-// latencies"; here they are compiled into the instruction stream).  `build()` also compiles it
-// ahead of time with the BASELINE config-2 prologue as a build check.
+// plan's constants -- NPIX, NCHAN, the delay table, the width list, the ring length, the tile shape --
+// so every dedispersion shift is an immediate and every register array is statically indexed
+// ("shift indices for each frequency channel [are] pre-computed and loaded onto the GPU
+// to minimize latencies"; here they are compiled into the instruction stream).  `build()` also compiles
+// it ahead of time with the BASELINE config-2 prologue as a build check.
 //
-// Prologue (see nsfrb_jit.cu: make_stream_prologue):
-//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD INCR LIGHT NW_ALL CUBES   integers (INCR, LIGHT: see StreamParams and Worker::light; NW_ALL: length of the caller's width list; CUBES = 1 compiles the cube outputs in)
+// Prologue (nsfrb_stream.cu: make_prologue):
+//   NPIX NCHAN NU KK GPC SEG TT NW CMAX NSUPER MINB ROWS PFD INCR LIGHT NW_ALL CUBES DHIST COARSE LRING GUARD   integers
+//     (INCR: statistics kept by k_stream_stats; LIGHT: plain runs take a shortcut; DHIST: the march reads the ring of
+//      dedispersed samples; COARSE: and its 8-row block sums; LRING, GUARD: ring length and guard rows; NW_ALL: length of the
+//      caller's width list; CUBES = 1 compiles the cube outputs in)
 //   D_TAB[NU][NCHAN]   integer delays d[u][c] of the unique trials, DM ascending
 //   DMAX_TAB[NU]       dmax_u                 K_OF_U[NU]  lowest original dm index of the trial
 //   W_TAB[NW]          widths, ascending      J_OF_W[NW]  original width index   RSQ_W[NW]  1/sqrt(width)
 //
-// Reverse frame.  The ring holds raw samples rho in [0, len); s = len-1-rho counts back from the
-// newest one.  Series u has T_u = len - dmax_u samples; its r-th sample from the end (r = 1..T_u) is
-//     D_u(r) = sum_c R[c][s = (r-1) + dmax_u - d[u][c]]
-// i.e. a dedispersion in reversed time.  The KK trials of a thread march together in the GROUP frame
-// rg = r - delta_u, delta_u = DMAXG - dmax_u (DMAXG = the group's largest dmax): there trial u reads
-// s = (rg-1) + e[u][c], e[u][c] = DMAXG - d[u][c], so consecutive trials differ only in the channels
-// whose delay differs (differential dedispersion keeps working), every trial of the group ends at the
-// same group step len - DMAXG, and the delta_u newest samples of trial u are covered by a masked lead-in.
-// With Q_u(r) = sum_{r'<=r} (D_u(r') - mu0_u) (suffix sums of the series), the boxcar of width w whose
-// window excludes the newest i samples is B(i, w) = Q(i+w) - Q(i); rule S5 (only windows whose last
-// raw sample arrived in this push) keeps exactly i in [0, chunk_nt) for every trial.  One backward
-// march therefore needs, per (pixel, trial): Q (register), Q at the C ends (shared memory, Qe) and
-// the running max per width (M: one width at a time in registers, the rest in an L2-resident
-// workspace -- wide widths have disjoint start ranges) -- no prefix history, no P ring.
+// Reverse frame (all modes).  Series u has T_u = len - dmax_u samples; count them back from the newest one, r = 1..T_u.
+// With Q_u(r) = sum_{r'<=r} (D_u(r') - mu0_u) (suffix sums of the series), the boxcar of width w whose window
+// excludes the newest i samples is B(i, w) = Q(i+w) - Q(i); rule S5 (only windows whose last raw sample arrived
+// in this push) keeps exactly i in [0, chunk_nt) for every trial.  One backward march therefore needs, per
+// (pixel, trial): Q (register), Q at the C ends (shared memory, Qe) and the running max per width (M: one width
+// at a time in registers, the rest in an L2-resident workspace -- wide widths have disjoint start ranges) -- no
+// prefix history, no P ring.  Lane = pixel; thread = 1 pixel x KK consecutive trials x 1 of SEG time segments; a
+// tile is TT steps; tiles that touch a width's start range also evaluate its cells (a5).  End of march:
+// S = (M + Off - w delta)/(sigma sqrt(w)), reduced over widths, trials and DM groups of the CTA (a6).
 //
-// Mapping.  Lane = pixel.  The ring is stored per block of 32 pixels, [block][row][chan][32]: every load is
-// one coalesced 128-byte segment and a warp streams through one contiguous region (a tile's new rows are
-// TT*NCHAN*128 contiguous bytes), which is what HBM row buffers and the TLB want.  Thread = 1 pixel x KK consecutive trials x 1 of SEG time segments.  A tile is TT steps:
-// the thread holds the raw window of every channel in registers (TT new rows + a carried halo of
-// span_c = max_kk e - min_kk e rows), forms D for its first trial as the plain channel sum and every
-// next trial differentially (a2), then x = D - mu0, Q += x, S2 += x^2 (a1, a3, a4).  Tiles that touch
-// a width's start range also evaluate its cells (a5).  Segments are cut between start ranges, so a
-// width belongs to one segment and its maxima are relative to that segment's offset, added at the end.
-// End of march: delta = S1/T, var = S2/T - delta^2, S = (M + Off - w delta)/(sigma sqrt(w)), reduced over
-// widths, trials and DM groups of the CTA (a6).  The rows of tile n+1 are requested as soon as tile n's
-// dedispersion has consumed its rows (same registers), PFD tiles further ahead they are prefetched to L2.
+// DHIST = 1 (the default): k_stream_stats dedisperses every sample ONCE, when it enters the valid set, and stores
+// D_u(t) in dh[pixel block][row][trial][32] at the row of raw sample t + dmax_u -- so the r-th sample from the end of
+// EVERY series sits in row top - (r - 1) and all trials march in step, each in its own frame.  k_stream reads one
+// float per (trial, step), KK*TT values one tile ahead; in the plain runs between start ranges it adds whole 8-row
+// blocks from dh8 (COARSE) and the ragged rows at the two ends.  Nothing but the trial column depends on the DM
+// group: ONE instance of the march serves all groups (the instruction supply was the limit with one per group).
+//
+// DHIST = 0 (raw-ring march): the ring holds raw samples, D_u(r) = sum_c R[c][(r-1) + dmax_u - d[u][c]].  The KK
+// trials of a thread march together in the GROUP frame rg = r - delta_u, delta_u = DMAXG - dmax_u: there trial u
+// reads s = (rg-1) + e[u][c], e[u][c] = DMAXG - d[u][c], so consecutive trials differ only in the channels whose
+// delay differs (differential dedispersion), every trial of the group ends at the same group step, and the delta_u
+// newest samples of trial u are covered by a masked lead-in.  The ring is [block][row][chan][32]: every load is one
+// coalesced 128-byte segment; the thread holds the raw window of every channel in registers (TT new rows + a
+// carried halo of span_c rows), forms D for its first trial as the plain channel sum and every next trial
+// differentially (a2).  One template instance per DM group.
 #ifndef NSFRB_STREAM_KERNEL_CUH
 #define NSFRB_STREAM_KERNEL_CUH
 
