@@ -769,11 +769,13 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
     StatsParams tp;
     tp.ring = ss->ring; tp.s1 = ss->st1; tp.s2 = ss->st2; tp.mu = ss->mu0; tp.dlt = ss->dlt; tp.rsig = ss->rsig; tp.sig_out = nullptr;
     tp.dh = ss->dhist; tp.dh8 = ss->dh8; tp.pad = 0; tp.lo_prev = lo_prev; tp.n_prev = n_prev; tp.lo = lo; tp.n = n;
-    const dim3 stat_grid((pl->npix + 31) / 32, (pl->nuniq + 7) / 8);
+    int stat_warps = 8; // trials (warps) per CTA of k_stream_stats
+    if (const char *e = getenv("NSFRB_STREAM_STATS_WARPS")) stat_warps = std::max(1, std::min(8, atoi(e)));
+    const dim3 stat_grid((pl->npix + 31) / 32, (pl->nuniq + stat_warps - 1) / stat_warps), stat_block(32 * stat_warps);
     if (c.INCR && !c.DHIST && lo > lo_prev && n_prev > 0) { // (DHIST: the leaving samples come from the history, in the launch below)
         tp.row_lo = ss->guard + (int)(lo_prev % L); tp.ring_lo = lo_prev; tp.add = 0; tp.first = 0;
         void *args[] = {&tp};
-        SCU(cudaLaunchKernel((const void *)ss->fn_stats[variant], stat_grid, dim3(256), args, 0, st), "k_stream_stats launch");
+        SCU(cudaLaunchKernel((const void *)ss->fn_stats[variant], stat_grid, stat_block, args, 0, st), "k_stream_stats launch");
         ++*launches;
     }
     // ---- a8: ring update
@@ -803,7 +805,7 @@ int stream_push(nsfrb_plan *pl, const float *chunk, int chunk_nt, cudaStream_t s
         tp.row_lo = ss->guard + (int)(lo % L); tp.ring_lo = lo; tp.add = c.DHIST ? 2 : 1; tp.first = n_prev == 0 ? 1 : 0;
         tp.sig_out = running ? ss->sig : nullptr;
         void *args[] = {&tp};
-        SCU(cudaLaunchKernel((const void *)ss->fn_stats[variant], stat_grid, dim3(256), args, 0, st), "k_stream_stats launch");
+        SCU(cudaLaunchKernel((const void *)ss->fn_stats[variant], stat_grid, stat_block, args, 0, st), "k_stream_stats launch");
         ++*launches;
     }
     if (pl->profiling && pl->ev[1]) cudaEventRecord(pl->ev[1], st);

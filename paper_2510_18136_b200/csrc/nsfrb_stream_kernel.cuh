@@ -1038,7 +1038,7 @@ __device__ __forceinline__ void stats_trial(const StatsParams &P, int U, int lan
 extern "C" __global__ void __launch_bounds__(256) k_stream_stats(const StatsParams P)
 {
     const int lane = threadIdx.x & 31;
-    const int u = blockIdx.y * 8 + (threadIdx.x >> 5);
+    const int u = blockIdx.y * (blockDim.x >> 5) + (threadIdx.x >> 5); // warp = trial; the warps of a CTA share the raw rows in L1
     if (u >= NU) return;
     int pix = blockIdx.x * 32 + lane;
     const bool live = pix < NPIX;
