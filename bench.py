@@ -739,7 +739,7 @@ def stream_read_bytes(wl, info, mode):
     steps = min(wl.nt, int(info["wmax"]) + C)
     if mode <= 1:
         return steps * wl.nchan * wl.npix * 4, "raw rows up to the widest window, every channel"
-    tt = 4
+    tt = 6
     cell = [False] * (steps + tt + 1)
     for w in sorted(set(int(x) for x in wl.width_list)):
         for r in range(max(0, w // tt * tt), min(steps, (w + C - 1) // tt * tt + tt)):

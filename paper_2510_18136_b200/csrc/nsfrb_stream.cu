@@ -111,8 +111,8 @@ bool choose_cfg(const nsfrb_plan *pl, int chunk_nt, const char *variant, StreamC
     if (c.DHIST) {
         // a thread holds KK*TT history values and no raw rows, the trials of a thread share nothing and every DM group runs the
         // same instance of the code: fewer trials per thread and more warps per CTA (the shared-memory Qe block of a CTA is per
-        // trial either way) -- 4 trials x 4 groups measured best on C2 (profiles/r02.md)
-        kk = 4; gpc = 4; seg = 1; tt = 4; minb = 4; pfd = 2;
+        // trial either way) -- 4 trials x 4 groups, six steps per tile (128 registers) measured best on C2 (profiles/r02.md)
+        kk = 4; gpc = 4; seg = 1; tt = 6; minb = 4; pfd = 2;
     } else if (pl->nchan > 24) { // the thread holds nchan*TT raw rows in registers: one time step per tile, more registers
         tt = 1;
         minb = 2;

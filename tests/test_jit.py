@@ -34,11 +34,11 @@ def test_duplicate_trials_and_unused_widths_are_dropped_from_the_kernel():
 
 def test_default_shape_and_modes_are_in_the_prologue(monkeypatch):
     """Default: incremental statistics + dedispersed history with 8-row block sums, 4 trials x 4 groups per CTA, one time segment,
-    four steps per tile.  NSFRB_STREAM_DHIST=0 gives the raw-ring march (light tiles, three steps per tile),
+    six steps per tile.  NSFRB_STREAM_DHIST=0 gives the raw-ring march (light tiles, three steps per tile),
     NSFRB_STREAM_STATS=march the whole-ring march with the v4 shape; the raw march above 24 channels takes one step per tile."""
     wl = W.config("c2")
     src = nsfrb.jit_stream_kernel(*_args(wl), 25).decode()
-    for d in ("#define INCR 1", "#define LIGHT 1", "#define DHIST 1", "#define COARSE 1", "#define SEG 1", "#define TT 4", "#define KK 4",
+    for d in ("#define INCR 1", "#define LIGHT 1", "#define DHIST 1", "#define COARSE 1", "#define SEG 1", "#define TT 6", "#define KK 4",
               "#define GPC 4", "#define PFD 2", "#define LRING 1536"):
         assert d in src, d
     assert "k_stream_stats" in src
