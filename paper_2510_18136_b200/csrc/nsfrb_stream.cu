@@ -83,7 +83,8 @@ size_t cfg_smem(const StreamCfg &c)
     const size_t trials = (size_t)c.GPC * c.KK;
     const size_t qe = trials * c.CMAX * 32, sg = trials * c.SEG * 32, red = (size_t)c.GPC * 32 * 4;
     (void)sg;
-    return (qe + red + (size_t)c.GPC * c.SEG * 2) * 4;
+    const size_t qpad = c.DHIST ? (size_t)c.TT * 32 : 0; // padding rows before and after Qe (nsfrb_stream_kernel.cuh: QPAD)
+    return (qe + 2 * qpad + red + (size_t)c.GPC * c.SEG * 2) * 4;
 }
 
 // Tile shape for a plan: KK trials per thread, GPC groups x SEG segments of warps per CTA.

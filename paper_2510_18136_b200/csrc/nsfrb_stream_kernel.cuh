@@ -158,10 +158,11 @@ constexpr int kTrialsPerCta = GPC * KK;
 // the range of widths that segment evaluated.  Segment totals S1, S2 [kTrialsPerCta][SEG][32] go through
 // the global workspace sws (written once per thread).
 constexpr int kQeFloats = kTrialsPerCta * CMAX * 32;
+constexpr int QPAD = DHIST ? TT * 32 : 0; // floats of padding before and after Qe (the branch-free partial tiles read up to TT - 1 rows outside)
 constexpr int kSegFloats = kTrialsPerCta * SEG * 32;
 constexpr int kRedFloats = GPC * 32 * 4;
 constexpr int kRangeInts = GPC * SEG * 2;
-constexpr int kSmemBytes = (kQeFloats + kRedFloats + kRangeInts) * 4;
+constexpr int kSmemBytes = (kQeFloats + 2 * QPAD + kRedFloats + kRangeInts) * 4;
 
 __device__ __forceinline__ float ldrow(const float *p) { return __ldg(p); }
 
@@ -191,6 +192,8 @@ template <int G> struct Worker {
     float carry[DHIST ? 1 : T::CARRY];
     float mu[KK], dmu[KK], Q[KK], S2[KK]; // mu: provisional means (mu[0] and the differences dmu are live in the loop)
     int ja, jb; // widths [ja, jb) can have cells in the current tile
+    const int *wt; // W_TAB in shared memory: a __device__ table indexed at run time is a global load, and these lookups sit on
+                   // the critical path of every tile
     // register cache of one width's running maxima (the rest live in mws/aws)
     int jc, jfirst, jseen;
     float mc[KK];
@@ -481,12 +484,12 @@ template <int G> struct Worker {
         }
         if (cells) {
             // a5: widths whose start range [w+i0, w+i0+C-1] (own frame) meets this tile
-            while (ja < NW && W_TAB[ja] + i0 + C - 1 < rb + 1) ++ja;
+            while (ja < NW && wt[ja] + i0 + C - 1 < rb + 1) ++ja;
             if (jb < ja) jb = ja;
-            while (jb < NW && W_TAB[jb] + i0 <= rb + TT + T::dspread()) ++jb;
+            while (jb < NW && wt[jb] + i0 <= rb + TT + T::dspread()) ++jb;
             for (int j = ja; j < jb; ++j) {
                 if (j != jc) fetch(j);
-                const int ib = rb + 1 - W_TAB[j] - i0; // end index (relative to i0) of group step rb+1 at delta = 0
+                const int ib = rb + 1 - wt[j] - i0; // end index (relative to i0) of group step rb+1 at delta = 0
                 const float *qb = qe + ib * 32;        // &Qe[0][ib]: every access below is a static offset from it
                 const bool inside = !MASKED && ib >= 0 && ib + TT - 1 + T::dspread() < C;
                 if (inside) { // every cell of the tile is defined: no range checks
@@ -507,10 +510,18 @@ template <int G> struct Worker {
                                     const int ro = rb + 1 + V(tt) + T::delta(V(kk));
                                     in = in && ro >= 1 && ro <= len - DMAX_TAB[uof(V(kk))];
                                 }
+#if DHIST
+                                // branch-free: an end outside [0, C) reads a neighbouring row of Qe (or its padding, QPAD rows on
+                                // either side) and is replaced by -inf, which never beats a defined cell
+                                const float d = Dv[V(kk)][V(tt)] - qb[(V(kk) * CMAX + V(tt)) * 32];
+                                const float v = in ? d : -kInf;
+                                if (v >= mc[V(kk)]) { mc[V(kk)] = v; ac[V(kk)] = ii; } // later step = earlier start
+#else
                                 if (in) {
                                     const float v = Dv[V(kk)][V(tt)] - qb[(V(kk) * CMAX + V(tt) + T::delta(V(kk))) * 32];
                                     if (v >= mc[V(kk)]) { mc[V(kk)] = v; ac[V(kk)] = ii; } // later step = earlier start
                                 }
+#endif
                             });
                     });
                 }
@@ -533,16 +544,17 @@ __device__ __forceinline__ bool better(float s, int k, int j, int t, float bs, i
 }
 
 template <int G>
-__device__ __forceinline__ void run_group(const StreamParams &P, float *smem, int gl, int seg, int lane, int pix, bool live, int u0 = 0)
+__device__ __forceinline__ void run_group(const StreamParams &P, float *smem, const int *wtab, int gl, int seg, int lane, int pix, bool live, int u0 = 0)
 {
     using T = GT<G>;
-    float *Qe = smem;
-    float *red = Qe + kQeFloats;
+    float *Qe = smem + QPAD;
+    float *red = Qe + kQeFloats + QPAD;
     float *S1s = P.sws + ((long long)blockIdx.x * NSUPER + blockIdx.y) * 2 * kSegFloats;
     float *S2s = S1s + kSegFloats;
     int *rng = reinterpret_cast<int *>(red + kRedFloats);
 
     Worker<G> w;
+    w.wt = wtab;
 #if DHIST
     w.u0 = u0;
 #endif
@@ -606,9 +618,9 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
                 cells = rb < qe_end;
                 if (!cells) {
                     int ja = w.ja;
-                    while (ja < NW && W_TAB[ja] + P.i0 + P.C - 1 < rb + 1) ++ja;
+                    while (ja < NW && w.wt[ja] + P.i0 + P.C - 1 < rb + 1) ++ja;
                     w.ja = ja;
-                    const int wnext = ja < NW ? W_TAB[ja] + P.i0 - T::dspread() : 0x3fffffff; // first step of the next start range
+                    const int wnext = ja < NW ? w.wt[ja] + P.i0 - T::dspread() : 0x3fffffff; // first step of the next start range
                     cells = wnext <= rb + TT;
                     if (!cells) { // a plain run begins: nothing stays cached across it
                         plain_until = wnext - TT; // rb < plain_until  <=>  rb + TT < wnext
@@ -788,13 +800,13 @@ __device__ __forceinline__ void run_group(const StreamParams &P, float *smem, in
 }
 
 template <int G0, int N>
-__device__ __forceinline__ void dispatch(int g, const StreamParams &P, float *smem, int gl, int seg, int lane, int pix, bool live)
+__device__ __forceinline__ void dispatch(int g, const StreamParams &P, float *smem, const int *wtab, int gl, int seg, int lane, int pix, bool live)
 {
     if constexpr (N == 1) {
-        run_group<G0>(P, smem, gl, seg, lane, pix, live);
+        run_group<G0>(P, smem, wtab, gl, seg, lane, pix, live);
     } else {
-        if (g < G0 + N / 2) dispatch<G0, N / 2>(g, P, smem, gl, seg, lane, pix, live);
-        else dispatch<G0 + N / 2, N - N / 2>(g, P, smem, gl, seg, lane, pix, live);
+        if (g < G0 + N / 2) dispatch<G0, N / 2>(g, P, smem, wtab, gl, seg, lane, pix, live);
+        else dispatch<G0 + N / 2, N - N / 2>(g, P, smem, wtab, gl, seg, lane, pix, live);
     }
 }
 
@@ -810,10 +822,13 @@ extern "C" __global__ void __launch_bounds__(sk::kThreads, MINB) k_stream(const 
     const bool live = pix < NPIX;
     if (!live) pix = NPIX - 1;
     const int g = blockIdx.y * GPC + gl; // DM group of this warp; NSUPER*GPC groups exist (the last may be padding)
+    __shared__ int s_wtab[NW];
+    for (int i = threadIdx.x; i < NW; i += sk::kThreads) s_wtab[i] = W_TAB[i];
+    __syncthreads();
 #if DHIST
-    sk::run_group<0>(P, smem, gl, seg, lane, pix, live, g * KK);
+    sk::run_group<0>(P, smem, s_wtab, gl, seg, lane, pix, live, g * KK);
 #else
-    sk::dispatch<0, NSUPER * GPC>(g, P, smem, gl, seg, lane, pix, live);
+    sk::dispatch<0, NSUPER * GPC>(g, P, smem, s_wtab, gl, seg, lane, pix, live);
 #endif
 }
 
