@@ -35,7 +35,7 @@ from paper_2510_18136_b200 import workloads as W  # noqa: E402
 CHUNK_DURATION_MS = 25 * W.TSAMP_S * 1e3  # 3355 ms (25 samples x 134 ms)
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed `ncu --set full`
 # capture named beside it (a constant of that capture, not measured in this run)
-NCU_TRAFFIC = {"c2": (2.507e9, "profiles/r02_k_stream_c2_details.csv / r02.md (dram__bytes_read 2.334 GB + write 0.174 GB, round-2 capture of the history-mode kernel)")}
+NCU_TRAFFIC = {"c2": (2.668e9, "profiles/r02_k_stream_c2_details.csv / r02.md (dram__bytes_read 2.493 GB + write 0.174 GB, round-2 capture of the history-mode kernel)")}
 
 
 # ---------------------------------------------------------------------------- helpers
