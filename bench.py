@@ -455,7 +455,9 @@ def run_cuda_arm(args, rank, world, local):
                         "re-reading the ring, not that the kernel beats HBM -- frac_read is its own DRAM rate over the peak",
                 "read_bytes": read_bytes, "read_bytes_note": read_note,
                 "achieved_read": read_bytes / (dominant_ms * 1e-3) / 1e9,
-                "frac_read": read_bytes / (dominant_ms * 1e-3) / 1e9 / hbm_peak}
+                "frac_read": read_bytes / (dominant_ms * 1e-3) / 1e9 / hbm_peak,
+                # the capture's DRAM bytes over this run's kernel time: how close the kernel is to the bandwidth roofline of what it moves
+                "frac_traffic": (traffic / (dominant_ms * 1e-3) / 1e9 / hbm_peak) if traffic else None}
     else:
         roof = offline_roofline(wl, bench, dominant_ms, ms_per_step, hbm_peak, peak_src, onchip, sm_max)
     line = {
